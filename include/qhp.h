@@ -1,0 +1,160 @@
+/*
+ * qhp.h -- C ABI of the B200-native Quantum-HP hot path (RPMD + adQTB MD step).
+ *
+ * What it computes is defined by /root/reference/PAPER.md (arXiv 2212.03137); citations are
+ * "PAPER.md:<line>, Eq. n".  Readings of passages where the paper is silent (G1..G23) are in
+ * DESIGN.md "Readings".  The force field (flexible 3-site water: harmonic bonds/angles,
+ * Lennard-Jones, damped-shifted-force Coulomb) is BASELINE.json configs[0], not the paper's.
+ *
+ * Conventions
+ *   units     Angstrom, ps, amu, kcal/mol, K, e.  Momenta amu*A/ps; forces kcal/mol/A.
+ *   layouts   x_beads, p_beads, f_beads: fp64 [P][n_atoms][3], bead-major ("replicas",
+ *             PAPER.md:32).  Momenta are bead momenta p_i = sqrt(P) sum_n T_in Pm_n (the map of
+ *             Eq. 4).  Internally the state lives in scaled normal modes (Eq. 1-4).
+ *   pointers  every pointer in qhp_topology / qhp_thermostat is a HOST pointer, deep-copied by
+ *             qhp_create.  Array arguments of all other calls are DEVICE pointers on the device
+ *             of the stream given to qhp_create, unless the function name ends in _host, in
+ *             which case they are HOST pointers and the call copies synchronously.
+ *   ownership the caller owns every buffer it passes; the library owns the qhp_system and all
+ *             device state behind it until qhp_destroy.
+ *   async     all calls enqueue work on the stream given at create time and return without
+ *             synchronising, except qhp_create / qhp_destroy / qhp_set_state (builds the first
+ *             neighbour list and sizes its storage) / *_host calls / qhp_check.
+ *   errors    every call returns 0 (QHP_OK) or a negative qhp_status; text in qhp_last_error.
+ *             No exceptions, no abort, no stdout.  There is no CPU fallback of any call.
+ */
+#ifndef QHP_H
+#define QHP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  QHP_OK = 0,
+  QHP_EINVAL = -1,  /* bad argument (P < 1, unsupported P, P_contract not in [1,P], box < 2 r_cut, ...) */
+  QHP_ENOMEM = -2,  /* device or host allocation failed */
+  QHP_ECUDA = -3,   /* CUDA error (sticky); text via qhp_last_error */
+  QHP_ESTATE = -4   /* call out of order (step before set_state, adQTB restart inside a segment,
+                       neighbour-list capacity overflow detected at a synchronising call) */
+} qhp_status;
+
+typedef struct qhp_system qhp_system; /* opaque */
+
+/* Topology and force field (BASELINE.json configs[0]; V = V_s + V_f, Eq. 18).
+ * Molecules must be contiguous in atom index (mol[] non-decreasing), bonds and angles join
+ * atoms of one molecule, and a molecule has at most QHP_MAX_MOL_ATOMS atoms.  Atom pairs of the
+ * same molecule are excluded from V_s. */
+#define QHP_MAX_MOL_ATOMS 48
+typedef struct {
+  int32_t n_atoms, n_types, n_bonds, n_angles;
+  const int32_t *type;     /* [n_atoms] atom type z (adQTB averages per type)     */
+  const int32_t *mol;      /* [n_atoms] molecule id                                            */
+  const double *mass;      /* [n_types] amu                                                    */
+  const double *charge;    /* [n_types] e                                                      */
+  const double *lj_eps;    /* [n_types] kcal/mol (0 => no LJ); Lorentz-Berthelot mixing        */
+  const double *lj_sigma;  /* [n_types] Angstrom                                               */
+  const double *tether_k;  /* [n_types] or NULL: extra V_f term 1/2 k |x|^2 (harmonic pins)    */
+  const int32_t *bond_idx; /* [n_bonds][2]                                                     */
+  const double *bond_k;    /* [n_bonds] kcal/mol/A^2, V = 1/2 k (r - r0)^2                     */
+  const double *bond_r0;   /* [n_bonds] A                                                      */
+  const int32_t *angle_idx;/* [n_angles][3] (end, centre, end)                                 */
+  const double *angle_k;   /* [n_angles] kcal/mol/rad^2, V = 1/2 k (th - th0)^2                */
+  const double *angle_th0; /* [n_angles] rad                                                   */
+  double box[3];           /* orthorhombic periodic box, A; every edge >= 2 r_cut              */
+  double r_cut;            /* V_s cutoff (LJ shifted, DSF Coulomb), A                          */
+  double dsf_alpha;        /* DSF damping, 1/A                                                 */
+  double skin;             /* neighbour-list skin, A: r_list = r_cut + skin     */
+} qhp_topology;
+
+typedef enum { QHP_THERMO_NONE = 0, QHP_THERMO_PILE = 1, QHP_THERMO_ADQTB = 2 } qhp_thermo_kind;
+
+typedef struct {
+  int32_t kind;          /* qhp_thermo_kind                                                     */
+  double gamma0;         /* 1/ps: PILE centroid friction / adQTB gamma_0 (Eq. 12)*/
+  uint64_t seed;         /* Philox4x32-10 key                                                   */
+  int32_t n_seg;         /* adQTB: steps per noise segment, power of two >= 8    */
+  double a_gamma;        /* adQTB: adaptation rate A (Eq. 23, reading G15); 0 = no adaptation   */
+  double gamma_min_frac; /* adQTB: gamma_z >= gamma_min_frac * gamma0; 0.01      */
+  int32_t classical;     /* adQTB: != 0 replaces Theta(omega) by kB T (test hook, hbar -> 0)    */
+} qhp_thermostat;
+
+/* Create a system of P beads with V_s evaluated on P_contract <= P contracted beads (ring-polymer
+ * contraction, Eq. 20) and V_f on all P.  dt in ps, T in K.  Supported P:
+ * 1,2,3,4,5,6,8,12,16,24,32.  adQTB requires P = 1.  cuda_stream is a cudaStream_t (NULL = legacy default
+ * stream). */
+int qhp_create(const qhp_topology *top, int P, int P_contract, double dt_ps, double T_K,
+               const qhp_thermostat *thermo, void *cuda_stream, qhp_system **out);
+int qhp_destroy(qhp_system *sys);
+
+/* Load bead positions / momenta (device [P][n_atoms][3]); transforms to normal modes (Eq. 4
+ * inverted), builds cells + neighbour list on the centroids and evaluates the
+ * forces.  step0 = index of the next step: Philox streams are functions of (seed, atom, mode,
+ * step), so get_state -> set_state resumes bit-identically.  adQTB: step0 % n_seg == 0. */
+int qhp_set_state(qhp_system *sys, const double *x_beads, const double *p_beads, int64_t step0);
+int qhp_get_state(qhp_system *sys, double *x_beads, double *p_beads, int64_t *step_host);
+int qhp_set_state_host(qhp_system *sys, const double *x_beads, const double *p_beads, int64_t step0);
+int qhp_get_state_host(qhp_system *sys, double *x_beads, double *p_beads, int64_t *step_host);
+
+/* Advance nsteps of B A O A B in normal modes (Eq. 16-17): exact free
+ * ring-polymer A blocks, PILE/TRPMD O block gamma_n = max(gamma0, omega_n) (l.146), or, for
+ * adQTB, classical BAOAB whose O block carries the coloured force (Eq. 12-14, l.199), with the
+ * segment generation (l.203-209) and gamma_z(omega) adaptation (Eq. 21-23, l.248) at segment
+ * boundaries. */
+int qhp_step(qhp_system *sys, int64_t nsteps);
+
+/* Bead-space forces at the current positions, device [P][n_atoms][3]:
+ * G_i = -grad V_f(x_i) + (P/P') sum_j C_ji (-grad V_s(xc_j))  (Eq. 10-11 and chain rule on Eq. 20). */
+int qhp_forces(qhp_system *sys, double *f_beads);
+
+/* out[0] = K_CV centroid-virial kinetic energy, out[1] = U = (1/P) sum V_f + (1/P') sum V_s
+ * (Eq. 6, Eq. 20), out[2] = K_nm = sum Pm^2/2m, out[3] = T_inst = 2 K_nm/(3 N P kB);
+ * kcal/mol, K.  n_out <= 4 values are written. */
+int qhp_observables(qhp_system *sys, double *out, int n_out);
+int qhp_observables_host(qhp_system *sys, double *out, int n_out);
+
+/* ---- parity hooks (device pointers) ---------------------------------------------------- */
+/* Canonical neighbour objects of the CURRENT centroids (rebuilds them): cell_of[n_atoms],
+ * order[n_atoms] (atoms stably sorted by cell), cell_start[ncell+1], n_cells3[3].
+ * Any pointer may be NULL. */
+int qhp_neighbor_lists(qhp_system *sys, int32_t *cell_of, int32_t *order, int32_t *cell_start,
+                       int32_t *n_cells3);
+/* Pair list of the current centroids in ATOM indices: count[n_atoms] and, if nbr != NULL,
+ * nbr[start(i) .. start(i)+count[i]) with start = exclusive prefix sum of count; entries are
+ * all j != i of another molecule with centroid distance^2 < r_list^2 (order unspecified).
+ * total_host (HOST pointer, may be NULL) receives sum(count) (synchronises). */
+int qhp_pair_list(qhp_system *sys, int32_t *count, int32_t *nbr, int64_t cap, int64_t *total_host);
+/* Contracted bead positions xc [P_contract][n_atoms][3] (Eq. 20) of the current state. */
+int qhp_contracted(qhp_system *sys, double *xc);
+/* adQTB: gamma_z(omega_j) [n_types][n_seg+1]; coloured force segment Fc and recorded
+ * velocities vseg, both [3 n_atoms][n_seg] (NULL to skip). */
+int qhp_adqtb_gamma(qhp_system *sys, double *gamma);
+int qhp_adqtb_segment(qhp_system *sys, double *Fc, double *vseg);
+/* Counters for measurement: out_host[0] = neighbour-list rebuilds so far, [1] = list entries,
+ * [2] = pair-bead interactions inside r_cut at the current positions (full list, both
+ * directions), [3] = list capacity, [4] = kernels launched so far, [5] = overflow flag.
+ * n_out <= 6.  HOST pointer; synchronises. */
+int qhp_counters(qhp_system *sys, int64_t *out_host, int n_out);
+/* Synchronise the stream and report sticky CUDA / overflow errors. */
+int qhp_check(qhp_system *sys);
+const char *qhp_last_error(const qhp_system *sys); /* sys may be NULL: last create error */
+
+/* ---- stand-alone primitives of the path (device pointers), for parity tests ------------- */
+/* Philox4x32-10 words and the three Box-Muller normals of counter (atom0+i, mode | tag<<24,
+ * step) for i < n: words [n][4] uint32 (may be NULL), z [n][3] (may be NULL). */
+int qhp_philox_normals(uint64_t seed, uint32_t atom0, uint32_t mode, uint32_t tag, uint64_t step,
+                       int64_t n, uint32_t *words, double *z, void *cuda_stream);
+/* Batched complex fp64 FFT of length n (power of two, 8..8192) by the shared-memory Stockham
+ * kernel used for the QTB noise and spectra: data [batch][n][2], in place; sign = -1 forward,
+ * +1 inverse (unnormalised). */
+int qhp_fft_c2c(double *data, int n, int64_t batch, int sign, void *cuda_stream);
+/* DFMA throughput probe: runs iters fused multiply-adds per thread on grid x block threads and
+ * writes one double per thread to sink (device, grid*block doubles). */
+int qhp_dfma_probe(double *sink, int grid, int block, int64_t iters, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QHP_H */

@@ -335,21 +335,24 @@ def qtb_colored_direct(top: Topology, n_seg: int, seed: int, seg: int, h_types: 
     return Fc
 
 
-def qtb_colored_fft(top: Topology, n_seg: int, seed: int, seg: int, h_types: np.ndarray):
+def qtb_colored_fft(top: Topology, n_seg: int, seed: int, seg: int, h_types: np.ndarray, atoms=None):
     """Same definition as `qtb_colored_direct`, the sum evaluated with numpy.fft as the DFT
-    (linear convolution through zero-padding to 4 n_seg).  Validated against the direct sum."""
+    (linear convolution through zero-padding to 4 n_seg).  Validated against the direct sum.
+    `atoms` (optional): only these atoms, rows returned in that order ([3 len(atoms)][n_seg]) --
+    lets the tests sample boxes too large to do in full."""
     nfft = 4 * n_seg
-    Fc = np.empty((3 * top.n_atoms, n_seg))
+    atom_list = range(top.n_atoms) if atoms is None else [int(a) for a in atoms]
+    Fc = np.empty((3 * len(atom_list), n_seg))
     hk = []
     for z in range(top.n_types):
         buf = np.zeros(nfft)
         buf[:2 * n_seg] = h_types[z]          # buf[m] = h[m - n_seg]
         hk.append(np.fft.rfft(buf))
-    for a in range(top.n_atoms):
+    for row, a in enumerate(atom_list):
         r = qtb_white(seed, a, seg * n_seg, 3 * n_seg)
         y = np.fft.irfft(np.fft.rfft(r, n=nfft, axis=1) * hk[top.type[a]][None, :], n=nfft, axis=1)
         # y[m] = sum_k h[k] r[m - n_seg - k]  =>  F_c[n] = y[n + 2 n_seg]
-        Fc[3 * a:3 * a + 3] = y[:, 2 * n_seg:3 * n_seg]
+        Fc[3 * row:3 * row + 3] = y[:, 2 * n_seg:3 * n_seg]
     return Fc
 
 

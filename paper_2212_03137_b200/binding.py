@@ -1,0 +1,302 @@
+"""ctypes binding of include/qhp.h.  Marshals torch CUDA tensors / numpy topology arrays into the
+C ABI; holds no arithmetic of the method.  Fails loudly if libqhp.so is missing."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libqhp.so")
+
+QHP_THERMO_NONE, QHP_THERMO_PILE, QHP_THERMO_ADQTB = 0, 1, 2
+_STATUS = {0: "QHP_OK", -1: "QHP_EINVAL", -2: "QHP_ENOMEM", -3: "QHP_ECUDA", -4: "QHP_ESTATE"}
+
+# every symbol include/qhp.h declares (tests check that the library exports them all)
+SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_state", "qhp_get_state", "qhp_set_state_host",
+           "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
+           "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma",
+           "qhp_adqtb_segment", "qhp_counters", "qhp_check", "qhp_last_error", "qhp_philox_normals",
+           "qhp_fft_c2c", "qhp_dfma_probe"]
+
+
+class QhpError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"{_STATUS.get(code, code)}: {text}")
+        self.code = code
+
+
+class _Topology(C.Structure):
+    _fields_ = [("n_atoms", C.c_int32), ("n_types", C.c_int32), ("n_bonds", C.c_int32), ("n_angles", C.c_int32),
+                ("type", C.c_void_p), ("mol", C.c_void_p), ("mass", C.c_void_p), ("charge", C.c_void_p),
+                ("lj_eps", C.c_void_p), ("lj_sigma", C.c_void_p), ("tether_k", C.c_void_p),
+                ("bond_idx", C.c_void_p), ("bond_k", C.c_void_p), ("bond_r0", C.c_void_p),
+                ("angle_idx", C.c_void_p), ("angle_k", C.c_void_p), ("angle_th0", C.c_void_p),
+                ("box", C.c_double * 3), ("r_cut", C.c_double), ("dsf_alpha", C.c_double), ("skin", C.c_double)]
+
+
+class _Thermostat(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("gamma0", C.c_double), ("seed", C.c_uint64), ("n_seg", C.c_int32),
+                ("a_gamma", C.c_double), ("gamma_min_frac", C.c_double), ("classical", C.c_int32)]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def lib():
+    """Load libqhp.so (built by `python -m paper_2212_03137_b200.build`).  No fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_2212_03137_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(_LIB_PATH)
+        vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int, C.c_double
+        L.qhp_create.argtypes = [C.POINTER(_Topology), i32, i32, dbl, dbl, C.POINTER(_Thermostat), vp, C.POINTER(vp)]
+        L.qhp_destroy.argtypes = [vp]
+        L.qhp_set_state.argtypes = [vp, vp, vp, i64]
+        L.qhp_get_state.argtypes = [vp, vp, vp, C.POINTER(i64)]
+        L.qhp_set_state_host.argtypes = [vp, vp, vp, i64]
+        L.qhp_get_state_host.argtypes = [vp, vp, vp, C.POINTER(i64)]
+        L.qhp_step.argtypes = [vp, i64]
+        L.qhp_forces.argtypes = [vp, vp]
+        L.qhp_observables.argtypes = [vp, vp, i32]
+        L.qhp_observables_host.argtypes = [vp, vp, i32]
+        L.qhp_neighbor_lists.argtypes = [vp, vp, vp, vp, vp]
+        L.qhp_pair_list.argtypes = [vp, vp, vp, i64, C.POINTER(i64)]
+        L.qhp_contracted.argtypes = [vp, vp]
+        L.qhp_adqtb_gamma.argtypes = [vp, vp]
+        L.qhp_adqtb_segment.argtypes = [vp, vp, vp]
+        L.qhp_counters.argtypes = [vp, C.POINTER(i64), i32]
+        L.qhp_check.argtypes = [vp]
+        L.qhp_last_error.argtypes = [vp]
+        L.qhp_last_error.restype = C.c_char_p
+        L.qhp_philox_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, i64, vp, vp, vp]
+        L.qhp_fft_c2c.argtypes = [vp, i32, i64, i32, vp]
+        L.qhp_dfma_probe.argtypes = [vp, i32, i32, i64, vp]
+        for name in SYMBOLS:
+            if name != "qhp_last_error":
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2212_03137_b200 needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream_ptr(stream=None):
+    torch = _torch()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _chk_dev(t, dtype, numel=None, name="tensor"):
+    torch = _torch()
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor of dtype {dtype}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name}: expected {numel} elements, got {t.numel()}")
+
+
+class System:
+    """One qhp_system.  Methods mirror the C ABI (qhp_<name>)."""
+
+    def __init__(self, top: dict, P: int, P_contract: int, dt_ps: float, T_K: float, thermostat: str | int = "none",
+                 gamma0: float = 1.0, seed: int = 0, n_seg: int = 0, a_gamma: float = 0.0,
+                 gamma_min_frac: float = 0.01, classical: bool = False, stream=None):
+        torch = _torch()
+        self._h = C.c_void_p()
+        self._L = lib()
+        kinds = {"none": 0, "pile": 1, "adqtb": 2}
+        kind = kinds[thermostat] if isinstance(thermostat, str) else int(thermostat)
+        keep = {}
+        t = _Topology()
+        t.n_atoms, t.n_types = int(top["n_atoms"]), int(top["n_types"])
+        t.n_bonds, t.n_angles = int(top["n_bonds"]), int(top["n_angles"])
+        for k in ("type", "mol", "bond_idx", "angle_idx"):
+            keep[k] = np.ascontiguousarray(top[k], dtype=np.int32)
+            setattr(t, k, keep[k].ctypes.data_as(C.c_void_p))
+        for k in ("mass", "charge", "lj_eps", "lj_sigma", "bond_k", "bond_r0", "angle_k", "angle_th0"):
+            keep[k] = np.ascontiguousarray(top[k], dtype=np.float64)
+            setattr(t, k, keep[k].ctypes.data_as(C.c_void_p))
+        if top.get("tether_k") is not None:
+            keep["tether_k"] = np.ascontiguousarray(top["tether_k"], dtype=np.float64)
+            t.tether_k = keep["tether_k"].ctypes.data_as(C.c_void_p)
+        for d in range(3):
+            t.box[d] = float(top["box"][d])
+        t.r_cut, t.dsf_alpha, t.skin = float(top["r_cut"]), float(top["dsf_alpha"]), float(top["skin"])
+        th = _Thermostat(kind, float(gamma0), int(seed), int(n_seg), float(a_gamma), float(gamma_min_frac),
+                         int(bool(classical)))
+        self.stream = torch.cuda.current_stream() if stream is None else stream
+        self.device = torch.device("cuda", torch.cuda.current_device())
+        self.N, self.P, self.Pc, self.n_types, self.n_seg = t.n_atoms, int(P), int(P_contract), t.n_types, int(n_seg)
+        rc = self._L.qhp_create(C.byref(t), int(P), int(P_contract), float(dt_ps), float(T_K), C.byref(th),
+                                C.c_void_p(self.stream.cuda_stream), C.byref(self._h))
+        if rc != 0:
+            raise QhpError(rc, (self._L.qhp_last_error(None) or b"").decode())
+
+    # -- helpers
+    def _ok(self, rc):
+        if rc != 0:
+            raise QhpError(rc, (self._L.qhp_last_error(self._h) or b"").decode())
+
+    def _empty(self, shape, dtype=None):
+        torch = _torch()
+        return torch.empty(shape, dtype=dtype or torch.float64, device=self.device)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            self._L.qhp_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- C ABI
+    def set_state(self, x_beads, p_beads, step0: int = 0):
+        torch = _torch()
+        n = self.P * self.N * 3
+        _chk_dev(x_beads, torch.float64, n, "x_beads")
+        _chk_dev(p_beads, torch.float64, n, "p_beads")
+        self._ok(self._L.qhp_set_state(self._h, _ptr(x_beads), _ptr(p_beads), int(step0)))
+
+    def get_state(self):
+        x, p = self._empty((self.P, self.N, 3)), self._empty((self.P, self.N, 3))
+        step = C.c_int64()
+        self._ok(self._L.qhp_get_state(self._h, _ptr(x), _ptr(p), C.byref(step)))
+        return x, p, step.value
+
+    def set_state_host(self, x_host, p_host, step0: int = 0):
+        """x_host, p_host: CPU tensors / numpy arrays [P][N][3] fp64 (pinned for full PCIe speed)."""
+        self._ok(self._L.qhp_set_state_host(self._h, _host_ptr(x_host, self.P * self.N * 3),
+                                            _host_ptr(p_host, self.P * self.N * 3), int(step0)))
+
+    def get_state_host(self, x_host, p_host):
+        step = C.c_int64()
+        self._ok(self._L.qhp_get_state_host(self._h, _host_ptr(x_host, self.P * self.N * 3),
+                                            _host_ptr(p_host, self.P * self.N * 3), C.byref(step)))
+        return step.value
+
+    def step(self, nsteps: int):
+        self._ok(self._L.qhp_step(self._h, int(nsteps)))
+
+    def forces(self):
+        f = self._empty((self.P, self.N, 3))
+        self._ok(self._L.qhp_forces(self._h, _ptr(f)))
+        return f
+
+    def observables(self):
+        out = self._empty((4,))
+        self._ok(self._L.qhp_observables(self._h, _ptr(out), 4))
+        return out
+
+    def observables_host(self) -> np.ndarray:
+        out = np.empty(4)
+        self._ok(self._L.qhp_observables_host(self._h, out.ctypes.data_as(C.c_void_p), 4))
+        return out
+
+    def neighbor_lists(self):
+        torch = _torch()
+        nc = self._empty((3,), torch.int32)
+        cell_of, order = self._empty((self.N,), torch.int32), self._empty((self.N,), torch.int32)
+        # ncell is not known before the call: size cell_start generously from the box, then trim
+        self._ok(self._L.qhp_neighbor_lists(self._h, _ptr(cell_of), _ptr(order), None, _ptr(nc)))
+        ncell = int(nc.prod().item())
+        cell_start = self._empty((ncell + 1,), torch.int32)
+        self._ok(self._L.qhp_neighbor_lists(self._h, None, None, _ptr(cell_start), None))
+        return nc, cell_of, order, cell_start
+
+    def pair_list(self):
+        torch = _torch()
+        count = self._empty((self.N,), torch.int32)
+        total = C.c_int64()
+        self._ok(self._L.qhp_pair_list(self._h, _ptr(count), None, 0, C.byref(total)))
+        nbr = self._empty((max(total.value, 1),), torch.int32)
+        self._ok(self._L.qhp_pair_list(self._h, _ptr(count), _ptr(nbr), total.value, C.byref(total)))
+        return count, nbr[:total.value]
+
+    def contracted(self):
+        xc = self._empty((self.Pc, self.N, 3))
+        self._ok(self._L.qhp_contracted(self._h, _ptr(xc)))
+        return xc
+
+    def adqtb_gamma(self):
+        g = self._empty((self.n_types, self.n_seg + 1))
+        self._ok(self._L.qhp_adqtb_gamma(self._h, _ptr(g)))
+        return g
+
+    def adqtb_segment(self, want_fc=True, want_v=True):
+        Fc = self._empty((3 * self.N, self.n_seg)) if want_fc else None
+        v = self._empty((3 * self.N, self.n_seg)) if want_v else None
+        self._ok(self._L.qhp_adqtb_segment(self._h, _ptr(Fc), _ptr(v)))
+        return Fc, v
+
+    def counters(self) -> dict:
+        out = (C.c_int64 * 6)()
+        self._ok(self._L.qhp_counters(self._h, out, 6))
+        keys = ["rebuilds", "list_entries", "pair_beads_in_cutoff", "list_capacity", "launches", "overflow"]
+        return dict(zip(keys, [int(v) for v in out]))
+
+    def check(self):
+        self._ok(self._L.qhp_check(self._h))
+
+
+def _host_ptr(a, numel):
+    import torch
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != torch.float64 or not a.is_contiguous() or a.numel() != numel:
+            raise TypeError("expected a contiguous CPU float64 tensor of the state's size")
+        return C.c_void_p(a.data_ptr())
+    a = np.asarray(a)
+    if a.dtype != np.float64 or not a.flags.c_contiguous or a.size != numel:
+        raise TypeError("expected a contiguous float64 array of the state's size")
+    return a.ctypes.data_as(C.c_void_p)
+
+
+# ---- stand-alone primitives --------------------------------------------------------------------
+def qhp_philox_normals(seed: int, atom0: int, mode: int, tag: int, step: int, n: int, stream=None):
+    torch = _torch()
+    words = torch.empty((n, 4), dtype=torch.int32, device="cuda")
+    z = torch.empty((n, 3), dtype=torch.float64, device="cuda")
+    rc = lib().qhp_philox_normals(int(seed), int(atom0), int(mode), int(tag), int(step), int(n), _ptr(words), _ptr(z),
+                                  _stream_ptr(stream))
+    if rc:
+        raise QhpError(rc, "qhp_philox_normals")
+    return words, z
+
+
+def qhp_fft_c2c(data, sign: int, stream=None):
+    """data: CUDA tensor [batch][n][2] fp64 (or complex128 [batch][n]); transformed in place."""
+    torch = _torch()
+    view = torch.view_as_real(data) if data.is_complex() else data
+    _chk_dev(view, torch.float64, None, "data")
+    batch, n = view.shape[0], view.shape[1]
+    rc = lib().qhp_fft_c2c(_ptr(view), int(n), int(batch), int(sign), _stream_ptr(stream))
+    if rc:
+        raise QhpError(rc, "qhp_fft_c2c")
+    return data
+
+
+def qhp_dfma_probe(grid: int, block: int, iters: int, stream=None):
+    torch = _torch()
+    sink = torch.empty(grid * block, dtype=torch.float64, device="cuda")
+    rc = lib().qhp_dfma_probe(_ptr(sink), int(grid), int(block), int(iters), _stream_ptr(stream))
+    if rc:
+        raise QhpError(rc, "qhp_dfma_probe")
+    return sink

@@ -1,0 +1,267 @@
+// cells.cu -- neighbour objects on the centroids (lists are
+// "computed with respect to centroid positions" and shared by all beads).
+//
+// Canonical integer objects (bit-exact contract with the oracle):
+//   nc[d]      = max(1, floor(L_d / r_list)),  r_list = r_cut + skin
+//   cell_of[a] : s = c*(1/L); s -= floor(s); q = min((int)(s*nc), nc-1); cell = (qx*ncy + qy)*ncz + qz
+//   order[]    = atoms stably sorted by cell (ties by atom index); cell_start[] = prefix sums
+//   pair set   = {(i,j): mol_i != mol_j, d2 < r_list^2}, dx = fma(-L, rint(dx*(1/L)), dx),
+//                d2 = fma(dz,dz, fma(dy,dy, dx*dx))
+// All floating-point steps that decide an integer use explicit _rn intrinsics so that nvcc's FMA
+// contraction cannot change them.
+//
+// The list is a fixed-stride table nbr[slot][k] in SLOT space (slot = position in `order`), built by
+// one warp per slot scanning the 27-cell stencil with ballot compaction (deterministic order).
+// Every kernel of the rebuild chain returns at once unless the integrator's list-validity statistic
+// max |xc - cref|^2 reached (skin/2)^2, so the chain can be enqueued every step without a host sync.
+#include "qhp_internal.cuh"
+
+struct CellArgs {
+  int N, nc[3], ncell;
+  double box[3], inv_box[3], rl2;
+  const unsigned long long *flag;
+  double thresh2;
+};
+
+__device__ __forceinline__ bool cells_skip(const CellArgs &a) {
+  return a.flag && __longlong_as_double((long long)*a.flag) < a.thresh2;
+}
+
+__global__ void k_cells_assign(const CellArgs a, const double *__restrict__ Q0, int32_t *cell_of, int32_t *cell_count) {
+  if (cells_skip(a)) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= a.N) return;
+  int q[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    double s = __dmul_rn(Q0[3LL * i + d], a.inv_box[d]);
+    s = __dsub_rn(s, floor(s));
+    int v = (int)__dmul_rn(s, (double)a.nc[d]);
+    if (v > a.nc[d] - 1) v = a.nc[d] - 1;
+    q[d] = v;
+  }
+  const int cell = (q[0] * a.nc[1] + q[1]) * a.nc[2] + q[2];
+  cell_of[i] = cell;
+  atomicAdd(&cell_count[cell], 1);
+}
+
+// single-CTA exclusive scan of n ints -> out[0..n]; optionally copies to out2 and zeroes `in`
+__global__ void k_scan_excl(const CellArgs a, int32_t *in, int32_t *out, int32_t *out2, int n, int zero_in) {
+  if (cells_skip(a)) return;
+  __shared__ int32_t part[1024];
+  const int t = threadIdx.x, nt = blockDim.x;
+  const int len = (n + nt - 1) / nt;
+  const int b = min(n, t * len), e = min(n, b + len);
+  int32_t s = 0;
+  for (int k = b; k < e; ++k) s += in[k];
+  part[t] = s;
+  __syncthreads();
+  // Hillis-Steele inclusive scan over the per-thread sums
+  for (int o = 1; o < nt; o <<= 1) {
+    int32_t v = (t >= o) ? part[t - o] : 0;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  int32_t run = part[t] - s;
+  for (int k = b; k < e; ++k) {
+    const int32_t v = in[k];
+    out[k] = run;
+    if (out2) out2[k] = run;
+    if (zero_in) in[k] = 0;
+    run += v;
+  }
+  if (t == nt - 1) { out[n] = part[t]; if (out2) out2[n] = part[t]; }
+}
+
+__global__ void k_cells_fill(const CellArgs a, const int32_t *__restrict__ cell_of, int32_t *cursor, int32_t *tmp) {
+  if (cells_skip(a)) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= a.N) return;
+  tmp[atomicAdd(&cursor[cell_of[i]], 1)] = i;
+}
+
+// stable order inside each cell: slot = cell_start + #{members with a smaller atom index}
+__global__ void k_cells_rank(const CellArgs a, const int32_t *__restrict__ cell_of, const int32_t *__restrict__ cell_start,
+                             const int32_t *__restrict__ tmp, int32_t *order, int32_t *rank) {
+  if (cells_skip(a)) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= a.N) return;
+  const int c = cell_of[i], b = cell_start[c], e = cell_start[c + 1];
+  int cnt = 0;
+  for (int k = b; k < e; ++k) cnt += (tmp[k] < i);
+  order[b + cnt] = i;
+  rank[i] = b + cnt;
+}
+
+// one warp per slot; nbr == NULL: count only
+__global__ void __launch_bounds__(256) k_list_build(const CellArgs a, const double *__restrict__ cent4,
+                                                    const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
+                                                    const int32_t *__restrict__ cell_start, int32_t *nbr,
+                                                    int32_t *nbr_count, long long stride, long long *counters) {
+  if (cells_skip(a)) return;
+  const int lane = threadIdx.x & 31;
+  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i >= a.N) return;
+  if (i == 0 && lane == 0 && nbr) counters[0] += 1;
+  const double4 ci = reinterpret_cast<const double4 *>(cent4)[i];
+  const long long mi = __double_as_longlong(ci.w);
+  const int cell = cell_of[order[i]];
+  const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
+  const int nox = min(a.nc[0], 3), noy = min(a.nc[1], 3), noz = min(a.nc[2], 3);
+  const int sx = a.nc[0] >= 3 ? -1 : 0, sy = a.nc[1] >= 3 ? -1 : 0, sz = a.nc[2] >= 3 ? -1 : 0;
+  const unsigned lt = (1u << lane) - 1u;
+  int cnt = 0;
+  for (int ox = 0; ox < nox; ++ox)
+    for (int oy = 0; oy < noy; ++oy)
+      for (int oz = 0; oz < noz; ++oz) {
+        const int qx = (cx + sx + ox + a.nc[0]) % a.nc[0], qy = (cy + sy + oy + a.nc[1]) % a.nc[1],
+                  qz = (cz + sz + oz + a.nc[2]) % a.nc[2];
+        const int c2 = (qx * a.nc[1] + qy) * a.nc[2] + qz;
+        const int b = cell_start[c2], e = cell_start[c2 + 1];
+        for (int k0 = b; k0 < e; k0 += 32) {
+          const int k = k0 + lane;
+          bool hit = false;
+          if (k < e && k != i) {
+            const double4 cj = reinterpret_cast<const double4 *>(cent4)[k];
+            if (__double_as_longlong(cj.w) != mi) {
+              double dx = __dsub_rn(ci.x, cj.x), dy = __dsub_rn(ci.y, cj.y), dz = __dsub_rn(ci.z, cj.z);
+              dx = __fma_rn(-a.box[0], rint(__dmul_rn(dx, a.inv_box[0])), dx);
+              dy = __fma_rn(-a.box[1], rint(__dmul_rn(dy, a.inv_box[1])), dy);
+              dz = __fma_rn(-a.box[2], rint(__dmul_rn(dz, a.inv_box[2])), dz);
+              const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+              hit = d2 < a.rl2;
+            }
+          }
+          const unsigned mask = __ballot_sync(0xffffffffu, hit);
+          if (hit && nbr) {
+            const int pos = cnt + __popc(mask & lt);
+            if (pos < stride) nbr[i * stride + pos] = k;
+          }
+          cnt += __popc(mask);
+        }
+      }
+  if (lane == 0) {
+    if (nbr) {
+      nbr_count[i] = (int)min((long long)cnt, stride);
+      if (cnt > stride) counters[1] = 1;
+    } else {
+      nbr_count[i] = cnt;
+    }
+    atomicMax((unsigned long long *)&counters[2], (unsigned long long)cnt);
+  }
+}
+
+// ---- export in atom indices (parity hook) ---------------------------------------------------------
+__global__ void k_export_count(int N, const int32_t *__restrict__ order, const int32_t *__restrict__ nbr_count, int32_t *count) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < N) count[order[i]] = nbr_count[i];
+}
+__global__ void k_export_fill(int N, const int32_t *__restrict__ order, const int32_t *__restrict__ nbr_count,
+                              const int32_t *__restrict__ nbr, long long stride, const int32_t *__restrict__ start,
+                              int32_t *out, long long cap) {
+  const int lane = threadIdx.x & 31;
+  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i >= N) return;
+  const int a = order[i], n = nbr_count[i];
+  const long long s0 = start[a];
+  for (int k = lane; k < n; k += 32)
+    if (s0 + k < cap) out[s0 + k] = order[nbr[i * stride + k]];
+}
+
+static CellArgs cell_args(qhp_system *s, bool force) {
+  CellArgs a{};
+  a.N = s->N; a.ncell = s->ncell;
+  const double rl = s->r_cut + s->skin;
+  for (int d = 0; d < 3; ++d) { a.nc[d] = s->nc[d]; a.box[d] = s->box[d]; a.inv_box[d] = s->inv_box[d]; }
+  a.rl2 = rl * rl;
+  a.flag = force ? nullptr : &s->d2max[s->flag_idx];
+  const double th = 0.5 * s->skin;
+  a.thresh2 = th * th;
+  return a;
+}
+
+// cells (assign, scan, fill, rank) of the current centroids Q_0
+static int cells_only(qhp_system *s, const CellArgs &a) {
+  const int tb = 256, grid = (s->N + tb - 1) / tb;
+  k_cells_assign<<<grid, tb, 0, s->stream>>>(a, s->Q, s->cell_of, s->cell_count);
+  QHP_LAUNCH_OK(s);
+  k_scan_excl<<<1, 1024, 0, s->stream>>>(a, s->cell_count, s->cell_start, s->cell_cursor, s->ncell, 1);
+  QHP_LAUNCH_OK(s);
+  k_cells_fill<<<grid, tb, 0, s->stream>>>(a, s->cell_of, s->cell_cursor, s->cell_tmp);
+  QHP_LAUNCH_OK(s);
+  k_cells_rank<<<grid, tb, 0, s->stream>>>(a, s->cell_of, s->cell_start, s->cell_tmp, s->order, s->rank);
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+static int list_build(qhp_system *s, const CellArgs &a, bool count_only) {
+  const int tb = 256;
+  const long long threads = 32LL * s->N;
+  const unsigned grid = (unsigned)((threads + tb - 1) / tb);
+  k_list_build<<<grid, tb, 0, s->stream>>>(a, s->cent4, s->cell_of, s->order, s->cell_start,
+                                          count_only ? nullptr : s->nbr, s->nbr_count, s->nbr_stride,
+                                          (long long *)s->counters);
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+int qhp_cells_rebuild(qhp_system *s, bool force) {
+  const CellArgs a = cell_args(s, force);
+  int rc = cells_only(s, a);
+  if (rc) return rc;
+  rc = qhp_nm_contract(s, true, force);
+  if (rc) return rc;
+  if (force) {
+    // synchronising call sites only: size the fixed-stride table from a counting pass
+    QHP_CUDA_OK(s, cudaMemsetAsync(&s->counters[2], 0, sizeof(int64_t), s->stream));
+    rc = list_build(s, a, true);
+    if (rc) return rc;
+    int64_t mx = 0;
+    QHP_CUDA_OK(s, cudaMemcpyAsync(&mx, &s->counters[2], sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
+    QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
+    if (s->nbr == nullptr || mx + 8 > s->nbr_stride) {
+      int64_t stride = (int64_t)((double)mx * 1.4) + 32;
+      stride = (stride + 3) / 4 * 4;
+      if (stride > s->N) stride = (s->N + 3) / 4 * 4;
+      if (stride < 4) stride = 4;
+      if (s->nbr) cudaFree(s->nbr);
+      s->nbr = nullptr;
+      s->nbr_stride = stride;
+      if (cudaMalloc(&s->nbr, sizeof(int32_t) * (size_t)stride * (size_t)s->N) != cudaSuccess) {
+        s->err = "neighbour table allocation failed";
+        s->nbr = nullptr;
+        return QHP_ENOMEM;
+      }
+    }
+  }
+  return list_build(s, a, false);
+}
+
+int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, int64_t *total_host) {
+  const int tb = 256;
+  int32_t *start = nullptr;
+  QHP_CUDA_OK(s, cudaMalloc(&start, sizeof(int32_t) * ((size_t)s->N + 1)));
+  int32_t *cnt = count;
+  int32_t *cnt_own = nullptr;
+  if (!cnt) { QHP_CUDA_OK(s, cudaMalloc(&cnt_own, sizeof(int32_t) * (size_t)s->N)); cnt = cnt_own; }
+  k_export_count<<<(s->N + tb - 1) / tb, tb, 0, s->stream>>>(s->N, s->order, s->nbr_count, cnt);
+  QHP_LAUNCH_OK(s);
+  CellArgs a{};
+  a.flag = nullptr;
+  k_scan_excl<<<1, 1024, 0, s->stream>>>(a, cnt, start, nullptr, s->N, 0);
+  QHP_LAUNCH_OK(s);
+  if (nbr) {
+    const long long threads = 32LL * s->N;
+    k_export_fill<<<(unsigned)((threads + tb - 1) / tb), tb, 0, s->stream>>>(s->N, s->order, s->nbr_count, s->nbr,
+                                                                           s->nbr_stride, start, nbr, cap);
+    QHP_LAUNCH_OK(s);
+  }
+  int32_t tot = 0;
+  QHP_CUDA_OK(s, cudaMemcpyAsync(&tot, start + s->N, sizeof(int32_t), cudaMemcpyDeviceToHost, s->stream));
+  QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
+  if (total_host) *total_host = tot;
+  cudaFree(start);
+  if (cnt_own) cudaFree(cnt_own);
+  return QHP_OK;
+}

@@ -1,0 +1,594 @@
+// nm_kernels.cu -- normal-mode side of the hot path:
+//   * bead <-> normal-mode transforms (Eq. 4),
+//   * the fused integrator pass: [B] B A O A in normal modes (Eq. 16-17) with the
+//     intramolecular forces V_f on all P beads, their projection on the modes
+//     (Eq. 10-11), the expansion of the contracted slow forces and the contraction of the new
+//     positions (Eq. 20) -- one read and one write of Q and Pm per step,
+//   * bead-space force output (O7) and observables (Eq. 6, O8).
+//
+// Layout: Q, Pm are [P][3N] (mode-major, DOF contiguous).  One CTA = one tile of whole
+// molecules; thread t of the CTA owns DOF 3*a0 + t of the tile for all P modes (coalesced
+// 8-byte accesses for every mode), and the tile's bead positions / forces are exchanged through
+// two shared-memory tiles [P][TD] so that the bonded terms can be evaluated per (molecule, bead).
+// The P x P transform matrix is a kernel parameter, i.e. lives in the constant bank: with the
+// loops fully unrolled every FMA takes its coefficient as an immediate constant operand.
+#include "qhp_internal.cuh"
+#include "philox.cuh"
+
+template <int P> struct NmTab { double T[P * P]; };   // T[i*P+n], Eq. 2 eigenvectors
+
+struct IntArgs {
+  int N, Pc, nt, TD;
+  long long ND;
+  const qhp_tile *tiles;
+  double *Q, *Pm;
+  const double *coef;
+  const int32_t *type, *molid, *mol_atom_start, *mol_bond_start, *mol_angle_start;
+  const int32_t *bond_idx, *angle_idx;
+  const double *bond_k, *bond_r0, *angle_k, *angle_th0, *tether_k, *mass;
+  const int32_t *rank;
+  double *pos4;
+  const double *Fs;
+  const double *cref;
+  unsigned long long *d2max;
+  int kick_prev, do_step;
+  long long step;
+  unsigned long long seed;
+  double hA, hdt;
+  // adQTB (P = 1)
+  const double *Fc;
+  double *vseg;
+  int n_seg, n_loc;
+  double qa, qbA;
+  // outputs of the auxiliary kernels
+  double *G;      // bead forces
+  double *part;   // per-CTA partial sums [n_tiles][4]
+  double kT;
+};
+
+// ---------------------------------------------------------------------------------------------
+// V_f of one (molecule, bead): harmonic bonds, harmonic angles, optional tether (BASELINE.json
+// configs[0]; oracle O3).  x, f point at the bead's row of the shared tiles; a0 = first atom of
+// the tile.  The calling thread owns this (molecule, bead), so plain read-modify-write is safe.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double bonded_molecule(const IntArgs &a, int m, int a0,
+                                                  const double *__restrict__ x, double *f) {
+  double U = 0.0;
+  const int b0 = a.mol_bond_start[m], b1 = a.mol_bond_start[m + 1];
+  for (int b = b0; b < b1; ++b) {
+    const int i = 3 * (a.bond_idx[2 * b] - a0), j = 3 * (a.bond_idx[2 * b + 1] - a0);
+    const double dx = x[i] - x[j], dy = x[i + 1] - x[j + 1], dz = x[i + 2] - x[j + 2];
+    const double r = sqrt(dx * dx + dy * dy + dz * dz);
+    const double k = a.bond_k[b], dr = r - a.bond_r0[b];
+    U += 0.5 * k * dr * dr;
+    const double g = -k * dr / r;
+    f[i] += g * dx; f[i + 1] += g * dy; f[i + 2] += g * dz;
+    f[j] -= g * dx; f[j + 1] -= g * dy; f[j + 2] -= g * dz;
+  }
+  const int g0 = a.mol_angle_start[m], g1 = a.mol_angle_start[m + 1];
+  for (int g = g0; g < g1; ++g) {
+    const int i = 3 * (a.angle_idx[3 * g] - a0), j = 3 * (a.angle_idx[3 * g + 1] - a0),
+              k = 3 * (a.angle_idx[3 * g + 2] - a0);                       // j = centre
+    const double ux = x[i] - x[j], uy = x[i + 1] - x[j + 1], uz = x[i + 2] - x[j + 2];
+    const double vx = x[k] - x[j], vy = x[k + 1] - x[j + 1], vz = x[k + 2] - x[j + 2];
+    const double ru = sqrt(ux * ux + uy * uy + uz * uz), rv = sqrt(vx * vx + vy * vy + vz * vz);
+    const double iruv = 1.0 / (ru * rv);
+    double cs = (ux * vx + uy * vy + uz * vz) * iruv;
+    cs = fmin(1.0, fmax(-1.0, cs));
+    const double th = acos(cs), dth = th - a.angle_th0[g], ka = a.angle_k[g];
+    U += 0.5 * ka * dth * dth;
+    const double sn = sqrt(1.0 - cs * cs);
+    const double gg = ka * dth / sn;
+    const double cu = cs / (ru * ru), cv = cs / (rv * rv);
+    const double fix = gg * (vx * iruv - cu * ux), fiy = gg * (vy * iruv - cu * uy), fiz = gg * (vz * iruv - cu * uz);
+    const double fkx = gg * (ux * iruv - cv * vx), fky = gg * (uy * iruv - cv * vy), fkz = gg * (uz * iruv - cv * vz);
+    f[i] += fix; f[i + 1] += fiy; f[i + 2] += fiz;
+    f[k] += fkx; f[k + 1] += fky; f[k + 2] += fkz;
+    f[j] -= fix + fkx; f[j + 1] -= fiy + fky; f[j + 2] -= fiz + fkz;
+  }
+  if (a.tether_k) {
+    const int s0 = a.mol_atom_start[m], s1 = a.mol_atom_start[m + 1];
+    for (int at = s0; at < s1; ++at) {
+      const double k = a.tether_k[a.type[at]];
+      const int i = 3 * (at - a0);
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const double xx = x[i + c];
+        U += 0.5 * k * xx * xx;
+        f[i + c] -= k * xx;
+      }
+    }
+  }
+  return U;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Common front end of the integrator / force / observable kernels for one tile:
+//   Qr[n]  <- Q_n of this thread's DOF,
+//   x_i = sqrt(P) sum_n T_in Q_n (Eq. 4) -> shared tile, V_f forces per (molecule, bead),
+//   fr[n] <- (1/sqrt P) sum_i T_in F^f_i (Eq. 10-11) + (1/sqrt P') sum_j T'_jn Fc_j  (n < P').
+// Returns this thread's share of sum_i V_f(x_i).
+// ---------------------------------------------------------------------------------------------
+template <int P>
+__device__ __forceinline__ double tile_forces(const IntArgs &a, const NmTab<P> &tab, const NmTab<P> &ctab,
+                                              const qhp_tile tl, double *xt, double *ft,
+                                              bool active, long long dof, int atom, int c,
+                                              double (&Qr)[P], double (&fr)[P]) {
+  const int t = threadIdx.x, TD = a.TD;
+  const double sp = sqrt((double)P);
+  if (active) {
+#pragma unroll
+    for (int n = 0; n < P; ++n) Qr[n] = a.Q[n * a.ND + dof];
+#pragma unroll
+    for (int i = 0; i < P; ++i) {
+      double s = 0.0;
+#pragma unroll
+      for (int n = 0; n < P; ++n) s += tab.T[i * P + n] * Qr[n];
+      xt[i * TD + t] = sp * s;
+      ft[i * TD + t] = 0.0;
+    }
+  }
+  __syncthreads();
+  double U = 0.0;
+  const int nm = tl.m1 - tl.m0;
+  for (int w = t; w < nm * P; w += blockDim.x) {
+    const int m = tl.m0 + w % nm, bead = w / nm;
+    U += bonded_molecule(a, m, tl.a0, xt + bead * TD, ft + bead * TD);
+  }
+  __syncthreads();
+  if (active) {
+#pragma unroll
+    for (int n = 0; n < P; ++n) fr[n] = 0.0;
+#pragma unroll
+    for (int i = 0; i < P; ++i) {
+      const double Fi = ft[i * TD + t];
+#pragma unroll
+      for (int n = 0; n < P; ++n) fr[n] += tab.T[i * P + n] * Fi;
+    }
+    const double isp = 1.0 / sp;
+#pragma unroll
+    for (int n = 0; n < P; ++n) fr[n] *= isp;
+    // slow forces of the contracted beads, chain rule on Eq. 20
+    const int Pc = a.Pc;
+    const double ispc = 1.0 / sqrt((double)Pc);
+    const long long slot = a.rank[atom];
+    for (int j = 0; j < Pc; ++j) {
+      const double Fj = a.Fs[((long long)j * a.N + slot) * 3 + c] * ispc;
+#pragma unroll
+      for (int n = 0; n < P; ++n)
+        if (n < Pc) fr[n] += ctab.T[j * Pc + n] * Fj;
+    }
+  }
+  return U;
+}
+
+__device__ __forceinline__ double block_max(double v, double *scratch) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+  __syncthreads();
+  if (l == 0) scratch[w] = v;
+  __syncthreads();
+  v = (l < nw) ? scratch[l] : 0.0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// deterministic block sum (fixed tree)
+__device__ __forceinline__ double block_sum(double v, double *scratch) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+  __syncthreads();
+  if (l == 0) scratch[w] = v;
+  __syncthreads();
+  v = (l < nw) ? scratch[l] : 0.0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused integrator pass.  THERMO: 0 none, 1 PILE/TRPMD, 2 adQTB (P = 1).
+//   kick_prev: apply the final B(dt/2) of the previous step (forces at the current Q);
+//   do_step  : B(dt/2) A(dt/2) O(dt) A(dt/2) of this step, then write the contracted positions
+//              of the new Q (slot order) and the list-validity statistic max |xc - cref|^2.
+// ---------------------------------------------------------------------------------------------
+template <int P, int THERMO>
+__global__ void __launch_bounds__(288) k_integrate(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab) {
+  extern __shared__ double sm[];
+  const int TD = a.TD, t = threadIdx.x;
+  double *xt = sm, *ft = sm + P * TD, *sc = ft + P * TD, *scratch = sc + a.nt * P * QHP_NCOEF;
+  const qhp_tile tl = a.tiles[blockIdx.x];
+  const int nd = 3 * (tl.a1 - tl.a0);
+  const bool active = t < nd;
+  const long long dof = 3LL * tl.a0 + t;
+  const int atom = tl.a0 + t / 3, c = t % 3;
+  for (int k = t; k < a.nt * P * QHP_NCOEF; k += blockDim.x) sc[k] = a.coef[k];
+  if (blockIdx.x == 0 && t == 0 && a.do_step) a.d2max[(a.step + 1) & 1] = 0ull;
+
+  double Qr[P], fr[P];
+  tile_forces<P>(a, tab, ctab, tl, xt, ft, active, dof, atom, c, Qr, fr);   // syncs inside
+
+  double d2 = 0.0;
+  if (active) {
+    const int ty = a.type[atom];
+    const double m = a.mass[ty];
+    const double *cf = sc + ty * P * QHP_NCOEF;
+#pragma unroll
+    for (int n = 0; n < P; ++n) {
+      double q = Qr[n];
+      double p = a.Pm[n * a.ND + dof];
+      if (a.kick_prev) p += a.hA * fr[n];
+      if (a.do_step) {
+        p += a.hA * fr[n];
+        const double cs = cf[n * QHP_NCOEF + 0], s1 = cf[n * QHP_NCOEF + 1], s2 = cf[n * QHP_NCOEF + 2];
+        // A(dt/2): centroid translation / exact free ring-polymer rotation
+        if (n == 0) q += a.hdt * p / m;
+        else { const double qn = cs * q + s1 * p; p = s2 * q + cs * p; q = qn; }
+        // O(dt)
+        if (THERMO == 1) {
+          const double z = qhp_normal_comp(a.seed, (uint32_t)atom, (uint32_t)n, QHP_TAG_PILE,
+                                           (uint64_t)a.step, c);
+          p = cf[n * QHP_NCOEF + 3] * p + cf[n * QHP_NCOEF + 4] * z;
+        } else if (THERMO == 2) {
+          // classical BAOAB carrying the coloured force (Eq. 12, l.199; readings G14, G16)
+          const long long k = dof * a.n_seg + a.n_loc;
+          const double pn = a.qa * p + a.qbA * a.Fc[k];
+          a.vseg[k] = (p + pn) / (2.0 * m);
+          p = pn;
+        }
+        // A(dt/2)
+        if (n == 0) q += a.hdt * p / m;
+        else { const double qn = cs * q + s1 * p; p = s2 * q + cs * p; q = qn; }
+        a.Q[n * a.ND + dof] = q;
+        Qr[n] = q;
+      }
+      a.Pm[n * a.ND + dof] = p;
+    }
+    if (a.do_step) {
+      // contraction of the new positions (Eq. 20) into slot order + list-validity statistic
+      const int Pc = a.Pc;
+      const double spc = sqrt((double)Pc);
+      const long long slot = a.rank[atom];
+      const double cr = a.cref[dof];
+      for (int j = 0; j < Pc; ++j) {
+        double s = 0.0;
+#pragma unroll
+        for (int n = 0; n < P; ++n)
+          if (n < Pc) s += ctab.T[j * Pc + n] * Qr[n];
+        const double xc = spc * s;
+        a.pos4[((long long)j * a.N + slot) * 4 + c] = xc;
+        const double dd = xc - cr;
+        d2 = fmax(d2, dd * dd);
+      }
+    }
+  }
+  if (a.do_step) {
+    // per-atom |xc - cref|^2 <= sum over components of the per-component maxima over beads
+    __syncthreads();
+    xt[t] = d2;
+    __syncthreads();
+    double v = 0.0;
+    if (active && c == 0) v = xt[t] + xt[t + 1] + xt[t + 2];
+    v = block_max(v, scratch);
+    if (t == 0) atomicMax(&a.d2max[a.step & 1], (unsigned long long)__double_as_longlong(v));
+  }
+}
+
+// bead-space forces G_i = sqrt(P) sum_n T_in f_n (O7)
+template <int P>
+__global__ void __launch_bounds__(288) k_bead_forces(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab) {
+  extern __shared__ double sm[];
+  const int TD = a.TD, t = threadIdx.x;
+  double *xt = sm, *ft = sm + P * TD;
+  const qhp_tile tl = a.tiles[blockIdx.x];
+  const bool active = t < 3 * (tl.a1 - tl.a0);
+  const long long dof = 3LL * tl.a0 + t;
+  const int atom = tl.a0 + t / 3, c = t % 3;
+  double Qr[P], fr[P];
+  tile_forces<P>(a, tab, ctab, tl, xt, ft, active, dof, atom, c, Qr, fr);
+  if (active) {
+    const double sp = sqrt((double)P);
+#pragma unroll
+    for (int i = 0; i < P; ++i) {
+      double s = 0.0;
+#pragma unroll
+      for (int n = 0; n < P; ++n) s += tab.T[i * P + n] * fr[n];
+      a.G[i * a.ND + dof] = sp * s;
+    }
+  }
+}
+
+// partial sums of the observables (O8): part[cta] = {sum_{n>0} Q_n f_n, sum_i V_f(x_i), sum Pm^2/2m}
+template <int P>
+__global__ void __launch_bounds__(288) k_observe(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab) {
+  extern __shared__ double sm[];
+  const int TD = a.TD, t = threadIdx.x;
+  double *xt = sm, *ft = sm + P * TD, *scratch = ft + P * TD + a.nt * P * QHP_NCOEF;
+  const qhp_tile tl = a.tiles[blockIdx.x];
+  const bool active = t < 3 * (tl.a1 - tl.a0);
+  const long long dof = 3LL * tl.a0 + t;
+  const int atom = tl.a0 + t / 3, c = t % 3;
+  double Qr[P], fr[P];
+  double U = tile_forces<P>(a, tab, ctab, tl, xt, ft, active, dof, atom, c, Qr, fr);
+  double vir = 0.0, kin = 0.0;
+  if (active) {
+    const double m = a.mass[a.type[atom]];
+#pragma unroll
+    for (int n = 0; n < P; ++n) {
+      if (n > 0) vir += Qr[n] * fr[n];
+      const double p = a.Pm[n * a.ND + dof];
+      kin += p * p / (2.0 * m);
+    }
+  }
+  vir = block_sum(vir, scratch);
+  U = block_sum(U, scratch);
+  kin = block_sum(kin, scratch);
+  if (t == 0) {
+    a.part[4 * blockIdx.x + 0] = vir;
+    a.part[4 * blockIdx.x + 1] = U;
+    a.part[4 * blockIdx.x + 2] = kin;
+    a.part[4 * blockIdx.x + 3] = 0.0;
+  }
+}
+
+// final fixed-order reduction of the per-CTA partial sums and of the pair-energy partials
+__global__ void k_observe_final(const double *part, int n_part, const double *pair_part, int n_pair,
+                                double *obs, int N, int P, int Pc, double kT) {
+  __shared__ double scratch[32];
+  double v = 0, u = 0, k = 0, us = 0;
+  for (int i = threadIdx.x; i < n_part; i += blockDim.x) { v += part[4 * i]; u += part[4 * i + 1]; k += part[4 * i + 2]; }
+  for (int i = threadIdx.x; i < n_pair; i += blockDim.x) us += pair_part[i];
+  v = block_sum(v, scratch); u = block_sum(u, scratch); k = block_sum(k, scratch); us = block_sum(us, scratch);
+  if (threadIdx.x == 0) {
+    obs[0] = 1.5 * N * kT - 0.5 * v;
+    obs[1] = u / P + 0.5 * us / Pc;       // full list: every pair energy was counted twice
+    obs[2] = k / QHP_ACC;
+    obs[3] = 2.0 * obs[2] / (3.0 * (double)N * (double)P * QHP_KB);
+  }
+}
+
+// ---- plain per-DOF transforms (no tile) ---------------------------------------------------------
+template <int P>
+__global__ void k_to_modes(const double *__restrict__ xb, const double *__restrict__ pb, double *Q, double *Pm,
+                           long long ND, const NmTab<P> tab) {
+  const long long d = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (d >= ND) return;
+  const double sp = sqrt((double)P);
+  for (int which = 0; which < 2; ++which) {
+    const double *in = which ? pb : xb;
+    double *out = which ? Pm : Q;
+    if (!in) continue;
+    double v[P];
+#pragma unroll
+    for (int i = 0; i < P; ++i) v[i] = in[i * ND + d];
+#pragma unroll
+    for (int n = 0; n < P; ++n) {
+      double s = 0.0;
+#pragma unroll
+      for (int i = 0; i < P; ++i) s += tab.T[i * P + n] * v[i];
+      out[n * ND + d] = s / sp;
+    }
+  }
+}
+
+template <int P>
+__global__ void k_to_beads(const double *__restrict__ Q, const double *__restrict__ Pm, double *xb, double *pb,
+                           long long ND, const NmTab<P> tab) {
+  const long long d = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (d >= ND) return;
+  const double sp = sqrt((double)P);
+  for (int which = 0; which < 2; ++which) {
+    const double *in = which ? Pm : Q;
+    double *out = which ? pb : xb;
+    if (!out) continue;
+    double v[P];
+#pragma unroll
+    for (int n = 0; n < P; ++n) v[n] = in[n * ND + d];
+#pragma unroll
+    for (int i = 0; i < P; ++i) {
+      double s = 0.0;
+#pragma unroll
+      for (int n = 0; n < P; ++n) s += tab.T[i * P + n] * v[n];
+      out[i * ND + d] = sp * s;
+    }
+  }
+}
+
+// Contraction (Eq. 20) of the current Q.  mode 0: write pos4 in slot order (after a list rebuild
+// also cent4 = sorted centroids + molecule id, cref = centroids in atom order, pos4.w = type);
+// mode 1: write xc_out [Pc][N][3] in atom order (parity hook).
+// `need` (may be NULL): device flag words; the kernel returns at once unless forced or the
+// list-validity statistic exceeds the threshold.
+__global__ void k_contract(const double *__restrict__ Q, int N, int Pc, const double *__restrict__ Tc,
+                           const int32_t *__restrict__ rank, const int32_t *__restrict__ type,
+                           const int32_t *__restrict__ molid, double *pos4, double *cent4, double *cref,
+                           double *xc_out, int mode, const unsigned long long *d2max, double thresh2) {
+  if (d2max && __longlong_as_double((long long)*d2max) < thresh2) return;
+  const long long ND = 3LL * N;
+  const long long d = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (d >= ND) return;
+  const int atom = (int)(d / 3), c = (int)(d % 3);
+  const double spc = sqrt((double)Pc);
+  const long long slot = rank ? rank[atom] : atom;
+  for (int j = 0; j < Pc; ++j) {
+    double s = 0.0;
+    for (int n = 0; n < Pc; ++n) s += Tc[j * Pc + n] * Q[n * ND + d];
+    const double xc = spc * s;
+    if (mode == 0) {
+      pos4[((long long)j * N + slot) * 4 + c] = xc;
+      if (c == 0) reinterpret_cast<long long *>(pos4)[((long long)j * N + slot) * 4 + 3] = type[atom];
+    } else {
+      xc_out[(long long)j * ND + d] = xc;
+    }
+  }
+  if (mode == 0 && cent4) {
+    const double q0 = Q[d];
+    cent4[slot * 4 + c] = q0;
+    if (c == 0) reinterpret_cast<long long *>(cent4)[slot * 4 + 3] = molid[atom];
+    cref[d] = q0;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+template <int P> static NmTab<P> make_tab(const std::vector<double> &T, int n) {
+  NmTab<P> t;
+  for (int k = 0; k < P * P; ++k) t.T[k] = 0.0;
+  for (int k = 0; k < n * n; ++k) t.T[k] = T[k];   // dense [n][n] with stride n (n = P or Pc)
+  return t;
+}
+
+static IntArgs make_args(qhp_system *s) {
+  IntArgs a{};
+  a.N = s->N; a.Pc = s->Pc; a.nt = s->nt; a.TD = s->tile_threads; a.ND = 3LL * s->N;
+  a.tiles = s->dt_.tiles; a.Q = s->Q; a.Pm = s->Pm; a.coef = s->coef;
+  a.type = s->dt_.type; a.molid = s->dt_.molid; a.mol_atom_start = s->dt_.mol_atom_start;
+  a.mol_bond_start = s->dt_.mol_bond_start; a.mol_angle_start = s->dt_.mol_angle_start;
+  a.bond_idx = s->dt_.bond_idx; a.angle_idx = s->dt_.angle_idx;
+  a.bond_k = s->dt_.bond_k; a.bond_r0 = s->dt_.bond_r0; a.angle_k = s->dt_.angle_k; a.angle_th0 = s->dt_.angle_th0;
+  a.tether_k = s->has_tether ? s->dt_.tether_k : nullptr; a.mass = s->dt_.mass;
+  a.rank = s->rank; a.pos4 = s->pos4; a.Fs = s->Fs; a.cref = s->cref; a.d2max = s->d2max;
+  a.seed = s->th.seed; a.hdt = 0.5 * s->dt; a.hA = 0.5 * s->dt * QHP_ACC;
+  a.Fc = s->Fc; a.vseg = s->vseg; a.n_seg = s->n_seg;
+  a.kT = QHP_KB * s->T;
+  return a;
+}
+
+#define QHP_DISPATCH_P(s, FN)                      \
+  switch ((s)->P) {                                \
+    case 1: FN(1); break;                          \
+    case 2: FN(2); break;                          \
+    case 3: FN(3); break;                          \
+    case 4: FN(4); break;                          \
+    case 5: FN(5); break;                          \
+    case 6: FN(6); break;                          \
+    case 8: FN(8); break;                          \
+    case 12: FN(12); break;                        \
+    case 16: FN(16); break;                        \
+    case 24: FN(24); break;                        \
+    case 32: FN(32); break;                        \
+    default: (s)->err = "unsupported P"; return QHP_EINVAL; \
+  }
+
+template <typename K> static cudaError_t set_smem(K kern, size_t bytes) {
+  return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+int qhp_nm_integrate(qhp_system *s, bool kick_prev, bool do_step, int64_t step) {
+  IntArgs a = make_args(s);
+  a.kick_prev = kick_prev; a.do_step = do_step; a.step = step;
+  if (do_step) s->flag_idx = (int)(step & 1);
+  if (s->th.kind == QHP_THERMO_ADQTB) {
+    a.n_loc = (int)(step % s->n_seg);
+    a.qa = exp(-s->th.gamma0 * s->dt);
+    a.qbA = sqrt((1.0 - a.qa * a.qa) * s->dt / (2.0 * s->th.gamma0)) * QHP_ACC;
+  }
+  const size_t smem = s->int_smem;
+  const int thermo = s->th.kind;
+#define FN(PP)                                                                                   \
+  {                                                                                              \
+    NmTab<PP> tab = make_tab<PP>(s->T_P, PP), ctab = make_tab<PP>(s->T_Pc, s->Pc);               \
+    if (thermo == QHP_THERMO_PILE) {                                                             \
+      QHP_CUDA_OK(s, set_smem(k_integrate<PP, 1>, smem));                                        \
+      k_integrate<PP, 1><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, tab, ctab);        \
+    } else if (thermo == QHP_THERMO_ADQTB) {                                                     \
+      QHP_CUDA_OK(s, set_smem(k_integrate<1, 2>, smem));                                         \
+      k_integrate<1, 2><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, make_tab<1>(s->T_P, 1), make_tab<1>(s->T_Pc, 1)); \
+    } else {                                                                                     \
+      QHP_CUDA_OK(s, set_smem(k_integrate<PP, 0>, smem));                                        \
+      k_integrate<PP, 0><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, tab, ctab);        \
+    }                                                                                            \
+  }
+  QHP_DISPATCH_P(s, FN)
+#undef FN
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+int qhp_nm_bead_forces(qhp_system *s, double *G) {
+  IntArgs a = make_args(s);
+  a.G = G;
+  const size_t smem = s->int_smem;
+#define FN(PP)                                                                               \
+  {                                                                                          \
+    QHP_CUDA_OK(s, set_smem(k_bead_forces<PP>, smem));                                       \
+    k_bead_forces<PP><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, make_tab<PP>(s->T_P, PP), make_tab<PP>(s->T_Pc, s->Pc)); \
+  }
+  QHP_DISPATCH_P(s, FN)
+#undef FN
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+int qhp_nm_observe(qhp_system *s) {
+  IntArgs a = make_args(s);
+  a.part = s->red;
+  const size_t smem = s->int_smem;
+#define FN(PP)                                                                               \
+  {                                                                                          \
+    QHP_CUDA_OK(s, set_smem(k_observe<PP>, smem));                                           \
+    k_observe<PP><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, make_tab<PP>(s->T_P, PP), make_tab<PP>(s->T_Pc, s->Pc)); \
+  }
+  QHP_DISPATCH_P(s, FN)
+#undef FN
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+// pair-energy partials live behind the tile partials in s->red: [4*n_tiles .. 4*n_tiles + n_pair)
+int qhp_nm_observe_final(qhp_system *s, int n_pair) {
+  k_observe_final<<<1, 256, 0, s->stream>>>(s->red, s->n_tiles, s->red + 4 * (size_t)s->n_tiles, n_pair, s->obs,
+                                            s->N, s->P, s->Pc, QHP_KB * s->T);
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+int qhp_nm_to_modes(qhp_system *s, const double *xb, const double *pb) {
+  const long long ND = 3LL * s->N;
+  const int tb = 128;
+  const unsigned grid = (unsigned)((ND + tb - 1) / tb);
+#define FN(PP) k_to_modes<PP><<<grid, tb, 0, s->stream>>>(xb, pb, s->Q, s->Pm, ND, make_tab<PP>(s->T_P, PP));
+  QHP_DISPATCH_P(s, FN)
+#undef FN
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+int qhp_nm_to_beads(qhp_system *s, double *xb, double *pb) {
+  const long long ND = 3LL * s->N;
+  const int tb = 128;
+  const unsigned grid = (unsigned)((ND + tb - 1) / tb);
+#define FN(PP) k_to_beads<PP><<<grid, tb, 0, s->stream>>>(s->Q, s->Pm, xb, pb, ND, make_tab<PP>(s->T_P, PP));
+  QHP_DISPATCH_P(s, FN)
+#undef FN
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+int qhp_nm_contract(qhp_system *s, bool rebuild_mode, bool force) {
+  const long long ND = 3LL * s->N;
+  const int tb = 256;
+  const unsigned grid = (unsigned)((ND + tb - 1) / tb);
+  const double th = 0.5 * s->skin;
+  // in rebuild mode the kernel reads the statistic written by the last integrator pass
+  const unsigned long long *flag = (rebuild_mode && !force) ? &s->d2max[s->flag_idx] : nullptr;
+  k_contract<<<grid, tb, 0, s->stream>>>(s->Q, s->N, s->Pc, s->d_Tc, s->rank, s->dt_.type, s->dt_.molid,
+                                        s->pos4, rebuild_mode ? s->cent4 : nullptr, s->cref, nullptr, 0,
+                                        flag, th * th);
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+int qhp_nm_contracted_out(qhp_system *s, double *xc) {
+  const long long ND = 3LL * s->N;
+  const int tb = 256;
+  const unsigned grid = (unsigned)((ND + tb - 1) / tb);
+  k_contract<<<grid, tb, 0, s->stream>>>(s->Q, s->N, s->Pc, s->d_Tc, nullptr, s->dt_.type, s->dt_.molid,
+                                        nullptr, nullptr, nullptr, xc, 1, nullptr, 0.0);
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}

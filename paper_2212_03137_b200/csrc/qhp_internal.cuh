@@ -1,0 +1,153 @@
+// qhp_internal.cuh -- internal declarations of the B200 (sm_100a) Quantum-HP hot path.
+// Shared by the translation units of libqhp.so only; nothing here is used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/qhp.h"
+
+// ---- physical constants (SURVEY.md §8(c) "Units and constants", CODATA 2018) ---------------
+#define QHP_KB 1.987204258640832e-3    // kcal/mol/K
+#define QHP_HBAR 1.5178728306651436e-2 // kcal/mol*ps
+#define QHP_ACC 418.4                  // kcal/mol -> amu A^2/ps^2
+#define QHP_COUL 332.063713            // kcal*A/(mol*e^2)
+#define QHP_PI 3.14159265358979323846
+
+#define QHP_MAX_P 32
+#define QHP_MAX_TYPES 8
+
+// Philox stream tags
+#define QHP_TAG_PILE 3u
+#define QHP_TAG_QTB 4u
+
+// One CTA of the integrator handles one tile = a run of whole molecules.
+struct qhp_tile {
+  int32_t a0, a1; // atoms [a0, a1)
+  int32_t m0, m1; // molecules [m0, m1)
+};
+
+// Per-(type, mode) coefficients of the A and O blocks, laid out [type][mode][QHP_NCOEF].
+#define QHP_NCOEF 6
+// 0: cos(w dt/2)  1: sin/(m w)  2: -m w sin  3: c1 = exp(-g dt)  4: sqrt(m kB T ACC) c2  5: 1/m (unused for n>0)
+
+struct qhp_dev_topology {
+  int32_t *type;   // [N]
+  int32_t *molid;  // [N] dense molecule index 0..n_mol-1
+  int32_t *mol_atom_start;  // [n_mol+1]
+  int32_t *mol_bond_start;  // [n_mol+1]
+  int32_t *mol_angle_start; // [n_mol+1]
+  int32_t *bond_idx;  double *bond_k, *bond_r0;   // sorted by molecule
+  int32_t *angle_idx; double *angle_k, *angle_th0;
+  double *mass;      // [nt]
+  double *tether_k;  // [nt] (zeros when absent)
+  qhp_tile *tiles;   // [n_tiles]
+};
+
+struct qhp_system {
+  // ---- configuration (host) ----
+  int N = 0, nt = 0, n_mol = 0, n_bonds = 0, n_angles = 0;
+  int P = 1, Pc = 1;
+  double dt = 0, T = 0;
+  qhp_thermostat th{};
+  double box[3]{}, inv_box[3]{};
+  double r_cut = 0, alpha = 0, skin = 0;
+  bool has_tether = false;
+  cudaStream_t stream = nullptr;
+  int device = 0;
+  std::string err;
+
+  // ---- host tables ----
+  std::vector<double> mass, charge, lj_eps, lj_sigma;
+  std::vector<double> T_P, T_Pc;      // normal-mode matrices T^(P) [i*P+n], T^(Pc)
+  std::vector<double> omega;          // [P]
+
+  // ---- device state ----
+  qhp_dev_topology dt_{};
+  int n_tiles = 0, tile_atoms = 0, tile_threads = 0;
+  size_t int_smem = 0;
+  double *Q = nullptr, *Pm = nullptr;      // [P][3N] normal modes
+  double *coef = nullptr;                  // [nt][P][QHP_NCOEF]
+  double *d_Tc = nullptr;                  // [Pc][Pc] T^(Pc) on the device
+  int flag_idx = 0;                        // slot of d2max written by the last integrator pass
+  double *pos4 = nullptr;                  // [Pc][N] double4 (x,y,z,type bits) in slot order
+  double *Fs = nullptr;                    // [Pc][N][3] slow forces in slot order
+  double *cent4 = nullptr;                 // [N] double4 (centroid xyz, molecule bits) in slot order
+  double *cref = nullptr;                  // [3N] centroids at the last list build (atom order)
+  double *pair_tab = nullptr;              // [nt*nt][4]: qq, 48 eps s^12, 24 eps s^6, (4 eps s^12, 4 eps s^6, shift) ...
+  // cells and list
+  int nc[3]{1, 1, 1}, ncell = 1;
+  int32_t *cell_of = nullptr, *cell_count = nullptr, *cell_start = nullptr, *cell_cursor = nullptr;
+  int32_t *cell_tmp = nullptr, *order = nullptr, *rank = nullptr;
+  int32_t *nbr = nullptr, *nbr_count = nullptr;
+  int64_t nbr_stride = 0;
+  unsigned long long *d2max = nullptr;     // [2] double bits, max |xc - cref|^2, double-buffered by step parity
+  int64_t *counters = nullptr;             // [8] device: 0 rebuilds, 1 overflow flag, 2 max row count, 3 in-cutoff count
+  double *red = nullptr;                   // scratch for reductions
+  size_t red_len = 0;
+  double *obs = nullptr;                   // [8] device observables
+  double *stage_x = nullptr, *stage_p = nullptr;  // device staging of the *_host calls
+  // adQTB
+  int n_seg = 0;
+  double *gamma = nullptr;   // [nt][n_seg+1]
+  double *Hf = nullptr;      // [nt][n_seg+1] filter H_z
+  double *hk = nullptr;      // [nt][2 n_seg] kernel h_z
+  double *H4 = nullptr;      // [nt][4 n_seg][2] spectrum of the zero-padded shifted kernel
+  double *Fc = nullptr, *vseg = nullptr;  // [3N][n_seg]
+  double *tw = nullptr;      // twiddles exp(-2 pi i k / NT) [NT][2], NT = 4 n_seg
+  int32_t *atoms_by_type = nullptr; // [N]
+  std::vector<int> type_start;     // [nt+1] offsets into atoms_by_type
+  int32_t *spec_cta = nullptr;     // [n_spec_cta][3] (type, begin, end) into atoms_by_type
+  int n_spec_cta = 0;
+  std::vector<int> spec_cta_host;
+  double *spec_part = nullptr;     // [n_spec_cta][2][n_seg+1]
+  double *Cvv = nullptr, *CvF = nullptr; // [nt][n_seg+1]
+  int64_t fc_segment = -1;
+
+  // ---- run state (host) ----
+  bool have_state = false;
+  bool pending_kick = false;   // the final B(dt/2) of the last step has not been applied yet
+  int64_t step = 0;
+  int64_t n_launch = 0;        // kernels launched (for bench gpu_launches)
+};
+
+// ---- launch helpers implemented in the .cu files ----------------------------------------------
+// nm_kernels.cu
+int qhp_nm_to_modes(qhp_system *s, const double *xb, const double *pb);          // beads -> Q, Pm
+int qhp_nm_to_beads(qhp_system *s, double *xb, double *pb);                      // Q, Pm -> beads
+int qhp_nm_integrate(qhp_system *s, bool kick_prev, bool do_step, int64_t step); // fused pass
+int qhp_nm_contract(qhp_system *s, bool rebuild_mode, bool force);               // Q -> pos4 (+ cent4, cref)
+int qhp_nm_bead_forces(qhp_system *s, double *G);                                 // O7
+int qhp_nm_observe(qhp_system *s);                                                // partial sums -> s->red
+int qhp_nm_observe_final(qhp_system *s, int n_pair);                              // s->red -> s->obs
+int qhp_nm_contracted_out(qhp_system *s, double *xc);
+// cells.cu
+int qhp_cells_rebuild(qhp_system *s, bool force);   // early-exits on device unless needed/forced
+int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, int64_t *total_host);
+// pair.cu
+int qhp_pair_forces(qhp_system *s, bool energy);     // pos4 -> Fs (+ U_s, count into obs/counters)
+// qtb.cu
+int qhp_qtb_init(qhp_system *s);
+int qhp_qtb_generate(qhp_system *s, int64_t seg);
+int qhp_qtb_adapt(qhp_system *s);
+int qhp_fft_launch(double *data, int n, int64_t batch, int sign, const double *tw, int tw_n, cudaStream_t st);
+
+#define QHP_CUDA_OK(s, call)                                                          \
+  do {                                                                                \
+    cudaError_t e_ = (call);                                                          \
+    if (e_ != cudaSuccess) {                                                          \
+      (s)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                  \
+      return QHP_ECUDA;                                                               \
+    }                                                                                 \
+  } while (0)
+
+#define QHP_LAUNCH_OK(s)                                                              \
+  do {                                                                                \
+    cudaError_t e_ = cudaGetLastError();                                              \
+    if (e_ != cudaSuccess) {                                                          \
+      (s)->err = std::string("kernel launch: ") + cudaGetErrorString(e_);             \
+      return QHP_ECUDA;                                                               \
+    }                                                                                 \
+    (s)->n_launch++;                                                                  \
+  } while (0)

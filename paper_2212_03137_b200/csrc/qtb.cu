@@ -1,0 +1,395 @@
+// qtb.cu -- adaptive Quantum Thermal Bath:
+//   Q2  white noise regenerated from Philox (nothing stored; the paper keeps 3 N_seg numbers per
+//       DOF),
+//   Q3  filter H_z(omega_j) = sqrt(2 m_z gamma_z(omega_j) Theta(omega_j, beta) / dt)
+//       (Eq. 13-14),
+//   Q4  coloured segment F_c = h_z (*) r by FFT convolution,
+//   Q5  segment spectra |v~|^2 and Re(v~ F~*) (Eq. 21-22),
+//   Q6  per-type averages,
+//   Q7  SIMPLE adaptation with lower bound (Eq. 23; readings G12-G15).
+// The FFT is a hand-written shared-memory Stockham autosort transform (radix 4 with one radix-2
+// pass when log2 n is odd), fp64 complex, one CTA of n/4 threads per transform; each pass stages
+// its butterfly in registers so a single n x 16 B buffer is enough.
+#include "qhp_internal.cuh"
+#include "philox.cuh"
+
+// ---------------------------------------------------------------------------------------------
+// FFT
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
+  return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+
+// tw[m] = exp(-2 pi i m / tw_n); returns exp(sign * 2 pi i * num / den), den | tw_n, 0 <= num < den
+__device__ __forceinline__ double2 twiddle(const double2 *__restrict__ tw, int tw_n, int num, int den, int sign) {
+  double2 w = tw[num * (tw_n / den)];
+  if (sign > 0) w.y = -w.y;
+  return w;
+}
+
+// In-place Stockham FFT of buf[0..n) by blockDim.x >= n/4 threads (all threads of the CTA must call).
+// sign = -1 forward, +1 inverse (unnormalised).  Result in natural order.
+__device__ void fft_smem(double2 *buf, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
+  const int t = threadIdx.x;
+  for (int Ns = 1; Ns < n;) {
+    const int rem = n / Ns;
+    if ((rem & 3) == 0) {
+      const int nb = n >> 2;
+      double2 v0, v1, v2, v3;
+      int j0 = 0;
+      const bool on = t < nb;
+      if (on) {
+        const int k = t & (Ns - 1);
+        v0 = buf[t]; v1 = buf[t + nb]; v2 = buf[t + 2 * nb]; v3 = buf[t + 3 * nb];
+        if (k) {
+          v1 = cmul(v1, twiddle(tw, tw_n, k, Ns * 4, sign));
+          v2 = cmul(v2, twiddle(tw, tw_n, 2 * k, Ns * 4, sign));
+          v3 = cmul(v3, twiddle(tw, tw_n, 3 * k, Ns * 4, sign));
+        }
+        j0 = (t - k) * 4 + k;
+      }
+      __syncthreads();
+      if (on) {
+        const double2 t0 = make_double2(v0.x + v2.x, v0.y + v2.y), t1 = make_double2(v0.x - v2.x, v0.y - v2.y);
+        const double2 t2 = make_double2(v1.x + v3.x, v1.y + v3.y);
+        const double2 d = make_double2(v1.x - v3.x, v1.y - v3.y);
+        // (v1 - v3) * (sign * i)
+        const double2 t3 = (sign < 0) ? make_double2(d.y, -d.x) : make_double2(-d.y, d.x);
+        buf[j0] = make_double2(t0.x + t2.x, t0.y + t2.y);
+        buf[j0 + Ns] = make_double2(t1.x + t3.x, t1.y + t3.y);
+        buf[j0 + 2 * Ns] = make_double2(t0.x - t2.x, t0.y - t2.y);
+        buf[j0 + 3 * Ns] = make_double2(t1.x - t3.x, t1.y - t3.y);
+      }
+      __syncthreads();
+      Ns <<= 2;
+    } else {
+      const int nb = n >> 1;
+      double2 a[2], b[2];
+      int j0[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int j = t + u * (nb >> 1);
+        j0[u] = -1;
+        if (t < (nb >> 1) || (nb == 1 && t == 0 && u == 0)) {
+          const int k = j & (Ns - 1);
+          a[u] = buf[j]; b[u] = buf[j + nb];
+          if (k) b[u] = cmul(b[u], twiddle(tw, tw_n, k, Ns * 2, sign));
+          j0[u] = (j - k) * 2 + k;
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int u = 0; u < 2; ++u)
+        if (j0[u] >= 0) {
+          buf[j0[u]] = make_double2(a[u].x + b[u].x, a[u].y + b[u].y);
+          buf[j0[u] + Ns] = make_double2(a[u].x - b[u].x, a[u].y - b[u].y);
+        }
+      __syncthreads();
+      Ns <<= 1;
+    }
+  }
+}
+
+__global__ void k_twiddle(double2 *tw, int n) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= n) return;
+  double s, c;
+  sincospi(-2.0 * (double)m / (double)n, &s, &c);
+  tw[m] = make_double2(c, s);
+}
+
+__global__ void k_fft_batch(double2 *data, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
+  extern __shared__ double2 fbuf[];
+  double2 *d = data + (long long)blockIdx.x * n;
+  for (int k = threadIdx.x; k < n; k += blockDim.x) fbuf[k] = d[k];
+  __syncthreads();
+  fft_smem(fbuf, n, sign, tw, tw_n);
+  for (int k = threadIdx.x; k < n; k += blockDim.x) d[k] = fbuf[k];
+}
+
+static int fft_threads(int n) { return n / 4 < 32 ? 32 : n / 4; }
+
+int qhp_fft_launch(double *data, int n, int64_t batch, int sign, const double *tw, int tw_n, cudaStream_t st) {
+  const size_t smem = sizeof(double2) * (size_t)n;
+  cudaError_t e = cudaFuncSetAttribute(k_fft_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return QHP_ECUDA;
+  k_fft_batch<<<(unsigned)batch, fft_threads(n), smem, st>>>((double2 *)data, n, sign, (const double2 *)tw, tw_n);
+  return cudaGetLastError() == cudaSuccess ? QHP_OK : QHP_ECUDA;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Q3: filter, kernel and the spectrum used by the convolution
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double qtb_theta(double w, double kT) {   // Eq. 14
+  if (w == 0.0) return kT;
+  const double hw = QHP_HBAR * fabs(w);
+  return 0.5 * hw / tanh(0.5 * hw / kT);
+}
+
+// Hf[z][j] = sqrt(2 (m_z/ACC) gamma_z[j] Theta(omega_j) / dt), omega_j = 2 pi j / (2 n_seg dt)
+__global__ void k_qtb_filter(int nt, int n_seg, double dt, double kT, int classical, const double *__restrict__ mass,
+                             const double *__restrict__ gamma, double *Hf) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nf = n_seg + 1;
+  if (idx >= nt * nf) return;
+  const int z = idx / nf, j = idx % nf;
+  const double w = 2.0 * QHP_PI * j / (2.0 * n_seg * dt);
+  const double th = classical ? kT : qtb_theta(w, kT);
+  Hf[idx] = sqrt(2.0 * (mass[z] / QHP_ACC) * gamma[idx] * th / dt);
+}
+
+// hk[z][k + n_seg] = (1/N_k) sum_j H_ext[j] cos(2 pi j k / N_k), k = -n_seg..n_seg-1 (real, even)
+__global__ void k_qtb_kernel(int nt, int n_seg, const double *__restrict__ Hf, double *hk) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nk = 2 * n_seg;
+  if (idx >= nt * nk) return;
+  const int z = idx / nk, k = idx % nk - n_seg;
+  const double *H = Hf + z * (n_seg + 1);
+  double s = 0.0;
+  for (int j = 0; j < nk; ++j) {
+    const double Hj = (j <= n_seg) ? H[j] : H[nk - j];
+    long long jk = ((long long)j * k) % nk;
+    if (jk < 0) jk += nk;
+    s += Hj * cospi(2.0 * (double)jk / (double)nk);
+  }
+  hk[idx] = s / nk;
+}
+
+// H4[z][q] = sum_{m < 2 n_seg} hk[z][m] exp(-2 pi i q m / (4 n_seg)): spectrum of buf[m] = h[m - n_seg]
+__global__ void k_qtb_spectrum4(int nt, int n_seg, const double *__restrict__ hk, double2 *H4) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nk = 2 * n_seg, nf = 4 * n_seg;
+  if (idx >= nt * nf) return;
+  const int z = idx / nf, q = idx % nf;
+  const double *h = hk + z * nk;
+  double re = 0.0, im = 0.0;
+  for (int m = 0; m < nk; ++m) {
+    const long long qm = ((long long)q * m) % nf;
+    double s, c;
+    sincospi(-2.0 * (double)qm / (double)nf, &s, &c);
+    re += h[m] * c;
+    im += h[m] * s;
+  }
+  H4[idx] = make_double2(re, im);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Q2 + Q4: one CTA per atom.  (x, y) white noise of the atom go through one complex FFT (the
+// kernel h is real, so real and imaginary parts are filtered independently), z through a second.
+//   F_c[dof][n] = sum_k h_z[k] r(dof, seg*n_seg + n - k + n_seg),  n = 0..n_seg-1
+// ---------------------------------------------------------------------------------------------
+__global__ void k_qtb_noise(int n_seg, unsigned long long seed, long long seg, const int32_t *__restrict__ type,
+                            const double2 *__restrict__ H4, const double2 *__restrict__ tw, double *Fc) {
+  extern __shared__ double2 nbuf[];
+  const int nf = 4 * n_seg, nw = 3 * n_seg;
+  double *zb = reinterpret_cast<double *>(nbuf + nf);
+  const int atom = blockIdx.x, t = threadIdx.x;
+  const double2 *Hz = H4 + (long long)type[atom] * nf;
+  for (int m = t; m < nf; m += blockDim.x) {
+    if (m < nw) {
+      double z[3];
+      qhp_normals3(seed, (uint32_t)atom, 0u, QHP_TAG_QTB, (uint64_t)(seg * n_seg + m), z);
+      nbuf[m] = make_double2(z[0], z[1]);
+      zb[m] = z[2];
+    } else {
+      nbuf[m] = make_double2(0.0, 0.0);
+    }
+  }
+  const double inv = 1.0 / (double)nf;
+  for (int pass = 0; pass < 2; ++pass) {
+    __syncthreads();
+    fft_smem(nbuf, nf, -1, tw, nf);
+    for (int q = t; q < nf; q += blockDim.x) nbuf[q] = cmul(nbuf[q], Hz[q]);
+    __syncthreads();
+    fft_smem(nbuf, nf, +1, tw, nf);
+    double *out = Fc + (3LL * atom) * n_seg;
+    for (int n = t; n < n_seg; n += blockDim.x) {
+      const double2 y = nbuf[n + 2 * n_seg];
+      if (pass == 0) { out[n] = y.x * inv; out[n_seg + n] = y.y * inv; }
+      else out[2LL * n_seg + n] = y.x * inv;
+    }
+    if (pass == 0) {
+      __syncthreads();
+      for (int m = t; m < nf; m += blockDim.x) nbuf[m] = make_double2(m < nw ? zb[m] : 0.0, 0.0);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Q5 + Q6: spectra.  One CTA walks a run of atoms of one type; v and F_c of a DOF are the real and
+// imaginary part of one zero-padded N_k-point transform.  Per-CTA sums -> fixed-order reduction.
+// ---------------------------------------------------------------------------------------------
+__global__ void k_qtb_spectra(int n_seg, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
+                              const double *__restrict__ vseg, const double *__restrict__ Fc,
+                              const double2 *__restrict__ tw, int tw_n, double *part) {
+  extern __shared__ double2 sbuf[];
+  const int nk = 2 * n_seg, nf = n_seg + 1, t = threadIdx.x;
+  double *avv = reinterpret_cast<double *>(sbuf + nk), *avf = avv + nf;
+  for (int j = t; j < nf; j += blockDim.x) { avv[j] = 0.0; avf[j] = 0.0; }
+  const int b = cta_tab[3 * blockIdx.x + 1], e = cta_tab[3 * blockIdx.x + 2];
+  for (int ia = b; ia < e; ++ia) {
+    const int atom = atoms[ia];
+    for (int c = 0; c < 3; ++c) {
+      const long long d = 3LL * atom + c;
+      __syncthreads();
+      for (int n = t; n < nk; n += blockDim.x)
+        sbuf[n] = (n < n_seg) ? make_double2(vseg[d * n_seg + n], Fc[d * n_seg + n]) : make_double2(0.0, 0.0);
+      __syncthreads();
+      fft_smem(sbuf, nk, -1, tw, tw_n);
+      for (int j = t; j < nf; j += blockDim.x) {
+        const double2 A = sbuf[j], Zm = sbuf[(nk - j) & (nk - 1)];
+        const double vx = 0.5 * (A.x + Zm.x), vy = 0.5 * (A.y - Zm.y);     // V_j
+        const double px = 0.5 * (A.y + Zm.y), py = -0.5 * (A.x - Zm.x);    // Phi_j
+        avv[j] += vx * vx + vy * vy;
+        avf[j] += vx * px + vy * py;
+      }
+    }
+  }
+  __syncthreads();
+  double *o = part + (long long)blockIdx.x * 2 * nf;
+  for (int j = t; j < nf; j += blockDim.x) { o[j] = avv[j]; o[nf + j] = avf[j]; }
+}
+
+__global__ void k_qtb_reduce(int nt, int n_seg, int n_cta, const int32_t *__restrict__ cta_tab, const double *__restrict__ part,
+                             const double *__restrict__ ndof_type, double dt, double *Cvv, double *CvF) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nf = n_seg + 1;
+  if (idx >= nt * nf) return;
+  const int z = idx / nf, j = idx % nf;
+  double sv = 0.0, sf = 0.0;
+  for (int c = 0; c < n_cta; ++c)
+    if (cta_tab[3 * c] == z) { sv += part[(long long)c * 2 * nf + j]; sf += part[(long long)c * 2 * nf + nf + j]; }
+  const double nd = ndof_type[z];
+  if (nd > 0) {
+    Cvv[idx] = dt / n_seg * sv / nd;
+    CvF[idx] = dt / n_seg * sf / nd;
+  } else { Cvv[idx] = 0.0; CvF[idx] = 0.0; }
+}
+
+// Q7: one CTA per type
+__global__ void k_qtb_adapt(int n_seg, const double *__restrict__ mass, double gamma0, double a_gamma, double gmin_frac,
+                            const double *__restrict__ Cvv, const double *__restrict__ CvF, double *gamma) {
+  __shared__ double scratch[32];
+  __shared__ double nrm_s;
+  const int z = blockIdx.x, nf = n_seg + 1, t = threadIdx.x;
+  const double mz = mass[z] / QHP_ACC;
+  double s = 0.0;
+  for (int j = t; j < nf; j += blockDim.x) {
+    const double dl = mz * gamma[z * nf + j] * Cvv[z * nf + j] - CvF[z * nf + j];
+    s += dl * dl;
+  }
+  // fixed-order block sum
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if ((t & 31) == 0) scratch[t >> 5] = s;
+  __syncthreads();
+  if (t == 0) {
+    double tot = 0.0;
+    for (int k = 0; k < (int)(blockDim.x >> 5); ++k) tot += scratch[k];
+    nrm_s = sqrt(tot);
+  }
+  __syncthreads();
+  const double nrm = nrm_s;
+  if (nrm == 0.0) return;
+  const double gmin = gmin_frac * gamma0;
+  for (int j = t; j < nf; j += blockDim.x) {
+    const double dl = mz * gamma[z * nf + j] * Cvv[z * nf + j] - CvF[z * nf + j];
+    const double g = gamma[z * nf + j] - a_gamma * gamma0 * dl / nrm;
+    gamma[z * nf + j] = g > gmin ? g : gmin;
+  }
+}
+
+__global__ void k_fill(double *p, long long n, double v) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+int qhp_qtb_init(qhp_system *s) {
+  const int ns = s->n_seg, nf = ns + 1, nt = s->nt, N = s->N;
+  const size_t seg_bytes = sizeof(double) * 3 * (size_t)N * ns;
+  QHP_CUDA_OK(s, cudaMalloc(&s->gamma, sizeof(double) * nt * nf));
+  QHP_CUDA_OK(s, cudaMalloc(&s->Hf, sizeof(double) * nt * nf));
+  QHP_CUDA_OK(s, cudaMalloc(&s->hk, sizeof(double) * nt * 2 * ns));
+  QHP_CUDA_OK(s, cudaMalloc(&s->H4, sizeof(double) * 2 * nt * 4 * ns));
+  QHP_CUDA_OK(s, cudaMalloc(&s->Cvv, sizeof(double) * nt * nf));
+  QHP_CUDA_OK(s, cudaMalloc(&s->CvF, sizeof(double) * nt * nf));
+  QHP_CUDA_OK(s, cudaMalloc(&s->tw, sizeof(double) * 2 * 4 * ns));
+  if (cudaMalloc(&s->Fc, seg_bytes) != cudaSuccess || cudaMalloc(&s->vseg, seg_bytes) != cudaSuccess) {
+    s->err = "adQTB segment buffers: out of device memory";
+    return QHP_ENOMEM;
+  }
+  QHP_CUDA_OK(s, cudaMemsetAsync(s->Fc, 0, seg_bytes, s->stream));
+  QHP_CUDA_OK(s, cudaMemsetAsync(s->vseg, 0, seg_bytes, s->stream));
+  k_twiddle<<<(4 * ns + 255) / 256, 256, 0, s->stream>>>((double2 *)s->tw, 4 * ns);
+  QHP_LAUNCH_OK(s);
+  k_fill<<<(nt * nf + 255) / 256, 256, 0, s->stream>>>(s->gamma, (long long)nt * nf, s->th.gamma0);
+  QHP_LAUNCH_OK(s);
+  // atoms grouped by type; spectra CTAs walk runs of <= chunk atoms of one type
+  std::vector<int32_t> by_type, type_host(N);
+  QHP_CUDA_OK(s, cudaMemcpy(type_host.data(), s->dt_.type, sizeof(int32_t) * N, cudaMemcpyDeviceToHost));
+  s->type_start.assign(nt + 1, 0);
+  for (int z = 0; z < nt; ++z) {
+    s->type_start[z] = (int)by_type.size();
+    for (int a = 0; a < N; ++a) if (type_host[a] == z) by_type.push_back(a);
+  }
+  s->type_start[nt] = (int)by_type.size();
+  int chunk = (N + 148 * 4 - 1) / (148 * 4);
+  if (chunk < 1) chunk = 1;
+  std::vector<int32_t> tab;
+  std::vector<double> ndof(nt);
+  for (int z = 0; z < nt; ++z) {
+    ndof[z] = 3.0 * (s->type_start[z + 1] - s->type_start[z]);
+    for (int b = s->type_start[z]; b < s->type_start[z + 1]; b += chunk) {
+      tab.push_back(z); tab.push_back(b); tab.push_back(std::min(b + chunk, s->type_start[z + 1]));
+    }
+  }
+  s->n_spec_cta = (int)tab.size() / 3;
+  QHP_CUDA_OK(s, cudaMalloc(&s->atoms_by_type, sizeof(int32_t) * N));
+  QHP_CUDA_OK(s, cudaMemcpy(s->atoms_by_type, by_type.data(), sizeof(int32_t) * N, cudaMemcpyHostToDevice));
+  QHP_CUDA_OK(s, cudaMalloc(&s->spec_cta, sizeof(int32_t) * tab.size()));
+  QHP_CUDA_OK(s, cudaMemcpy(s->spec_cta, tab.data(), sizeof(int32_t) * tab.size(), cudaMemcpyHostToDevice));
+  QHP_CUDA_OK(s, cudaMalloc(&s->spec_part, sizeof(double) * (size_t)s->n_spec_cta * 2 * nf + sizeof(double) * nt));
+  // per-type DOF counts live behind the partials
+  QHP_CUDA_OK(s, cudaMemcpy(s->spec_part + (size_t)s->n_spec_cta * 2 * nf, ndof.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
+  return QHP_OK;
+}
+
+// Q3 + Q2 + Q4 for segment `seg` with the current gamma_z
+int qhp_qtb_generate(qhp_system *s, int64_t seg) {
+  const int ns = s->n_seg, nf = ns + 1, nt = s->nt;
+  k_qtb_filter<<<(nt * nf + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->dt, QHP_KB * s->T, s->th.classical, s->dt_.mass, s->gamma, s->Hf);
+  QHP_LAUNCH_OK(s);
+  k_qtb_kernel<<<(nt * 2 * ns + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->Hf, s->hk);
+  QHP_LAUNCH_OK(s);
+  k_qtb_spectrum4<<<(nt * 4 * ns + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->hk, (double2 *)s->H4);
+  QHP_LAUNCH_OK(s);
+  const int n4 = 4 * ns;
+  const size_t smem = sizeof(double2) * n4 + sizeof(double) * 3 * ns;
+  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_noise, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_qtb_noise<<<s->N, fft_threads(n4), smem, s->stream>>>(ns, s->th.seed, seg, s->dt_.type, (const double2 *)s->H4,
+                                                         (const double2 *)s->tw, s->Fc);
+  QHP_LAUNCH_OK(s);
+  s->fc_segment = seg;
+  return QHP_OK;
+}
+
+// Q5-Q7 at the end of a segment
+int qhp_qtb_adapt(qhp_system *s) {
+  const int ns = s->n_seg, nf = ns + 1, nt = s->nt, nk = 2 * ns;
+  const size_t smem = sizeof(double2) * nk + sizeof(double) * 2 * nf;
+  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_spectra, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_qtb_spectra<<<s->n_spec_cta, fft_threads(nk), smem, s->stream>>>(ns, s->spec_cta, s->atoms_by_type, s->vseg, s->Fc,
+                                                                     (const double2 *)s->tw, 4 * ns, s->spec_part);
+  QHP_LAUNCH_OK(s);
+  k_qtb_reduce<<<(nt * nf + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->n_spec_cta, s->spec_cta, s->spec_part,
+                                                           s->spec_part + (size_t)s->n_spec_cta * 2 * nf, s->dt, s->Cvv, s->CvF);
+  QHP_LAUNCH_OK(s);
+  if (s->th.a_gamma != 0.0) {
+    k_qtb_adapt<<<nt, 256, 0, s->stream>>>(ns, s->dt_.mass, s->th.gamma0, s->th.a_gamma, s->th.gamma_min_frac, s->Cvv, s->CvF, s->gamma);
+    QHP_LAUNCH_OK(s);
+  }
+  return QHP_OK;
+}

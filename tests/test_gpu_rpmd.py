@@ -1,0 +1,163 @@
+"""GPU-vs-oracle parity of the RPMD path (BASELINE.json north_star tolerances):
+neighbour objects bit-exact; forces within 1e-10 * max|F|; positions within 1e-8 A after 20 steps."""
+import numpy as np
+import pytest
+
+from gpu_common import T_K, make_pair, to_dev
+from workloads import water as W
+
+pytestmark = pytest.mark.gpu
+
+FTOL = 1e-10     # relative to max|F|   (north_star)
+XTOL = 1e-8      # Angstrom after 20 steps (north_star)
+
+
+def _lists_check(sysg, top, x0):
+    import oracle as O
+    otop = O.Topology(top)
+    cent = x0.mean(axis=0)
+    nc, cell_of, order, cell_start = sysg.neighbor_lists()
+    onc, ocell_of, oorder, ocell_start = O.cells(otop, O.beads_to_nm(x0)[0])
+    assert np.array_equal(nc.cpu().numpy(), onc)
+    assert np.array_equal(cell_of.cpu().numpy(), ocell_of)
+    assert np.array_equal(order.cpu().numpy(), oorder)
+    assert np.array_equal(cell_start.cpu().numpy(), ocell_start)
+    return otop, O.beads_to_nm(x0)[0]
+
+
+def _pairs_from_gpu(sysg):
+    count, nbr = sysg.pair_list()
+    count = count.cpu().numpy().astype(np.int64)
+    nbr = nbr.cpu().numpy().astype(np.int64)
+    i = np.repeat(np.arange(count.size), count)
+    return count, i, nbr
+
+
+@pytest.mark.parametrize("n_mol,P,Pc", [(216, 8, 8), (216, 8, 4), (343, 3, 2)])
+def test_small_box_lists_forces_observables(n_mol, P, Pc):
+    import oracle as O
+    top = W.water_box(n_mol)
+    sysg, ref, x0, p0 = make_pair(top, P, Pc, 0.25, "pile", sigma_bead=0.05)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    otop, cent = _lists_check(sysg, top, x0)
+    # pair set == brute force definition, bit-exact
+    count, i, j = _pairs_from_gpu(sysg)
+    half = np.stack([i[i < j], j[i < j]], 1)
+    half = half[np.lexsort((half[:, 1], half[:, 0]))]
+    assert np.array_equal(half, O.pairs_brute(otop, cent))
+    assert (i < j).sum() * 2 == i.size                      # full list is symmetric
+    # contraction
+    xc = sysg.contracted().cpu().numpy()
+    assert np.abs(xc - O.contract(ref.Q, Pc)).max() < 1e-13
+    # forces
+    G = sysg.forces().cpu().numpy()
+    Gref = O.bead_forces(otop, P, Pc, x0)
+    assert np.abs(G - Gref).max() < FTOL * np.abs(Gref).max()
+    # observables
+    obs = sysg.observables().cpu().numpy()
+    oref = ref.observables()
+    assert np.abs(obs - oref).max() < 1e-10 * np.abs(oref).max()
+    # state round trip through the normal modes
+    x1, p1, step = sysg.get_state()
+    assert step == 0
+    assert np.abs(x1.cpu().numpy() - x0).max() < 1e-13 and np.abs(p1.cpu().numpy() - p0).max() < 1e-11
+
+
+@pytest.mark.parametrize("thermo,P,Pc", [("pile", 8, 8), ("none", 8, 8), ("pile", 8, 4), ("pile", 1, 1)])
+def test_c0_20_steps_positions(thermo, P, Pc):
+    """configs[0]: 216 waters, P = 8, dt = 0.25 fs, PILE gamma0 = 1/ps (plus contracted / classical variants)."""
+    top = W.water_box(216)
+    sysg, ref, x0, p0 = make_pair(top, P, Pc, 0.25, thermo, gamma0=1.0)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    sysg.step(7)
+    sysg.step(13)                       # two calls: the deferred half kick must carry over
+    ref.step(20)
+    x1, p1, step = sysg.get_state()
+    xr, pr = ref.get_state()
+    assert step == 20
+    assert np.abs(x1.cpu().numpy() - xr).max() < XTOL
+    assert np.abs(p1.cpu().numpy() - pr).max() < 1e-6 * np.abs(pr).max()
+    G = sysg.forces().cpu().numpy()
+    Gr = ref.forces()
+    assert np.abs(G - Gr).max() < 1e-7 * np.abs(Gr).max()    # forces at positions that agree to 1e-8 A
+    sysg.check()
+
+
+def test_resume_is_bit_identical():
+    top = W.water_box(216)
+    sysg, _, x0, p0 = make_pair(top, 8, 4, 0.25, "pile")
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    sysg.step(10)
+    xa, pa, st = sysg.get_state()
+    sysg.step(10)
+    xb, pb, _ = sysg.get_state()
+    sys2, _, _, _ = make_pair(top, 8, 4, 0.25, "pile")
+    sys2.set_state(xa.clone(), pa.clone(), st)
+    sys2.step(10)
+    xc, pc, st2 = sys2.get_state()
+    assert st2 == 20
+    # get_state/set_state pass through the bead representation: equal up to the round trip
+    assert (xb - xc).abs().max().item() < 1e-12
+    assert (pb - pc).abs().max().item() < 1e-9
+
+
+def test_c2_lists_forces_steps():
+    """configs[2]: 4096 waters (12,288 atoms), P = 32, P' = 4: cell path (4x4x4 cells), several tiles,
+    ragged last tile."""
+    import oracle as O
+    top = W.water_box(4096)
+    sysg, ref, x0, p0 = make_pair(top, 32, 4, 0.25, "pile")
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    otop, cent = _lists_check(sysg, top, x0)
+    count, i, j = _pairs_from_gpu(sysg)
+    half = np.stack([i[i < j], j[i < j]], 1)
+    half = half[np.lexsort((half[:, 1], half[:, 0]))]
+    assert np.array_equal(half, O.pairs_brute(otop, cent))
+    G = sysg.forces().cpu().numpy()
+    Gref = O.bead_forces(otop, 32, 4, x0)
+    assert np.abs(G - Gref).max() < FTOL * np.abs(Gref).max()
+    sysg.step(20)
+    ref.step(20)
+    x1, _, _ = sysg.get_state()
+    xr, _ = ref.get_state()
+    assert np.abs(x1.cpu().numpy() - xr).max() < XTOL
+    obs = sysg.observables().cpu().numpy()
+    oref = ref.observables()
+    assert np.abs(obs - oref).max() < 1e-8 * np.abs(oref).max()
+    sysg.check()
+
+
+def test_rebuild_during_run_keeps_parity():
+    """A tiny skin forces list rebuilds inside qhp_step; forces must not depend on the list."""
+    top = W.water_box(216)
+    top["skin"] = 0.05
+    sysg, ref, x0, p0 = make_pair(top, 4, 2, 0.5, "pile", gamma0=5.0, sigma_bead=0.02)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    sysg.step(20)
+    ref.step(20)
+    x1, _, _ = sysg.get_state()
+    xr, _ = ref.get_state()
+    assert np.abs(x1.cpu().numpy() - xr).max() < XTOL
+    c = sysg.counters()
+    assert c["rebuilds"] >= 3 and c["overflow"] == 0
+
+
+def test_harmonic_oscillators_single_atom_molecules():
+    """Tethered, non-interacting atoms (each its own molecule, no bonds): the harmonic system of the
+    closed-form pins; exercises tether forces and ragged tiles."""
+    top = W.oscillator_box(1000, 1.008, 769.3)
+    sysg, ref, x0, p0 = make_pair(top, 6, 6, 0.25, "pile", gamma0=2.0, sigma_bead=0.02)
+    sysg.set_state(to_dev(x0), to_dev(p0), 5)
+    ref.set_state(x0, p0, 5)
+    sysg.step(20)
+    ref.step(20)
+    x1, _, st = sysg.get_state()
+    xr, _ = ref.get_state()
+    assert st == 25
+    assert np.abs(x1.cpu().numpy() - xr).max() < 1e-10
+    obs = sysg.observables().cpu().numpy()
+    assert np.abs(obs - ref.observables()).max() < 1e-9 * np.abs(ref.observables()).max()
