@@ -134,7 +134,7 @@ int qhp_adqtb_gamma(qhp_system *sys, double *gamma);
 int qhp_adqtb_segment(qhp_system *sys, double *Fc, double *vseg);
 /* Counters for measurement: out_host[0] = neighbour-list rebuilds so far, [1] = list entries,
  * [2] = pair-bead interactions inside r_cut at the current positions (full list, both
- * directions), [3] = list capacity, [4] = kernels launched so far, [5] = overflow flag.
+ * directions), [3] = list capacity, [4] = kernels launched so far, [5] = error flags (bit 0 list overflow, bit 1 skin < 2 x bead spread).
  * n_out <= 6.  HOST pointer; synchronises. */
 int qhp_counters(qhp_system *sys, int64_t *out_host, int n_out);
 /* Synchronise the stream and report sticky CUDA / overflow errors. */

@@ -405,7 +405,8 @@ __global__ void k_to_beads(const double *__restrict__ Q, const double *__restric
 __global__ void k_contract(const double *__restrict__ Q, int N, int Pc, const double *__restrict__ Tc,
                            const int32_t *__restrict__ rank, const int32_t *__restrict__ type,
                            const int32_t *__restrict__ molid, double *pos4, double *cent4, double *cref,
-                           double *xc_out, int mode, const unsigned long long *d2max, double thresh2) {
+                           double *xc_out, int mode, const unsigned long long *d2max, double thresh2,
+                           long long *counters) {
   if (d2max && __longlong_as_double((long long)*d2max) < thresh2) return;
   const long long ND = 3LL * N;
   const long long d = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -418,6 +419,8 @@ __global__ void k_contract(const double *__restrict__ Q, int N, int Pc, const do
     for (int n = 0; n < Pc; ++n) s += Tc[j * Pc + n] * Q[n * ND + d];
     const double xc = spc * s;
     if (mode == 0) {
+      // a list built on the centroids can only cover beads closer than skin/2 to their centroid
+      if (cent4 && (xc - Q[d]) * (xc - Q[d]) > thresh2) counters[6] = 1;
       pos4[((long long)j * N + slot) * 4 + c] = xc;
       if (c == 0) reinterpret_cast<long long *>(pos4)[((long long)j * N + slot) * 4 + 3] = type[atom];
     } else {
@@ -578,7 +581,7 @@ int qhp_nm_contract(qhp_system *s, bool rebuild_mode, bool force) {
   const unsigned long long *flag = (rebuild_mode && !force) ? &s->d2max[s->flag_idx] : nullptr;
   k_contract<<<grid, tb, 0, s->stream>>>(s->Q, s->N, s->Pc, s->d_Tc, s->rank, s->dt_.type, s->dt_.molid,
                                         s->pos4, rebuild_mode ? s->cent4 : nullptr, s->cref, nullptr, 0,
-                                        flag, th * th);
+                                        flag, th * th, (long long *)s->counters);
   QHP_LAUNCH_OK(s);
   return QHP_OK;
 }
@@ -588,7 +591,7 @@ int qhp_nm_contracted_out(qhp_system *s, double *xc) {
   const int tb = 256;
   const unsigned grid = (unsigned)((ND + tb - 1) / tb);
   k_contract<<<grid, tb, 0, s->stream>>>(s->Q, s->N, s->Pc, s->d_Tc, nullptr, s->dt_.type, s->dt_.molid,
-                                        nullptr, nullptr, nullptr, xc, 1, nullptr, 0.0);
+                                        nullptr, nullptr, nullptr, xc, 1, nullptr, 0.0, nullptr);
   QHP_LAUNCH_OK(s);
   return QHP_OK;
 }

@@ -474,7 +474,7 @@ extern "C" int qhp_counters(qhp_system *s, int64_t *out_host, int n_out) {
   int64_t c[8];
   QHP_CUDA_OK(s, cudaMemcpyAsync(c, s->counters, sizeof(c), cudaMemcpyDeviceToHost, s->stream));
   QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
-  const int64_t v[6] = {c[0], total, c[3], s->nbr_stride * s->N, s->n_launch, c[1]};
+  const int64_t v[6] = {c[0], total, c[3], s->nbr_stride * s->N, s->n_launch, c[1] | (c[6] << 1)};
   for (int k = 0; k < std::min(n_out, 6); ++k) out_host[k] = v[k];
   return QHP_OK;
 }
@@ -484,9 +484,10 @@ extern "C" int qhp_check(qhp_system *s) {
   QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
   QHP_CUDA_OK(s, cudaGetLastError());
   if (s->counters) {
-    int64_t ov = 0;
-    QHP_CUDA_OK(s, cudaMemcpy(&ov, &s->counters[1], sizeof(ov), cudaMemcpyDeviceToHost));
-    if (ov) { s->err = "neighbour table overflow: a row exceeded its capacity"; return QHP_ESTATE; }
+    int64_t c[8];
+    QHP_CUDA_OK(s, cudaMemcpy(c, s->counters, sizeof(c), cudaMemcpyDeviceToHost));
+    if (c[1]) { s->err = "neighbour table overflow: a row exceeded its capacity"; return QHP_ESTATE; }
+    if (c[6]) { s->err = "skin too small: a contracted bead is farther than skin/2 from its centroid, the centroid list cannot cover it"; return QHP_ESTATE; }
   }
   return QHP_OK;
 }

@@ -83,7 +83,7 @@ struct qhp_system {
   int32_t *nbr = nullptr, *nbr_count = nullptr;
   int64_t nbr_stride = 0;
   unsigned long long *d2max = nullptr;     // [2] double bits, max |xc - cref|^2, double-buffered by step parity
-  int64_t *counters = nullptr;             // [8] device: 0 rebuilds, 1 overflow flag, 2 max row count, 3 in-cutoff count
+  int64_t *counters = nullptr;             // [8] device: 0 rebuilds, 1 overflow flag, 2 max row count, 3 in-cutoff count, 6 skin-too-small flag
   double *red = nullptr;                   // scratch for reductions
   size_t red_len = 0;
   double *obs = nullptr;                   // [8] device observables

@@ -98,7 +98,7 @@ __global__ void k_twiddle(double2 *tw, int n) {
   tw[m] = make_double2(c, s);
 }
 
-__global__ void k_fft_batch(double2 *data, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
+__global__ void __launch_bounds__(1024) k_fft_batch(double2 *data, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
   extern __shared__ double2 fbuf[];
   double2 *d = data + (long long)blockIdx.x * n;
   for (int k = threadIdx.x; k < n; k += blockDim.x) fbuf[k] = d[k];
@@ -178,7 +178,7 @@ __global__ void k_qtb_spectrum4(int nt, int n_seg, const double *__restrict__ hk
 // kernel h is real, so real and imaginary parts are filtered independently), z through a second.
 //   F_c[dof][n] = sum_k h_z[k] r(dof, seg*n_seg + n - k + n_seg),  n = 0..n_seg-1
 // ---------------------------------------------------------------------------------------------
-__global__ void k_qtb_noise(int n_seg, unsigned long long seed, long long seg, const int32_t *__restrict__ type,
+__global__ void __launch_bounds__(1024) k_qtb_noise(int n_seg, unsigned long long seed, long long seg, const int32_t *__restrict__ type,
                             const double2 *__restrict__ H4, const double2 *__restrict__ tw, double *Fc) {
   extern __shared__ double2 nbuf[];
   const int nf = 4 * n_seg, nw = 3 * n_seg;
@@ -219,7 +219,7 @@ __global__ void k_qtb_noise(int n_seg, unsigned long long seed, long long seg, c
 // Q5 + Q6: spectra.  One CTA walks a run of atoms of one type; v and F_c of a DOF are the real and
 // imaginary part of one zero-padded N_k-point transform.  Per-CTA sums -> fixed-order reduction.
 // ---------------------------------------------------------------------------------------------
-__global__ void k_qtb_spectra(int n_seg, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
+__global__ void __launch_bounds__(1024) k_qtb_spectra(int n_seg, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
                               const double *__restrict__ vseg, const double *__restrict__ Fc,
                               const double2 *__restrict__ tw, int tw_n, double *part) {
   extern __shared__ double2 sbuf[];

@@ -130,20 +130,33 @@ def test_c2_lists_forces_steps():
     sysg.check()
 
 
-def test_rebuild_during_run_keeps_parity():
-    """A tiny skin forces list rebuilds inside qhp_step; forces must not depend on the list."""
+@pytest.mark.parametrize("P,Pc,skin,min_rebuilds", [(1, 1, 0.1, 5), (4, 2, 0.7, 1)])
+def test_rebuild_during_run_keeps_parity(P, Pc, skin, min_rebuilds):
+    """A small skin forces list rebuilds inside qhp_step; forces must not depend on the list."""
     top = W.water_box(216)
-    top["skin"] = 0.05
-    sysg, ref, x0, p0 = make_pair(top, 4, 2, 0.5, "pile", gamma0=5.0, sigma_bead=0.02)
+    top["skin"] = skin
+    sysg, ref, x0, p0 = make_pair(top, P, Pc, 0.5, "pile", gamma0=5.0, sigma_bead=0.002)
     sysg.set_state(to_dev(x0), to_dev(p0), 0)
     ref.set_state(x0, p0, 0)
     sysg.step(20)
     ref.step(20)
     x1, _, _ = sysg.get_state()
     xr, _ = ref.get_state()
+    sysg.check()
     assert np.abs(x1.cpu().numpy() - xr).max() < XTOL
     c = sysg.counters()
-    assert c["rebuilds"] >= 3 and c["overflow"] == 0
+    assert c["rebuilds"] >= 1 + min_rebuilds and c["overflow"] == 0
+
+
+def test_skin_smaller_than_bead_spread_is_reported():
+    """A centroid list cannot cover beads farther than skin/2 from their centroid: ESTATE at check."""
+    import paper_2212_03137_b200 as qhp
+    top = W.water_box(216)
+    top["skin"] = 0.05
+    sysg, _, x0, p0 = make_pair(top, 4, 2, 0.5, "pile", sigma_bead=0.05)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    with pytest.raises(qhp.QhpError):
+        sysg.check()
 
 
 def test_harmonic_oscillators_single_atom_molecules():
