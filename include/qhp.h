@@ -137,6 +137,13 @@ int qhp_adqtb_segment(qhp_system *sys, double *Fc, double *vseg);
  * directions), [3] = list capacity, [4] = kernels launched so far, [5] = error flags (bit 0 list overflow, bit 1 skin < 2 x bead spread).
  * n_out <= 6.  HOST pointer; synchronises. */
 int qhp_counters(qhp_system *sys, int64_t *out_host, int n_out);
+/* Per-phase device timing with CUDA events recorded on the library stream inside qhp_step:
+ * qhp_profile(sys, 1) starts recording (and clears the sums), qhp_profile(sys, 0) stops.
+ * qhp_profile_read synchronises and writes ms_host[0..3] = summed milliseconds of
+ * {integrator pass, neighbour rebuild chain, pair forces, adQTB segment work} and
+ * n_host[0..3] = number of timed intervals of each.  HOST pointers. */
+int qhp_profile(qhp_system *sys, int enable);
+int qhp_profile_read(qhp_system *sys, double *ms_host, int64_t *n_host);
 /* Synchronise the stream and report sticky CUDA / overflow errors. */
 int qhp_check(qhp_system *sys);
 const char *qhp_last_error(const qhp_system *sys); /* sys may be NULL: last create error */

@@ -17,7 +17,7 @@ _STATUS = {0: "QHP_OK", -1: "QHP_EINVAL", -2: "QHP_ENOMEM", -3: "QHP_ECUDA", -4:
 SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_state", "qhp_get_state", "qhp_set_state_host",
            "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
            "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma",
-           "qhp_adqtb_segment", "qhp_counters", "qhp_check", "qhp_last_error", "qhp_philox_normals",
+           "qhp_adqtb_segment", "qhp_counters", "qhp_profile", "qhp_profile_read", "qhp_check", "qhp_last_error", "qhp_philox_normals",
            "qhp_fft_c2c", "qhp_dfma_probe"]
 
 
@@ -74,6 +74,8 @@ def lib():
         L.qhp_adqtb_segment.argtypes = [vp, vp, vp]
         L.qhp_counters.argtypes = [vp, C.POINTER(i64), i32]
         L.qhp_check.argtypes = [vp]
+        L.qhp_profile.argtypes = [vp, i32]
+        L.qhp_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
         L.qhp_last_error.argtypes = [vp]
         L.qhp_last_error.restype = C.c_char_p
         L.qhp_philox_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, i64, vp, vp, vp]
@@ -255,6 +257,15 @@ class System:
 
     def check(self):
         self._ok(self._L.qhp_check(self._h))
+
+    def profile(self, enable: bool):
+        self._ok(self._L.qhp_profile(self._h, int(bool(enable))))
+
+    def profile_read(self) -> dict:
+        ms, n = (C.c_double * 4)(), (C.c_int64 * 4)()
+        self._ok(self._L.qhp_profile_read(self._h, ms, n))
+        keys = ["integrate", "rebuild", "pair", "qtb"]
+        return {k: dict(ms=float(ms[i]), n=int(n[i])) for i, k in enumerate(keys)}
 
 
 def _host_ptr(a, numel):

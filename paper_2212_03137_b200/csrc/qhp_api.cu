@@ -273,7 +273,8 @@ extern "C" int qhp_create(const qhp_topology *top, int P, int P_contract, double
 
 extern "C" int qhp_destroy(qhp_system *s) {
   if (!s) return QHP_OK;
-  if (s->stream || true) cudaStreamSynchronize(s->stream);
+  cudaStreamSynchronize(s->stream);
+  for (cudaEvent_t e : s->prof_ev) cudaEventDestroy(e);
   qhp_dev_topology &d = s->dt_;
   void *ptrs[] = {d.type, d.molid, d.mol_atom_start, d.mol_bond_start, d.mol_angle_start, d.bond_idx, d.bond_k,
                   d.bond_r0, d.angle_idx, d.angle_k, d.angle_th0, d.mass, d.tether_k, d.tiles, s->Q, s->Pm, s->coef,
@@ -357,6 +358,52 @@ extern "C" int qhp_get_state_host(qhp_system *s, double *x_beads, double *p_bead
   return qhp_check(s);
 }
 
+// ---- per-phase profiling ----------------------------------------------------------------------
+static int prof_drain(qhp_system *s) {
+  if (s->prof_ev.empty()) return QHP_OK;
+  QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
+  for (size_t k = 0; k < s->prof_kind.size(); ++k) {
+    float ms = 0.f;
+    QHP_CUDA_OK(s, cudaEventElapsedTime(&ms, s->prof_ev[2 * k], s->prof_ev[2 * k + 1]));
+    s->prof_ms[s->prof_kind[k]] += ms;
+    s->prof_n[s->prof_kind[k]] += 1;
+  }
+  for (cudaEvent_t e : s->prof_ev) cudaEventDestroy(e);
+  s->prof_ev.clear();
+  s->prof_kind.clear();
+  return QHP_OK;
+}
+struct prof_scope {
+  qhp_system *s; bool on;
+  prof_scope(qhp_system *s_, int kind) : s(s_), on(s_->prof) {
+    if (!on) return;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    s->prof_ev.push_back(a); s->prof_ev.push_back(b); s->prof_kind.push_back(kind);
+    cudaEventRecord(a, s->stream);
+  }
+  ~prof_scope() { if (on) cudaEventRecord(s->prof_ev.back(), s->stream); }
+};
+
+extern "C" int qhp_profile(qhp_system *s, int enable) {
+  if (!s) return QHP_EINVAL;
+  if (enable) {
+    int rc = prof_drain(s);
+    if (rc) return rc;
+    for (int k = 0; k < 4; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
+  }
+  s->prof = enable != 0;
+  return QHP_OK;
+}
+
+extern "C" int qhp_profile_read(qhp_system *s, double *ms_host, int64_t *n_host) {
+  if (!s) return QHP_EINVAL;
+  int rc = prof_drain(s);
+  if (rc) return rc;
+  for (int k = 0; k < 4; ++k) { if (ms_host) ms_host[k] = s->prof_ms[k]; if (n_host) n_host[k] = s->prof_n[k]; }
+  return QHP_OK;
+}
+
 extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
   if (!s || nsteps < 0) return QHP_EINVAL;
   if (!s->have_state) { s->err = "qhp_step before qhp_set_state"; return QHP_ESTATE; }
@@ -365,16 +412,29 @@ extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
     const int64_t st = s->step;
     int rc;
     if (adqtb && st % s->n_seg == 0 && s->fc_segment != st / s->n_seg) {
+      prof_scope ps(s, 3);
       rc = qhp_qtb_generate(s, st / s->n_seg);          // Q2-Q4 at the start of a segment
       if (rc) return rc;
     }
-    rc = qhp_nm_integrate(s, s->pending_kick, true, st);  // [B] B A O A + V_f + contraction
-    if (rc) return rc;
+    {
+      prof_scope ps(s, 0);
+      rc = qhp_nm_integrate(s, s->pending_kick, true, st);  // [B] B A O A + V_f + contraction
+      if (rc) return rc;
+    }
     s->pending_kick = true;
-    rc = rebuild_and_forces(s, false);                    // R7 (only when needed) + R8
-    if (rc) return rc;
+    {
+      prof_scope ps(s, 1);
+      rc = qhp_cells_rebuild(s, false);                   // R7 (returns at once on the device unless needed)
+      if (rc) return rc;
+    }
+    {
+      prof_scope ps(s, 2);
+      rc = qhp_pair_forces(s, false);                     // R8
+      if (rc) return rc;
+    }
     s->step = st + 1;
     if (adqtb && s->step % s->n_seg == 0) {
+      prof_scope ps(s, 3);
       rc = qhp_qtb_adapt(s);                              // Q5-Q7 at the end of a segment
       if (rc) return rc;
     }
@@ -466,6 +526,7 @@ extern "C" int qhp_adqtb_segment(qhp_system *s, double *Fc, double *vseg) {
 extern "C" int qhp_counters(qhp_system *s, int64_t *out_host, int n_out) {
   if (!s || !out_host) return QHP_EINVAL;
   if (!s->have_state) { s->err = "no state"; return QHP_ESTATE; }
+  const int64_t launches = s->n_launch;       // this call's own launches are not counted
   int rc = qhp_pair_forces(s, true);
   if (rc) return rc;
   int64_t total = 0;
@@ -474,7 +535,8 @@ extern "C" int qhp_counters(qhp_system *s, int64_t *out_host, int n_out) {
   int64_t c[8];
   QHP_CUDA_OK(s, cudaMemcpyAsync(c, s->counters, sizeof(c), cudaMemcpyDeviceToHost, s->stream));
   QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
-  const int64_t v[6] = {c[0], total, c[3], s->nbr_stride * s->N, s->n_launch, c[1] | (c[6] << 1)};
+  s->n_launch = launches;
+  const int64_t v[6] = {c[0], total, c[3], s->nbr_stride * s->N, launches, c[1] | (c[6] << 1)};
   for (int k = 0; k < std::min(n_out, 6); ++k) out_host[k] = v[k];
   return QHP_OK;
 }

@@ -105,6 +105,13 @@ struct qhp_system {
   double *Cvv = nullptr, *CvF = nullptr; // [nt][n_seg+1]
   int64_t fc_segment = -1;
 
+  // ---- per-phase profiling (qhp_profile) ----
+  bool prof = false;
+  std::vector<cudaEvent_t> prof_ev;      // flat list of (begin, end) pairs
+  std::vector<int> prof_kind;            // phase of each pair
+  double prof_ms[4] = {0, 0, 0, 0};
+  int64_t prof_n[4] = {0, 0, 0, 0};
+
   // ---- run state (host) ----
   bool have_state = false;
   bool pending_kick = false;   // the final B(dt/2) of the last step has not been applied yet
