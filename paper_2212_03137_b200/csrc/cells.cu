@@ -152,6 +152,66 @@ __global__ void __launch_bounds__(256) k_list_build(const CellArgs a, const doub
   }
 }
 
+// Same pair set, written as 16-bit indices into the staged array of the row's cell (pair_staged.cu):
+// index = (number of atoms in the stencil cells before this one, in the stencil order below) + (k - b).
+// Requires nc >= 4 in every dimension (27 distinct stencil cells).
+__global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const double *__restrict__ cent4,
+                                                      const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
+                                                      const int32_t *__restrict__ cell_start, uint16_t *nbr,
+                                                      int32_t *nbr_count, long long stride, long long *counters) {
+  if (cells_skip(a)) return;
+  const int lane = threadIdx.x & 31;
+  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i >= a.N) return;
+  if (i == 0 && lane == 0 && nbr) counters[0] += 1;
+  const double4 ci = reinterpret_cast<const double4 *>(cent4)[i];
+  const long long mi = __double_as_longlong(ci.w);
+  const int cell = cell_of[order[i]];
+  const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
+  const unsigned lt = (1u << lane) - 1u;
+  int cnt = 0, off = 0;
+  for (int ox = 0; ox < 3; ++ox)
+    for (int oy = 0; oy < 3; ++oy)
+      for (int oz = 0; oz < 3; ++oz) {
+        const int qx = (cx - 1 + ox + a.nc[0]) % a.nc[0], qy = (cy - 1 + oy + a.nc[1]) % a.nc[1],
+                  qz = (cz - 1 + oz + a.nc[2]) % a.nc[2];
+        const int c2 = (qx * a.nc[1] + qy) * a.nc[2] + qz;
+        const int b = cell_start[c2], e = cell_start[c2 + 1];
+        for (int k0 = b; k0 < e; k0 += 32) {
+          const int k = k0 + lane;
+          bool hit = false;
+          if (k < e && k != i) {
+            const double4 cj = reinterpret_cast<const double4 *>(cent4)[k];
+            if (__double_as_longlong(cj.w) != mi) {
+              double dx = __dsub_rn(ci.x, cj.x), dy = __dsub_rn(ci.y, cj.y), dz = __dsub_rn(ci.z, cj.z);
+              dx = __fma_rn(-a.box[0], rint(__dmul_rn(dx, a.inv_box[0])), dx);
+              dy = __fma_rn(-a.box[1], rint(__dmul_rn(dy, a.inv_box[1])), dy);
+              dz = __fma_rn(-a.box[2], rint(__dmul_rn(dz, a.inv_box[2])), dz);
+              const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+              hit = d2 < a.rl2;
+            }
+          }
+          const unsigned mask = __ballot_sync(0xffffffffu, hit);
+          if (hit && nbr) {
+            const int pos = cnt + __popc(mask & lt);
+            if (pos < stride) nbr[i * stride + pos] = (uint16_t)(off + k - b);
+          }
+          cnt += __popc(mask);
+        }
+        off += e - b;
+      }
+  if (lane == 0) {
+    if (nbr) {
+      nbr_count[i] = (int)min((long long)cnt, stride);
+      if (cnt > stride) counters[1] = 1;
+    } else {
+      nbr_count[i] = cnt;
+    }
+    atomicMax((unsigned long long *)&counters[2], (unsigned long long)cnt);
+    atomicMax((unsigned long long *)&counters[5], (unsigned long long)off);   // staged-region size
+  }
+}
+
 // ---- export in atom indices (parity hook) ---------------------------------------------------------
 __global__ void k_export_count(int N, const int32_t *__restrict__ order, const int32_t *__restrict__ nbr_count, int32_t *count) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -167,6 +227,39 @@ __global__ void k_export_fill(int N, const int32_t *__restrict__ order, const in
   const long long s0 = start[a];
   for (int k = lane; k < n; k += 32)
     if (s0 + k < cap) out[s0 + k] = order[nbr[i * stride + k]];
+}
+
+// staged format: translate the 16-bit staged index back to a slot, then to an atom
+__global__ void k_export_fill16(const CellArgs a, const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
+                                const int32_t *__restrict__ cell_start, const int32_t *__restrict__ nbr_count,
+                                const uint16_t *__restrict__ nbr, long long stride, const int32_t *__restrict__ start,
+                                int32_t *out, long long cap) {
+  const int lane = threadIdx.x & 31;
+  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i >= a.N) return;
+  const int at = order[i], n = nbr_count[i];
+  const int cell = cell_of[at];
+  const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
+  int cb = 0, cn = 0;                       // lane s < 27: first slot and size of stencil cell s
+  if (lane < 27) {
+    const int ox = lane / 9, oy = (lane / 3) % 3, oz = lane % 3;
+    const int qx = (cx - 1 + ox + a.nc[0]) % a.nc[0], qy = (cy - 1 + oy + a.nc[1]) % a.nc[1],
+              qz = (cz - 1 + oz + a.nc[2]) % a.nc[2];
+    const int c2 = (qx * a.nc[1] + qy) * a.nc[2] + qz;
+    cb = cell_start[c2]; cn = cell_start[c2 + 1] - cb;
+  }
+  const long long s0 = start[at];
+  for (int k0 = 0; k0 < n; k0 += 32) {
+    const int k = k0 + lane;
+    const int loc = k < n ? (int)nbr[i * stride + k] : 0;
+    int off = 0, slot = -1;
+    for (int s = 0; s < 27; ++s) {
+      const int b = __shfl_sync(0xffffffffu, cb, s), c = __shfl_sync(0xffffffffu, cn, s);
+      if (slot < 0 && loc < off + c) slot = b + loc - off;
+      off += c;
+    }
+    if (k < n && s0 + k < cap) out[s0 + k] = order[slot];
+  }
 }
 
 static CellArgs cell_args(qhp_system *s, bool force) {
@@ -199,9 +292,14 @@ static int list_build(qhp_system *s, const CellArgs &a, bool count_only) {
   const int tb = 256;
   const long long threads = 32LL * s->N;
   const unsigned grid = (unsigned)((threads + tb - 1) / tb);
-  k_list_build<<<grid, tb, 0, s->stream>>>(a, s->cent4, s->cell_of, s->order, s->cell_start,
-                                          count_only ? nullptr : s->nbr, s->nbr_count, s->nbr_stride,
-                                          (long long *)s->counters);
+  if (s->staged)
+    k_list_build16<<<grid, tb, 0, s->stream>>>(a, s->cent4, s->cell_of, s->order, s->cell_start,
+                                              count_only ? nullptr : s->nbr16, s->nbr_count, s->nbr_stride,
+                                              (long long *)s->counters);
+  else
+    k_list_build<<<grid, tb, 0, s->stream>>>(a, s->cent4, s->cell_of, s->order, s->cell_start,
+                                            count_only ? nullptr : s->nbr, s->nbr_count, s->nbr_stride,
+                                            (long long *)s->counters);
   QHP_LAUNCH_OK(s);
   return QHP_OK;
 }
@@ -214,23 +312,37 @@ int qhp_cells_rebuild(qhp_system *s, bool force) {
   if (rc) return rc;
   if (force) {
     // synchronising call sites only: size the fixed-stride table from a counting pass
-    QHP_CUDA_OK(s, cudaMemsetAsync(&s->counters[2], 0, sizeof(int64_t), s->stream));
-    rc = list_build(s, a, true);
-    if (rc) return rc;
+    // the staged pair kernel serves the system if its geometry allows it (qhp_pair_setup) and the
+    // densest 27-cell neighbourhood fits in shared memory with some room for drift between rebuilds
+    s->staged = s->staged_ok;
     int64_t mx = 0;
-    QHP_CUDA_OK(s, cudaMemcpyAsync(&mx, &s->counters[2], sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
-    QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
-    if (s->nbr == nullptr || mx + 8 > s->nbr_stride) {
+    for (int attempt = 0; attempt < 2; ++attempt) {
+      QHP_CUDA_OK(s, cudaMemsetAsync(&s->counters[2], 0, sizeof(int64_t), s->stream));
+      QHP_CUDA_OK(s, cudaMemsetAsync(&s->counters[5], 0, sizeof(int64_t), s->stream));
+      rc = list_build(s, a, true);
+      if (rc) return rc;
+      int64_t region = 0;
+      QHP_CUDA_OK(s, cudaMemcpyAsync(&mx, &s->counters[2], sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
+      QHP_CUDA_OK(s, cudaMemcpyAsync(&region, &s->counters[5], sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
+      QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
+      if (!s->staged || region + region / 16 + 32 <= s->staged_cap) break;
+      s->staged = false;                               // too dense: generic kernel and 32-bit list
+    }
+    const bool have = s->staged ? (s->nbr16 != nullptr) : (s->nbr != nullptr);
+    if (!have || mx + 8 > s->nbr_stride) {
       int64_t stride = (int64_t)((double)mx * 1.4) + 32;
-      stride = (stride + 3) / 4 * 4;
-      if (stride > s->N) stride = (s->N + 3) / 4 * 4;
+      stride = (stride + 31) / 32 * 32;
+      if (stride > s->N) stride = (s->N + 31) / 32 * 32;
       if (stride < 4) stride = 4;
       if (s->nbr) cudaFree(s->nbr);
-      s->nbr = nullptr;
+      if (s->nbr16) cudaFree(s->nbr16);
+      s->nbr = nullptr; s->nbr16 = nullptr;
       s->nbr_stride = stride;
-      if (cudaMalloc(&s->nbr, sizeof(int32_t) * (size_t)stride * (size_t)s->N) != cudaSuccess) {
+      const cudaError_t e = s->staged ? cudaMalloc(&s->nbr16, sizeof(uint16_t) * (size_t)stride * (size_t)s->N)
+                                      : cudaMalloc(&s->nbr, sizeof(int32_t) * (size_t)stride * (size_t)s->N);
+      if (e != cudaSuccess) {
         s->err = "neighbour table allocation failed";
-        s->nbr = nullptr;
+        s->nbr = nullptr; s->nbr16 = nullptr;
         return QHP_ENOMEM;
       }
     }
@@ -253,8 +365,14 @@ int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, i
   QHP_LAUNCH_OK(s);
   if (nbr) {
     const long long threads = 32LL * s->N;
-    k_export_fill<<<(unsigned)((threads + tb - 1) / tb), tb, 0, s->stream>>>(s->N, s->order, s->nbr_count, s->nbr,
-                                                                           s->nbr_stride, start, nbr, cap);
+    if (s->staged) {
+      const CellArgs ca = cell_args(s, true);
+      k_export_fill16<<<(unsigned)((threads + tb - 1) / tb), tb, 0, s->stream>>>(ca, s->cell_of, s->order, s->cell_start,
+                                                                               s->nbr_count, s->nbr16, s->nbr_stride, start, nbr, cap);
+    } else {
+      k_export_fill<<<(unsigned)((threads + tb - 1) / tb), tb, 0, s->stream>>>(s->N, s->order, s->nbr_count, s->nbr,
+                                                                             s->nbr_stride, start, nbr, cap);
+    }
     QHP_LAUNCH_OK(s);
   }
   int32_t tot = 0;

@@ -149,7 +149,24 @@ int qhp_pair_geometry(const qhp_system *s, int *NB_out, int *L_out, unsigned *gx
   return (int)(*gx * *gy);
 }
 
+int qhp_pair_staged_partials(const qhp_system *s);
+int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned long long *count);
+
+// upper bound of the per-CTA energy partials of either kernel (sizes s->red)
+int qhp_pair_partials(const qhp_system *s) {
+  int NB, L; unsigned gx, gy;
+  const int n = qhp_pair_geometry(s, &NB, &L, &gx, &gy);
+  const int m = s->staged_ok ? qhp_pair_staged_partials(s) : 0;
+  return n > m ? n : m;
+}
+
 int qhp_pair_forces(qhp_system *s, bool energy) {
+  if (energy) {
+    QHP_CUDA_OK(s, cudaMemsetAsync(&s->counters[3], 0, sizeof(int64_t), s->stream));
+    QHP_CUDA_OK(s, cudaMemsetAsync(s->red + 4 * (size_t)s->n_tiles, 0, sizeof(double) * (size_t)qhp_pair_partials(s), s->stream));
+  }
+  if (s->staged)
+    return qhp_pair_staged_forces(s, energy, s->red + 4 * (size_t)s->n_tiles, (unsigned long long *)&s->counters[3]);
   PairArgs a{};
   a.N = s->N; a.Pc = s->Pc; a.nt = s->nt;
   a.pos4 = s->pos4; a.Fs = s->Fs; a.nbr = s->nbr; a.nbr_count = s->nbr_count; a.stride = s->nbr_stride;
@@ -164,7 +181,6 @@ int qhp_pair_forces(qhp_system *s, bool energy) {
   qhp_pair_geometry(s, &NB, &L, &gx, &gy);
   a.part = s->red + 4 * (size_t)s->n_tiles;
   a.count = (unsigned long long *)&s->counters[3];
-  if (energy) QHP_CUDA_OK(s, cudaMemsetAsync(&s->counters[3], 0, sizeof(int64_t), s->stream));
   const dim3 grid(gx, gy);
   const size_t smem = sizeof(double) * 4 * s->nt * s->nt;
   switch (NB) {

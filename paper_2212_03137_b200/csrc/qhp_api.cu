@@ -257,10 +257,11 @@ extern "C" int qhp_create(const qhp_topology *top, int P, int P_contract, double
   CREATE_CUDA(cudaMemset(s->counters, 0, sizeof(int64_t) * 8));
   CREATE_CUDA(cudaMalloc(&s->obs, sizeof(double) * 8));
   {
-    int NB, L; unsigned gx, gy;
-    const int n_pair = qhp_pair_geometry(s, &NB, &L, &gx, &gy);
-    s->red_len = 4 * (size_t)s->n_tiles + (size_t)n_pair + 16;
+    const int rc = qhp_pair_setup(s);
+    if (rc) CREATE_FAIL(rc, s->err);
+    s->red_len = 4 * (size_t)s->n_tiles + (size_t)qhp_pair_partials(s) + 16;
     CREATE_CUDA(cudaMalloc(&s->red, sizeof(double) * s->red_len));
+    CREATE_CUDA(cudaMemset(s->red, 0, sizeof(double) * s->red_len));
   }
   if (kind == QHP_THERMO_ADQTB) {
     const int rc = qhp_qtb_init(s);
@@ -279,7 +280,7 @@ extern "C" int qhp_destroy(qhp_system *s) {
   void *ptrs[] = {d.type, d.molid, d.mol_atom_start, d.mol_bond_start, d.mol_angle_start, d.bond_idx, d.bond_k,
                   d.bond_r0, d.angle_idx, d.angle_k, d.angle_th0, d.mass, d.tether_k, d.tiles, s->Q, s->Pm, s->coef,
                   s->d_Tc, s->pos4, s->Fs, s->cent4, s->cref, s->pair_tab, s->cell_of, s->cell_count, s->cell_start,
-                  s->cell_cursor, s->cell_tmp, s->order, s->rank, s->nbr, s->nbr_count, s->d2max, s->counters,
+                  s->cell_cursor, s->cell_tmp, s->order, s->rank, s->nbr, s->nbr16, s->nbr_count, s->d2max, s->counters,
                   s->red, s->obs, s->gamma, s->Hf, s->hk, s->H4, s->Fc, s->vseg, s->tw, s->atoms_by_type,
                   s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p};
   for (void *p : ptrs) if (p) cudaFree(p);
@@ -457,9 +458,7 @@ extern "C" int qhp_observables(qhp_system *s, double *out, int n_out) {
   if (rc) return rc;
   rc = qhp_nm_observe(s);
   if (rc) return rc;
-  int NB, L; unsigned gx, gy;
-  const int n_pair = qhp_pair_geometry(s, &NB, &L, &gx, &gy);
-  rc = qhp_nm_observe_final(s, n_pair);
+  rc = qhp_nm_observe_final(s, qhp_pair_partials(s));
   if (rc) return rc;
   QHP_CUDA_OK(s, cudaMemcpyAsync(out, s->obs, sizeof(double) * std::min(n_out, 4), cudaMemcpyDeviceToDevice, s->stream));
   return QHP_OK;
@@ -549,6 +548,7 @@ extern "C" int qhp_check(qhp_system *s) {
     int64_t c[8];
     QHP_CUDA_OK(s, cudaMemcpy(c, s->counters, sizeof(c), cudaMemcpyDeviceToHost));
     if (c[1]) { s->err = "neighbour table overflow: a row exceeded its capacity"; return QHP_ESTATE; }
+    if (c[7]) { s->err = "staged pair kernel: a 27-cell neighbourhood outgrew shared memory between list builds"; return QHP_ESTATE; }
     if (c[6]) { s->err = "skin too small: a contracted bead is farther than skin/2 from its centroid, the centroid list cannot cover it"; return QHP_ESTATE; }
   }
   return QHP_OK;

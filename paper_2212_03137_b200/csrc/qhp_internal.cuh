@@ -17,6 +17,7 @@
 
 #define QHP_MAX_P 32
 #define QHP_MAX_TYPES 8
+#define QHP_NPOLY 18   // degree-17 polynomials of the damped Coulomb kernel (pair.cu)
 
 // Philox stream tags
 #define QHP_TAG_PILE 3u
@@ -82,6 +83,14 @@ struct qhp_system {
   int32_t *cell_tmp = nullptr, *order = nullptr, *rank = nullptr;
   int32_t *nbr = nullptr, *nbr_count = nullptr;
   int64_t nbr_stride = 0;
+  // staged pair kernel (pair.cu): one CTA stages the 27-cell neighbourhood of a cell in shared
+  // memory; the list then holds 16-bit indices into that staged array instead of slots
+  bool staged_ok = false;                  // geometry allows it (>= 4 cells per dimension, polynomial fits)
+  bool staged = false;                     // in use (decided at the synchronising list build)
+  uint16_t *nbr16 = nullptr;               // [N][nbr_stride]
+  int staged_cap = 0;                      // staged atoms that fit in shared memory
+  int staged_split = 1;                    // CTAs per (cell, bead)
+  double polyS[QHP_NPOLY]{}, polyE[QHP_NPOLY]{};   // alpha^3 S(w), alpha E(w) in u = 2 r^2/rc^2 - 1
   unsigned long long *d2max = nullptr;     // [2] double bits, max |xc - cref|^2, double-buffered by step parity
   int64_t *counters = nullptr;             // [8] device: 0 rebuilds, 1 overflow flag, 2 max row count, 3 in-cutoff count, 6 skin-too-small flag
   double *red = nullptr;                   // scratch for reductions
@@ -134,6 +143,8 @@ int qhp_cells_rebuild(qhp_system *s, bool force);   // early-exits on device unl
 int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, int64_t *total_host);
 // pair.cu
 int qhp_pair_forces(qhp_system *s, bool energy);     // pos4 -> Fs (+ U_s, count into obs/counters)
+int qhp_pair_setup(qhp_system *s);                   // polynomial tables, staged-kernel geometry
+int qhp_pair_partials(const qhp_system *s);          // upper bound of per-CTA energy partials
 // qtb.cu
 int qhp_qtb_init(qhp_system *s);
 int qhp_qtb_generate(qhp_system *s, int64_t seg);
