@@ -8,7 +8,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libqhp.so")
+_LIB_PATH = os.environ.get("QHP_LIB") or os.path.join(_HERE, "libqhp.so")   # QHP_LIB: another build of the same library
 
 QHP_THERMO_NONE, QHP_THERMO_PILE, QHP_THERMO_ADQTB = 0, 1, 2
 _STATUS = {0: "QHP_OK", -1: "QHP_EINVAL", -2: "QHP_ENOMEM", -3: "QHP_ECUDA", -4: "QHP_ESTATE"}

@@ -31,16 +31,17 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not stale():
+def build(force: bool = False, verbose: bool = False, extra=(), lib: str = LIB, objdir: str = "build") -> str:
+    """extra: more nvcc flags (e.g. -DSTG_THREADS=512) for an experimental build written to `lib`."""
+    if not force and not extra and not stale():
         return LIB
     objs = []
     procs = []
-    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    os.makedirs(os.path.join(HERE, objdir), exist_ok=True)
     for src in sources():
-        obj = os.path.join(HERE, "build", os.path.basename(src)[:-3] + ".o")
+        obj = os.path.join(HERE, objdir, os.path.basename(src)[:-3] + ".o")
         objs.append(obj)
-        procs.append((src, subprocess.Popen([NVCC, *FLAGS, "-c", src, "-o", obj],
+        procs.append((src, subprocess.Popen([NVCC, *FLAGS, *extra, "-c", src, "-o", obj],
                                             stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     log = []
     for src, p in procs:
@@ -49,12 +50,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if p.returncode != 0:
             sys.stderr.write("".join(log))
             raise RuntimeError(f"nvcc failed on {src}")
-    with open(os.path.join(HERE, "build", "ptxas.log"), "w") as fh:
+    with open(os.path.join(HERE, objdir, "ptxas.log"), "w") as fh:
         fh.write("".join(log))
     if verbose:
         print("".join(log))
-    subprocess.check_call([NVCC, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
-    return LIB
+    subprocess.check_call([NVCC, "-shared", "-o", lib, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    return lib
 
 
 if __name__ == "__main__":

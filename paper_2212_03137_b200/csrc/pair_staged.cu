@@ -26,7 +26,9 @@
 
 #include "qhp_internal.cuh"
 
-#define STG_THREADS 512
+#ifndef STG_THREADS
+#define STG_THREADS 768
+#endif
 #define STG_WARPS (STG_THREADS / 32)
 #define STG_QUEUE 64
 
@@ -73,7 +75,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   float4 *sf = reinterpret_cast<float4 *>(sz + a.cap);
   double *tab = reinterpret_cast<double *>(sf + a.cap);
   uint32_t *queue = reinterpret_cast<uint32_t *>(tab + QHP_MAX_TYPES * QHP_MAX_TYPES * 4);
-  __shared__ int off[28], cbeg[27];
+  __shared__ int off[28], cbeg[27], next_atom;
   __shared__ double su[STG_WARPS];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -92,6 +94,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   }
   __syncthreads();
   if (tid == 0) {
+    next_atom = 0;
     off[0] = 0;
     for (int s = 0; s < 27; ++s) off[s + 1] += off[s];
   }
@@ -124,14 +127,36 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   double U = 0.0;
   unsigned long long hits = 0;
 
-  for (int ii = part * STG_WARPS + warp; ii < nh; ii += STG_WARPS * a.split) {
+  // Atoms of the home cell are handed to the warps dynamically (the CTAs of one cell take the atoms
+  // ii = part, part + split, ...); each atom is summed by one warp in a fixed order, so the result
+  // does not depend on which warp took it.  The list row is read in blocks of 256 entries (one
+  // 16-byte load per lane, lane l holding entries 8l..8l+7 of the block); the next block -- of this
+  // row or of the next atom's row -- is in flight while the current one is processed.
+  auto grab = [&]() {
+    int t = 0;
+    if (lane == 0) t = atomicAdd(&next_atom, 1);
+    return part + a.split * __shfl_sync(0xffffffffu, t, 0);
+  };
+  auto load_block = [&](int ii, int m) {
+    const long long k = 256LL * m + 8 * lane;
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (k < a.stride) v = *reinterpret_cast<const uint4 *>(a.nbr16 + (slot0 + ii) * a.stride + k);
+    return v;
+  };
+
+  int ii = grab();
+  int n = (ii < nh) ? a.nbr_count[slot0 + ii] : 0;
+  uint4 cur = make_uint4(0u, 0u, 0u, 0u), nxt = cur;
+  if (ii < nh) cur = load_block(ii, 0);
+  int ii_n = grab();
+  int n_n = (ii_n < nh) ? a.nbr_count[slot0 + ii_n] : 0;
+
+  while (ii < nh) {
     const int ei = h0 + ii;
     const long long slot = slot0 + ii;
     const float4 fi = sf[ei];
     const double xi = sx[ei], yi = sy[ei], zi = sz[ei];
     const int ti = __float_as_int(fi.w);
-    const int n = a.nbr_count[slot];
-    const uint16_t *row = a.nbr16 + slot * a.stride;
     double Fx = 0.0, Fy = 0.0, Fz = 0.0;
     int qn = 0;
 
@@ -162,26 +187,34 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       }
     };
 
-    uint32_t enext = (lane < n) ? row[lane] : 0u;
-    for (int k0 = 0; k0 < n; k0 += 32) {
-      const bool valid = k0 + lane < n;
-      const uint32_t e = enext;
-      const int kn = k0 + 32 + lane;
-      enext = (kn < n) ? row[kn] : 0u;
-      const float4 pj = sf[e];
-      const float dxf = fi.x - pj.x, dyf = fi.y - pj.y, dzf = fi.z - pj.z;
-      const float r2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
-      const bool hit = valid && r2f < a.rc2f;
-      const unsigned mask = __ballot_sync(0xffffffffu, hit);
-      if (hit) q[qn + __popc(mask & lt)] = e | ((uint32_t)__float_as_int(pj.w) << 16);
-      qn += __popc(mask);
-      __syncwarp();
-      if (qn >= 32) {
-        qn -= 32;
-        eval(q[qn + lane], true);
+    int m = 0;
+    do {                                               // blocks of this row (at least one pass: n may be 0)
+      if (256 * (m + 1) < n) nxt = load_block(ii, m + 1);
+      else if (ii_n < nh) nxt = load_block(ii_n, 0);
+      const int kb = 256 * m + 8 * lane;
+      uint4 b = cur;
+      for (int j = 0; j < 8 && 256 * m + j < n; ++j) {
+        const uint32_t e = b.x & 0xffffu;
+        b.x = __funnelshift_r(b.x, b.y, 16); b.y = __funnelshift_r(b.y, b.z, 16);
+        b.z = __funnelshift_r(b.z, b.w, 16); b.w >>= 16;
+        const bool valid = kb + j < n;
+        const float4 pj = sf[valid ? e : 0u];
+        const float dxf = fi.x - pj.x, dyf = fi.y - pj.y, dzf = fi.z - pj.z;
+        const float r2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
+        const bool hit = valid && r2f < a.rc2f;
+        const unsigned mask = __ballot_sync(0xffffffffu, hit);
+        if (hit) q[qn + __popc(mask & lt)] = e | ((uint32_t)__float_as_int(pj.w) << 16);
+        qn += __popc(mask);
         __syncwarp();
+        if (qn >= 32) {
+          qn -= 32;
+          eval(q[qn + lane], true);
+          __syncwarp();
+        }
       }
-    }
+      cur = nxt;
+      ++m;
+    } while (256 * m < n);
     if (qn > 0) {
       const bool act = lane < qn;
       eval(act ? q[lane] : (uint32_t)ei, act);
@@ -197,6 +230,9 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       double *o = a.Fs + ((long long)bead * a.N + slot) * 3;
       o[0] = Fx; o[1] = Fy; o[2] = Fz;
     }
+    ii = ii_n; n = n_n;
+    ii_n = grab();
+    n_n = (ii_n < nh) ? a.nbr_count[slot0 + ii_n] : 0;
   }
   if (ENERGY) {
 #pragma unroll
