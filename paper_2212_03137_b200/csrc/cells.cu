@@ -194,12 +194,18 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
           const unsigned mask = __ballot_sync(0xffffffffu, hit);
           if (hit && nbr) {
             const int pos = cnt + __popc(mask & lt);
-            if (pos < stride) nbr[i * stride + pos] = (uint16_t)(off + k - b);
+            if (pos < stride) nbr[i * stride + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)(off + k - b);
           }
           cnt += __popc(mask);
         }
         off += e - b;
       }
+  if (nbr) {
+    // pad the last 256-entry block with index 0 (a valid staged index; the kernel masks these lanes)
+    const int n = (int)min((long long)cnt, stride), end = (int)min((long long)((n + 255) & ~255), stride);
+    for (int pos = n + lane; pos < end; pos += 32)
+      nbr[i * stride + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = 0;
+  }
   if (lane == 0) {
     if (nbr) {
       nbr_count[i] = (int)min((long long)cnt, stride);
@@ -251,7 +257,7 @@ __global__ void k_export_fill16(const CellArgs a, const int32_t *__restrict__ ce
   const long long s0 = start[at];
   for (int k0 = 0; k0 < n; k0 += 32) {
     const int k = k0 + lane;
-    const int loc = k < n ? (int)nbr[i * stride + k] : 0;
+    const int loc = k < n ? (int)nbr[i * stride + (k & ~255) + ((k & 31) << 3) + ((k & 255) >> 5)] : 0;
     int off = 0, slot = -1;
     for (int s = 0; s < 27; ++s) {
       const int b = __shfl_sync(0xffffffffu, cb, s), c = __shfl_sync(0xffffffffu, cn, s);
@@ -325,14 +331,13 @@ int qhp_cells_rebuild(qhp_system *s, bool force) {
       QHP_CUDA_OK(s, cudaMemcpyAsync(&mx, &s->counters[2], sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
       QHP_CUDA_OK(s, cudaMemcpyAsync(&region, &s->counters[5], sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
       QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
-      if (!s->staged || region + region / 16 + 32 <= s->staged_cap) break;
+      if (!s->staged || qhp_pair_staged_fit(s, region)) break;
       s->staged = false;                               // too dense: generic kernel and 32-bit list
     }
     const bool have = s->staged ? (s->nbr16 != nullptr) : (s->nbr != nullptr);
     if (!have || mx + 8 > s->nbr_stride) {
       int64_t stride = (int64_t)((double)mx * 1.4) + 32;
-      stride = (stride + 31) / 32 * 32;
-      if (stride > s->N) stride = (s->N + 31) / 32 * 32;
+      stride = (stride + 255) / 256 * 256;                 // whole 256-entry row blocks (pair_staged.cu)
       if (stride < 4) stride = 4;
       if (s->nbr) cudaFree(s->nbr);
       if (s->nbr16) cudaFree(s->nbr16);

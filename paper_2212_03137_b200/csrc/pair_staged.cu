@@ -27,10 +27,11 @@
 #include "qhp_internal.cuh"
 
 #ifndef STG_THREADS
-#define STG_THREADS 768
+#define STG_THREADS 768           // largest CTA; the host launches fewer warps when shared memory is short
 #endif
-#define STG_WARPS (STG_THREADS / 32)
-#define STG_QUEUE 64
+#define STG_MAX_WARPS (STG_THREADS / 32)
+#define STG_BLOCK 256             // list entries per row block (8 per lane)
+#define STG_QUEUE (STG_BLOCK + 32)
 
 struct StagedArgs {
   int N, Pc, nt, split, cap;
@@ -38,7 +39,7 @@ struct StagedArgs {
   double box[3], inv_box[3], cell_edge[3];
   const double *pos4;            // [Pc][N] (x, y, z, type bits), slot order
   double *Fs;                    // [Pc][N][3]
-  const uint16_t *nbr16;         // [N][stride] indices into the staged array of the row's cell
+  const uint16_t *nbr16;         // [N][stride] indices into the staged array of the row's cell (blocked, see below)
   const int32_t *nbr_count, *cell_start;
   long long stride;
   const double *pair_tab;        // [nt*nt][4] = qq, 4 eps, sigma^2, LJ shift
@@ -67,22 +68,25 @@ __device__ __forceinline__ double poly17(const double *c, double u) {
   return fma(b, u, a);
 }
 
+// Row layout of the 16-bit table (written by k_list_build16, cells.cu): the entry of rank `pos` in a
+// row sits at (pos / 256) * 256 + (pos % 32) * 8 + (pos % 256) / 32, i.e. one 16-byte load per lane
+// brings entries pos = 256 m + 32 j + lane, j = 0..7; rows are padded with index 0 up to a multiple
+// of 256 entries.
 template <bool ENERGY>
 __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double *sx = reinterpret_cast<double *>(smem_raw);
-  double *sy = sx + a.cap, *sz = sy + a.cap;
-  float4 *sf = reinterpret_cast<float4 *>(sz + a.cap);
+  double *sp = reinterpret_cast<double *>(smem_raw);                  // [cap][3] fp64, cell-centred
+  float4 *sf = reinterpret_cast<float4 *>(sp + 3 * (size_t)a.cap);    // [cap] fp32 copy + type bits
   double *tab = reinterpret_cast<double *>(sf + a.cap);
   uint32_t *queue = reinterpret_cast<uint32_t *>(tab + QHP_MAX_TYPES * QHP_MAX_TYPES * 4);
   __shared__ int off[28], cbeg[27], next_atom;
-  __shared__ double su[STG_WARPS];
+  __shared__ double su[STG_MAX_WARPS];
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = blockDim.x;
   const int cell = blockIdx.x / a.split, part = blockIdx.x % a.split, bead = blockIdx.y;
   const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
 
-  for (int k = tid; k < a.nt * a.nt * 4; k += STG_THREADS) tab[k] = a.pair_tab[k];
+  for (int k = tid; k < a.nt * a.nt * 4; k += nthr) tab[k] = a.pair_tab[k];
   if (tid < 27) {
     // same stencil order as the list build (cells.cu k_list_build16)
     const int ox = tid / 9, oy = (tid / 3) % 3, oz = tid % 3;
@@ -108,7 +112,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   // ---- stage the neighbourhood in coordinates relative to the cell centre ------------------------
   const double ctr[3] = {(cx + 0.5) * a.cell_edge[0], (cy + 0.5) * a.cell_edge[1], (cz + 0.5) * a.cell_edge[2]};
   const double4 *pos = reinterpret_cast<const double4 *>(a.pos4) + (long long)bead * a.N;
-  for (int g = tid; g < total; g += STG_THREADS) {
+  for (int g = tid; g < total; g += nthr) {
     int s = 0;
     while (g >= off[s + 1]) ++s;
     const double4 p = pos[cbeg[s] + g - off[s]];
@@ -116,38 +120,34 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
     lx = fma(-a.box[0], rint(lx * a.inv_box[0]), lx);
     ly = fma(-a.box[1], rint(ly * a.inv_box[1]), ly);
     lz = fma(-a.box[2], rint(lz * a.inv_box[2]), lz);
-    sx[g] = lx; sy[g] = ly; sz[g] = lz;
+    sp[3 * g] = lx; sp[3 * g + 1] = ly; sp[3 * g + 2] = lz;
     sf[g] = make_float4((float)lx, (float)ly, (float)lz, __int_as_float((int)__double_as_longlong(p.w)));
   }
   __syncthreads();
 
   const int h0 = off[13], nh = off[14] - off[13], slot0 = cbeg[13];
-  uint32_t *q = queue + warp * STG_QUEUE;
+  uint32_t *ql = queue + warp * STG_QUEUE + lane;          // this lane's view of the warp's queue
   const unsigned lt = (1u << lane) - 1u;
   double U = 0.0;
   unsigned long long hits = 0;
 
   // Atoms of the home cell are handed to the warps dynamically (the CTAs of one cell take the atoms
   // ii = part, part + split, ...); each atom is summed by one warp in a fixed order, so the result
-  // does not depend on which warp took it.  The list row is read in blocks of 256 entries (one
-  // 16-byte load per lane, lane l holding entries 8l..8l+7 of the block); the next block -- of this
-  // row or of the next atom's row -- is in flight while the current one is processed.
+  // does not depend on which warp took it.  The next row block -- of this row or of the next atom's
+  // row -- is in flight while the current one is processed.
   auto grab = [&]() {
     int t = 0;
     if (lane == 0) t = atomicAdd(&next_atom, 1);
     return part + a.split * __shfl_sync(0xffffffffu, t, 0);
   };
   auto load_block = [&](int ii, int m) {
-    const long long k = 256LL * m + 8 * lane;
-    uint4 v = make_uint4(0u, 0u, 0u, 0u);
-    if (k < a.stride) v = *reinterpret_cast<const uint4 *>(a.nbr16 + (slot0 + ii) * a.stride + k);
-    return v;
+    return *reinterpret_cast<const uint4 *>(a.nbr16 + (slot0 + ii) * a.stride + STG_BLOCK * m + 8 * lane);
   };
 
   int ii = grab();
   int n = (ii < nh) ? a.nbr_count[slot0 + ii] : 0;
   uint4 cur = make_uint4(0u, 0u, 0u, 0u), nxt = cur;
-  if (ii < nh) cur = load_block(ii, 0);
+  if (ii < nh && n > 0) cur = load_block(ii, 0);
   int ii_n = grab();
   int n_n = (ii_n < nh) ? a.nbr_count[slot0 + ii_n] : 0;
 
@@ -155,25 +155,26 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
     const int ei = h0 + ii;
     const long long slot = slot0 + ii;
     const float4 fi = sf[ei];
-    const double xi = sx[ei], yi = sy[ei], zi = sz[ei];
-    const int ti = __float_as_int(fi.w);
+    const double xi = sp[3 * ei], yi = sp[3 * ei + 1], zi = sp[3 * ei + 2];
+    const double *tab_i = tab + __float_as_int(fi.w) * a.nt * 4;
     double Fx = 0.0, Fy = 0.0, Fz = 0.0;
     int qn = 0;
 
+    // one pair per lane, fp64: LJ + damped-shifted-force Coulomb (oracle O3)
     auto eval = [&](uint32_t entry, bool active) {
-      const int e = entry & 0xffffu, tj = entry >> 16;
-      const double dx = xi - sx[e], dy = yi - sy[e], dz = zi - sz[e];
+      const double *pj = sp + 3 * (entry & 0xffffu);
+      const double *pt = tab_i + 4 * (entry >> 16);
+      const double dx = xi - pj[0], dy = yi - pj[1], dz = zi - pj[2];
       const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-      const bool in = active && r2 < a.rc2;          // the fp64 test decides (oracle O3)
+      const bool in = active && r2 < a.rc2;          // the fp64 test decides
       const double r2s = in ? r2 : a.rc2;
-      const double *pt = tab + (ti * a.nt + tj) * 4;
-      const double qq = pt[0], eps4 = pt[1], sig2 = pt[2];
+      const double qq = pt[0], eps4 = pt[1];
       const double y = rsqrt_seeded(r2s), y2 = y * y, y3 = y2 * y;
       const double u = fma(r2s, a.u_scale, -1.0);
       double fr = qq * fma(-a.fshift, y, y3 - poly17(a.cS, u));
       double s6 = 0.0;
       if (__any_sync(0xffffffffu, eps4 != 0.0)) {
-        const double s2 = sig2 * y2;
+        const double s2 = pt[2] * y2;
         s6 = s2 * s2 * s2;
         fr = fma(6.0 * eps4 * y2, fma(2.0 * s6, s6, -s6), fr);
       }
@@ -187,37 +188,35 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       }
     };
 
-    int m = 0;
-    do {                                               // blocks of this row (at least one pass: n may be 0)
-      if (256 * (m + 1) < n) nxt = load_block(ii, m + 1);
-      else if (ii_n < nh) nxt = load_block(ii_n, 0);
-      const int kb = 256 * m + 8 * lane;
-      uint4 b = cur;
-      for (int j = 0; j < 8 && 256 * m + j < n; ++j) {
-        const uint32_t e = b.x & 0xffffu;
-        b.x = __funnelshift_r(b.x, b.y, 16); b.y = __funnelshift_r(b.y, b.z, 16);
-        b.z = __funnelshift_r(b.z, b.w, 16); b.w >>= 16;
-        const bool valid = kb + j < n;
-        const float4 pj = sf[valid ? e : 0u];
+    for (int m = 0; STG_BLOCK * m < n; ++m) {
+      if (STG_BLOCK * (m + 1) < n) nxt = load_block(ii, m + 1);
+      else if (ii_n < nh && n_n > 0) nxt = load_block(ii_n, 0);
+      // ---- check: fp32 pre-test of 8 x 32 entries, survivors compacted into the queue ----------------
+      const int left = n - STG_BLOCK * m - lane;           // entry j of this lane is real iff 32 j < left
+      const uint32_t w[4] = {cur.x, cur.y, cur.z, cur.w};
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const uint32_t e = (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
+        const float4 pj = sf[e];
         const float dxf = fi.x - pj.x, dyf = fi.y - pj.y, dzf = fi.z - pj.z;
         const float r2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
-        const bool hit = valid && r2f < a.rc2f;
+        const bool hit = (32 * j < left) && r2f < a.rc2f;
         const unsigned mask = __ballot_sync(0xffffffffu, hit);
-        if (hit) q[qn + __popc(mask & lt)] = e | ((uint32_t)__float_as_int(pj.w) << 16);
+        if (hit) ql[qn + __popc(mask & lt) - lane] = e | ((uint32_t)__float_as_int(pj.w) << 16);
         qn += __popc(mask);
-        __syncwarp();
-        if (qn >= 32) {
-          qn -= 32;
-          eval(q[qn + lane], true);
-          __syncwarp();
-        }
       }
+      __syncwarp();
+      // ---- eval: full warps of survivors ---------------------------------------------------------------
+      while (qn >= 32) {
+        qn -= 32;
+        eval(ql[qn], true);
+      }
+      __syncwarp();
       cur = nxt;
-      ++m;
-    } while (256 * m < n);
+    }
     if (qn > 0) {
       const bool act = lane < qn;
-      eval(act ? q[lane] : (uint32_t)ei, act);
+      eval(act ? ql[0] : (uint32_t)ei, act);
       __syncwarp();
     }
 #pragma unroll
@@ -230,6 +229,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       double *o = a.Fs + ((long long)bead * a.N + slot) * 3;
       o[0] = Fx; o[1] = Fy; o[2] = Fz;
     }
+    if (n == 0 && ii_n < nh && n_n > 0) cur = load_block(ii_n, 0);   // nothing was prefetched for an empty row
     ii = ii_n; n = n_n;
     ii_n = grab();
     n_n = (ii_n < nh) ? a.nbr_count[slot0 + ii_n] : 0;
@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
     __syncthreads();
     if (tid == 0) {
       double s = 0.0;
-      for (int k = 0; k < STG_WARPS; ++k) s += su[k];
+      for (int k = 0; k < (int)(blockDim.x >> 5); ++k) s += su[k];
       a.part[(long long)blockIdx.y * gridDim.x + blockIdx.x] = s;
     }
   }
@@ -305,9 +305,9 @@ static long double fit_poly(int which, long double wmax, long double scale, doub
   return worst;
 }
 
-static size_t staged_smem_bytes(int cap) {
+static size_t staged_smem_bytes(int cap, int warps) {
   return (size_t)cap * (3 * sizeof(double) + sizeof(float4)) + sizeof(double) * QHP_MAX_TYPES * QHP_MAX_TYPES * 4 +
-         sizeof(uint32_t) * STG_WARPS * STG_QUEUE;
+         sizeof(uint32_t) * (size_t)warps * STG_QUEUE;
 }
 
 // decide whether the staged kernel can serve this system and fit the polynomial tables
@@ -322,21 +322,17 @@ int qhp_pair_setup(qhp_system *s) {
   if (!(eS < 2e-14L && eE < 2e-14L)) return QHP_OK;
   int max_smem = 0;
   QHP_CUDA_OK(s, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device));
-  const size_t fixed = staged_smem_bytes(0) + 1024;                    // + static shared
-  if ((size_t)max_smem <= fixed) return QHP_OK;
-  int cap = (int)(((size_t)max_smem - fixed) / (3 * sizeof(double) + sizeof(float4)));
-  if (cap > 65535) cap = 65535;                                        // 16-bit list entries
-  cap &= ~1;
-  s->staged_cap = cap;
-  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)staged_smem_bytes(cap)));
-  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)staged_smem_bytes(cap)));
+  s->staged_smem_max = max_smem - 1024;                                // room for the static shared variables
+  if (s->staged_smem_max < 64 * 1024) return QHP_OK;
+  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->staged_smem_max));
+  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->staged_smem_max));
   // CTAs per (cell, bead): aim at >= 6 waves of one CTA per SM, keep >= one atom per warp
   int sms = 148;
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device);
   long long ctas = (long long)s->ncell * s->Pc;
   int split = (int)((6LL * sms + ctas - 1) / ctas);
   const int per_cell = s->N / s->ncell + 1;
-  while (split > 1 && per_cell / split < STG_WARPS) --split;
+  while (split > 1 && per_cell / split < STG_MAX_WARPS) --split;
   if (split < 1) split = 1;
   if (split > 8) split = 8;
   s->staged_split = split;
@@ -345,6 +341,22 @@ int qhp_pair_setup(qhp_system *s) {
 }
 
 int qhp_pair_staged_partials(const qhp_system *s) { return s->ncell * 8 * s->Pc; }
+
+// Largest CTA (in warps) whose queues leave room for `region` staged atoms (+ 1/16 for drift between
+// list builds); sets staged_warps / staged_cap.  False: the neighbourhood does not fit at all.
+bool qhp_pair_staged_fit(qhp_system *s, long long region) {
+  static const int tries[] = {STG_MAX_WARPS, 16, 12, 8};
+  const long long need = region + region / 16 + 32;
+  for (int w : tries) {
+    if (w > STG_MAX_WARPS) continue;
+    const long long room = (long long)s->staged_smem_max - (long long)staged_smem_bytes(0, w);
+    long long cap = room / (long long)(3 * sizeof(double) + sizeof(float4));
+    if (cap > 65534) cap = 65534;                                      // 16-bit list entries
+    cap &= ~1LL;
+    if (cap >= need) { s->staged_warps = w; s->staged_cap = (int)cap; return true; }
+  }
+  return false;
+}
 
 int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned long long *count) {
   StagedArgs a{};
@@ -370,9 +382,10 @@ int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned lo
   for (int k = 0; k < QHP_NPOLY; ++k) { a.cS[k] = s->polyS[k]; a.cE[k] = s->polyE[k]; }
   a.part = part; a.count = count; a.counters = (long long *)s->counters;
   const dim3 grid((unsigned)(s->ncell * s->staged_split), (unsigned)s->Pc);
-  const size_t smem = staged_smem_bytes(s->staged_cap);
-  if (energy) k_pair_staged<true><<<grid, STG_THREADS, smem, s->stream>>>(a);
-  else k_pair_staged<false><<<grid, STG_THREADS, smem, s->stream>>>(a);
+  const size_t smem = staged_smem_bytes(s->staged_cap, s->staged_warps);
+  const int threads = 32 * s->staged_warps;
+  if (energy) k_pair_staged<true><<<grid, threads, smem, s->stream>>>(a);
+  else k_pair_staged<false><<<grid, threads, smem, s->stream>>>(a);
   QHP_LAUNCH_OK(s);
   return QHP_OK;
 }

@@ -89,6 +89,7 @@ struct qhp_system {
   bool staged = false;                     // in use (decided at the synchronising list build)
   uint16_t *nbr16 = nullptr;               // [N][nbr_stride]
   int staged_cap = 0;                      // staged atoms that fit in shared memory
+  int staged_warps = 0, staged_smem_max = 0; // CTA size in use, dynamic shared memory available
   int staged_split = 1;                    // CTAs per (cell, bead)
   double polyS[QHP_NPOLY]{}, polyE[QHP_NPOLY]{};   // alpha^3 S(w), alpha E(w) in u = 2 r^2/rc^2 - 1
   unsigned long long *d2max = nullptr;     // [2] double bits, max |xc - cref|^2, double-buffered by step parity
@@ -144,6 +145,7 @@ int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, i
 // pair.cu
 int qhp_pair_forces(qhp_system *s, bool energy);     // pos4 -> Fs (+ U_s, count into obs/counters)
 int qhp_pair_setup(qhp_system *s);                   // polynomial tables, staged-kernel geometry
+bool qhp_pair_staged_fit(qhp_system *s, long long region);  // CTA size / capacity for a neighbourhood size
 int qhp_pair_partials(const qhp_system *s);          // upper bound of per-CTA energy partials
 // qtb.cu
 int qhp_qtb_init(qhp_system *s);
