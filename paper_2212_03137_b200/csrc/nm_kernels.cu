@@ -102,11 +102,66 @@ __device__ __forceinline__ double bonded_molecule(const IntArgs &a, int m, int a
   return U;
 }
 
+// x_i = sqrt(P) sum_n T_in Q_n for one DOF (Eq. 4).  The bead loop is rolled (its index is
+// warp-uniform, so the coefficients come through the constant bank / uniform registers) and the
+// mode sum runs in four independent partial sums; a fully unrolled P x P body overflowed the
+// instruction cache at P = 32.
+template <int P>
+__device__ __forceinline__ void modes_to_beads_tile(const NmTab<P> &tab, const double (&Qr)[P], double *xt, double *ft,
+                                                    int TD, int t) {
+  const double sp = sqrt((double)P);
+#pragma unroll 1
+  for (int i = 0; i < P; ++i) {
+    double s[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int n = 0; n < P; ++n) s[n & 3] = fma(tab.T[i * P + n], Qr[n], s[n & 3]);
+    xt[i * TD + t] = sp * ((s[0] + s[1]) + (s[2] + s[3]));
+    ft[i * TD + t] = 0.0;
+  }
+}
+
+// fr[n] = (1/sqrt P) sum_i T_in F^f_i (Eq. 10-11) + (1/sqrt P') sum_j T'_jn Fs_j (n < P'), one DOF
+template <int P>
+__device__ __forceinline__ void project_forces_tile(const IntArgs &a, const NmTab<P> &tab, const NmTab<P> &ctab,
+                                                    const double *ft, int TD, int t, int atom, int c, double (&fr)[P]) {
+#pragma unroll
+  for (int n = 0; n < P; ++n) fr[n] = 0.0;
+#pragma unroll 1
+  for (int i = 0; i < P; ++i) {
+    const double Fi = ft[i * TD + t];
+#pragma unroll
+    for (int n = 0; n < P; ++n) fr[n] = fma(tab.T[i * P + n], Fi, fr[n]);
+  }
+  const double isp = 1.0 / sqrt((double)P);
+#pragma unroll
+  for (int n = 0; n < P; ++n) fr[n] *= isp;
+  // slow forces of the contracted beads, chain rule on Eq. 20
+  const int Pc = a.Pc;
+  const double ispc = 1.0 / sqrt((double)Pc);
+  const long long slot = a.rank[atom];
+  for (int j = 0; j < Pc; ++j) {
+    const double Fj = a.Fs[((long long)j * a.N + slot) * 3 + c] * ispc;
+#pragma unroll
+    for (int n = 0; n < P; ++n)
+      if (n < Pc) fr[n] = fma(ctab.T[j * Pc + n], Fj, fr[n]);
+  }
+}
+
+// V_f of every (molecule, bead) of the tile: positions in xt, forces accumulated into ft
+__device__ __forceinline__ double bonded_tile(const IntArgs &a, const qhp_tile tl, int P, const double *xt, double *ft) {
+  double U = 0.0;
+  const int nm = tl.m1 - tl.m0, TD = a.TD;
+  for (int w = threadIdx.x; w < nm * P; w += blockDim.x) {
+    const int m = tl.m0 + w % nm, bead = w / nm;
+    U += bonded_molecule(a, m, tl.a0, xt + bead * TD, ft + bead * TD);
+  }
+  return U;
+}
+
 // ---------------------------------------------------------------------------------------------
-// Common front end of the integrator / force / observable kernels for one tile:
-//   Qr[n]  <- Q_n of this thread's DOF,
-//   x_i = sqrt(P) sum_n T_in Q_n (Eq. 4) -> shared tile, V_f forces per (molecule, bead),
-//   fr[n] <- (1/sqrt P) sum_i T_in F^f_i (Eq. 10-11) + (1/sqrt P') sum_j T'_jn Fc_j  (n < P').
+// Common front end of the force / observable kernels for one tile:
+//   Qr[n]  <- Q_n of this thread's DOF, x_i -> shared tile, V_f forces per (molecule, bead),
+//   fr[n]  <- projected fast + expanded slow forces.
 // Returns this thread's share of sum_i V_f(x_i).
 // ---------------------------------------------------------------------------------------------
 template <int P>
@@ -115,50 +170,15 @@ __device__ __forceinline__ double tile_forces(const IntArgs &a, const NmTab<P> &
                                               bool active, long long dof, int atom, int c,
                                               double (&Qr)[P], double (&fr)[P]) {
   const int t = threadIdx.x, TD = a.TD;
-  const double sp = sqrt((double)P);
   if (active) {
 #pragma unroll
     for (int n = 0; n < P; ++n) Qr[n] = a.Q[n * a.ND + dof];
-#pragma unroll
-    for (int i = 0; i < P; ++i) {
-      double s = 0.0;
-#pragma unroll
-      for (int n = 0; n < P; ++n) s += tab.T[i * P + n] * Qr[n];
-      xt[i * TD + t] = sp * s;
-      ft[i * TD + t] = 0.0;
-    }
+    modes_to_beads_tile<P>(tab, Qr, xt, ft, TD, t);
   }
   __syncthreads();
-  double U = 0.0;
-  const int nm = tl.m1 - tl.m0;
-  for (int w = t; w < nm * P; w += blockDim.x) {
-    const int m = tl.m0 + w % nm, bead = w / nm;
-    U += bonded_molecule(a, m, tl.a0, xt + bead * TD, ft + bead * TD);
-  }
+  const double U = bonded_tile(a, tl, P, xt, ft);
   __syncthreads();
-  if (active) {
-#pragma unroll
-    for (int n = 0; n < P; ++n) fr[n] = 0.0;
-#pragma unroll
-    for (int i = 0; i < P; ++i) {
-      const double Fi = ft[i * TD + t];
-#pragma unroll
-      for (int n = 0; n < P; ++n) fr[n] += tab.T[i * P + n] * Fi;
-    }
-    const double isp = 1.0 / sp;
-#pragma unroll
-    for (int n = 0; n < P; ++n) fr[n] *= isp;
-    // slow forces of the contracted beads, chain rule on Eq. 20
-    const int Pc = a.Pc;
-    const double ispc = 1.0 / sqrt((double)Pc);
-    const long long slot = a.rank[atom];
-    for (int j = 0; j < Pc; ++j) {
-      const double Fj = a.Fs[((long long)j * a.N + slot) * 3 + c] * ispc;
-#pragma unroll
-      for (int n = 0; n < P; ++n)
-        if (n < Pc) fr[n] += ctab.T[j * Pc + n] * Fj;
-    }
-  }
+  if (active) project_forces_tile<P>(a, tab, ctab, ft, TD, t, atom, c, fr);
   return U;
 }
 
@@ -195,7 +215,7 @@ __device__ __forceinline__ double block_sum(double v, double *scratch) {
 //   do_step  : B(dt/2) A(dt/2) O(dt) A(dt/2) of this step, then write the contracted positions
 //              of the new Q (slot order) and the list-validity statistic max |xc - cref|^2.
 // ---------------------------------------------------------------------------------------------
-template <int P, int THERMO>
+template <int P, int THERMO, int PCM>   // PCM: compile-time bound on the contracted beads P'
 __global__ void __launch_bounds__(288) k_integrate(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab) {
   extern __shared__ double sm[];
   const int TD = a.TD, t = threadIdx.x;
@@ -208,17 +228,51 @@ __global__ void __launch_bounds__(288) k_integrate(const IntArgs a, const NmTab<
   for (int k = t; k < a.nt * P * QHP_NCOEF; k += blockDim.x) sc[k] = a.coef[k];
   if (blockIdx.x == 0 && t == 0 && a.do_step) a.d2max[(a.step + 1) & 1] = 0ull;
 
-  double Qr[P], fr[P];
-  tile_forces<P>(a, tab, ctab, tl, xt, ft, active, dof, atom, c, Qr, fr);   // syncs inside
-
+  // ---- phase 1: Q -> bead positions (shared tile), V_f per (molecule, bead) -------------------------
+  {
+    double Qr[P];
+    if (active) {
+#pragma unroll
+      for (int n = 0; n < P; ++n) Qr[n] = a.Q[n * a.ND + dof];
+      modes_to_beads_tile<P>(tab, Qr, xt, ft, TD, t);
+    }
+    __syncthreads();
+    bonded_tile(a, tl, P, xt, ft);
+    __syncthreads();
+    // the positions are dead: park this DOF's Q_n in its own column of xt (frees the registers for fr)
+    if (active) {
+#pragma unroll
+      for (int n = 0; n < P; ++n) xt[n * TD + t] = Qr[n];
+    }
+  }
+  // ---- phase 2: normal-mode forces of this DOF ---------------------------------------------------------
+  double fr[P];
+  if (active) project_forces_tile<P>(a, tab, ctab, ft, TD, t, atom, c, fr);
+  // ---- phase 3 (PILE): one Philox call per (atom, mode) gives the three Cartesian normals; they are
+  //      exchanged through the force tile, which is dead once every thread has its fr ---------------------
+  if (THERMO == 1 && a.do_step) {
+    __syncthreads();
+    const int na = tl.a1 - tl.a0;
+    for (int w = t; w < na * P; w += blockDim.x) {
+      const int al = w % na, n = w / na;
+      double z[3];
+      qhp_normals3(a.seed, (uint32_t)(tl.a0 + al), (uint32_t)n, QHP_TAG_PILE, (uint64_t)a.step, z);
+      ft[n * TD + 3 * al] = z[0]; ft[n * TD + 3 * al + 1] = z[1]; ft[n * TD + 3 * al + 2] = z[2];
+    }
+    __syncthreads();
+  }
+  // ---- phase 4: B A O A per mode, contraction of the new positions -----------------------------------------
   double d2 = 0.0;
   if (active) {
     const int ty = a.type[atom];
     const double m = a.mass[ty];
     const double *cf = sc + ty * P * QHP_NCOEF;
+    double xc[PCM];                     // contracted beads (first Pc entries used)
+#pragma unroll
+    for (int j = 0; j < PCM; ++j) xc[j] = 0.0;
 #pragma unroll
     for (int n = 0; n < P; ++n) {
-      double q = Qr[n];
+      double q = xt[n * TD + t];
       double p = a.Pm[n * a.ND + dof];
       if (a.kick_prev) p += a.hA * fr[n];
       if (a.do_step) {
@@ -229,9 +283,7 @@ __global__ void __launch_bounds__(288) k_integrate(const IntArgs a, const NmTab<
         else { const double qn = cs * q + s1 * p; p = s2 * q + cs * p; q = qn; }
         // O(dt)
         if (THERMO == 1) {
-          const double z = qhp_normal_comp(a.seed, (uint32_t)atom, (uint32_t)n, QHP_TAG_PILE,
-                                           (uint64_t)a.step, c);
-          p = cf[n * QHP_NCOEF + 3] * p + cf[n * QHP_NCOEF + 4] * z;
+          p = cf[n * QHP_NCOEF + 3] * p + cf[n * QHP_NCOEF + 4] * ft[n * TD + t];
         } else if (THERMO == 2) {
           // classical BAOAB carrying the coloured force (Eq. 12, l.199; readings G14, G16)
           const long long k = dof * a.n_seg + a.n_loc;
@@ -243,26 +295,28 @@ __global__ void __launch_bounds__(288) k_integrate(const IntArgs a, const NmTab<
         if (n == 0) q += a.hdt * p / m;
         else { const double qn = cs * q + s1 * p; p = s2 * q + cs * p; q = qn; }
         a.Q[n * a.ND + dof] = q;
-        Qr[n] = q;
+        // contraction of the new positions (Eq. 20): only the first Pc modes contribute
+        if (n < PCM && n < a.Pc) {
+#pragma unroll
+          for (int j = 0; j < PCM; ++j)
+            if (j < a.Pc) xc[j] = fma(ctab.T[j * a.Pc + n], q, xc[j]);
+        }
       }
       a.Pm[n * a.ND + dof] = p;
     }
     if (a.do_step) {
-      // contraction of the new positions (Eq. 20) into slot order + list-validity statistic
-      const int Pc = a.Pc;
-      const double spc = sqrt((double)Pc);
+      // contracted positions into slot order + list-validity statistic
+      const double spc = sqrt((double)a.Pc);
       const long long slot = a.rank[atom];
       const double cr = a.cref[dof];
-      for (int j = 0; j < Pc; ++j) {
-        double s = 0.0;
 #pragma unroll
-        for (int n = 0; n < P; ++n)
-          if (n < Pc) s += ctab.T[j * Pc + n] * Qr[n];
-        const double xc = spc * s;
-        a.pos4[((long long)j * a.N + slot) * 4 + c] = xc;
-        const double dd = xc - cr;
-        d2 = fmax(d2, dd * dd);
-      }
+      for (int j = 0; j < PCM; ++j)
+        if (j < a.Pc) {
+          const double x = spc * xc[j];
+          a.pos4[((long long)j * a.N + slot) * 4 + c] = x;
+          const double dd = x - cr;
+          d2 = fmax(d2, dd * dd);
+        }
     }
   }
   if (a.do_step) {
@@ -492,22 +546,24 @@ int qhp_nm_integrate(qhp_system *s, bool kick_prev, bool do_step, int64_t step) 
   }
   const size_t smem = s->int_smem;
   const int thermo = s->th.kind;
+#define LAUNCH_INT(PP, TH, PCM)                                                                  \
+  {                                                                                              \
+    QHP_CUDA_OK(s, set_smem(k_integrate<PP, TH, PCM>, smem));                                    \
+    k_integrate<PP, TH, PCM><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, make_tab<PP>(s->T_P, PP), make_tab<PP>(s->T_Pc, s->Pc)); \
+  }
 #define FN(PP)                                                                                   \
   {                                                                                              \
-    NmTab<PP> tab = make_tab<PP>(s->T_P, PP), ctab = make_tab<PP>(s->T_Pc, s->Pc);               \
-    if (thermo == QHP_THERMO_PILE) {                                                             \
-      QHP_CUDA_OK(s, set_smem(k_integrate<PP, 1>, smem));                                        \
-      k_integrate<PP, 1><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, tab, ctab);        \
-    } else if (thermo == QHP_THERMO_ADQTB) {                                                     \
-      QHP_CUDA_OK(s, set_smem(k_integrate<1, 2>, smem));                                         \
-      k_integrate<1, 2><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, make_tab<1>(s->T_P, 1), make_tab<1>(s->T_Pc, 1)); \
+    constexpr int PC4 = PP < 4 ? PP : 4;                                                         \
+    if (thermo == QHP_THERMO_ADQTB) LAUNCH_INT(1, 2, 1)                                          \
+    else if (thermo == QHP_THERMO_PILE) {                                                        \
+      if (s->Pc <= PC4) LAUNCH_INT(PP, 1, PC4) else LAUNCH_INT(PP, 1, PP)                        \
     } else {                                                                                     \
-      QHP_CUDA_OK(s, set_smem(k_integrate<PP, 0>, smem));                                        \
-      k_integrate<PP, 0><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, tab, ctab);        \
+      if (s->Pc <= PC4) LAUNCH_INT(PP, 0, PC4) else LAUNCH_INT(PP, 0, PP)                        \
     }                                                                                            \
   }
   QHP_DISPATCH_P(s, FN)
 #undef FN
+#undef LAUNCH_INT
   QHP_LAUNCH_OK(s);
   return QHP_OK;
 }

@@ -112,8 +112,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   // ---- stage the neighbourhood in coordinates relative to the cell centre ------------------------
   const double ctr[3] = {(cx + 0.5) * a.cell_edge[0], (cy + 0.5) * a.cell_edge[1], (cz + 0.5) * a.cell_edge[2]};
   const double4 *pos = reinterpret_cast<const double4 *>(a.pos4) + (long long)bead * a.N;
-  for (int g = tid; g < total; g += nthr) {
-    int s = 0;
+  for (int g = tid, s = 0; g < total; g += nthr) {
     while (g >= off[s + 1]) ++s;
     const double4 p = pos[cbeg[s] + g - off[s]];
     double lx = p.x - ctr[0], ly = p.y - ctr[1], lz = p.z - ctr[2];
@@ -196,6 +195,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       const uint32_t w[4] = {cur.x, cur.y, cur.z, cur.w};
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
+        if (32 * j >= n - STG_BLOCK * m) break;            // warp-uniform: the row ends before this step
         const uint32_t e = (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
         const float4 pj = sf[e];
         const float dxf = fi.x - pj.x, dyf = fi.y - pj.y, dzf = fi.z - pj.z;
