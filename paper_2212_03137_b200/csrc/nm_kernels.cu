@@ -215,17 +215,17 @@ __device__ __forceinline__ double block_sum(double v, double *scratch) {
 //   do_step  : B(dt/2) A(dt/2) O(dt) A(dt/2) of this step, then write the contracted positions
 //              of the new Q (slot order) and the list-validity statistic max |xc - cref|^2.
 // ---------------------------------------------------------------------------------------------
+// CTA size and residency: 48-atom tiles (160 threads, three CTAs per SM) for P >= 24, else 96-atom tiles
 template <int P, int THERMO, int PCM>   // PCM: compile-time bound on the contracted beads P'
-__global__ void __launch_bounds__(288) k_integrate(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab) {
+__global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integrate(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab) {
   extern __shared__ double sm[];
   const int TD = a.TD, t = threadIdx.x;
-  double *xt = sm, *ft = sm + P * TD, *sc = ft + P * TD, *scratch = sc + a.nt * P * QHP_NCOEF;
+  double *xt = sm, *ft = sm + P * TD, *scratch = ft + P * TD;
   const qhp_tile tl = a.tiles[blockIdx.x];
   const int nd = 3 * (tl.a1 - tl.a0);
   const bool active = t < nd;
   const long long dof = 3LL * tl.a0 + t;
   const int atom = tl.a0 + t / 3, c = t % 3;
-  for (int k = t; k < a.nt * P * QHP_NCOEF; k += blockDim.x) sc[k] = a.coef[k];
   if (blockIdx.x == 0 && t == 0 && a.do_step) a.d2max[(a.step + 1) & 1] = 0ull;
 
   // ---- phase 1: Q -> bead positions (shared tile), V_f per (molecule, bead) -------------------------
@@ -266,24 +266,33 @@ __global__ void __launch_bounds__(288) k_integrate(const IntArgs a, const NmTab<
   if (active) {
     const int ty = a.type[atom];
     const double m = a.mass[ty];
-    const double *cf = sc + ty * P * QHP_NCOEF;
+    const double *cf = a.coef + ty * P * QHP_NCOEF;   // read-only, L1-resident (two types x P x 6 doubles)
     double xc[PCM];                     // contracted beads (first Pc entries used)
 #pragma unroll
     for (int j = 0; j < PCM; ++j) xc[j] = 0.0;
+    // momenta are fetched eight modes ahead of their use: the stores of one mode must not
+    // serialise the loads of the next (Q and Pm may alias as far as the compiler knows)
+    constexpr int PF = P < 8 ? P : 8;
+    double pl[PF];
 #pragma unroll
     for (int n = 0; n < P; ++n) {
+      if (n % PF == 0) {
+#pragma unroll
+        for (int k = 0; k < PF; ++k)
+          if (n + k < P) pl[k] = a.Pm[(n + k) * a.ND + dof];
+      }
       double q = xt[n * TD + t];
-      double p = a.Pm[n * a.ND + dof];
+      double p = pl[n % PF];
       if (a.kick_prev) p += a.hA * fr[n];
       if (a.do_step) {
         p += a.hA * fr[n];
-        const double cs = cf[n * QHP_NCOEF + 0], s1 = cf[n * QHP_NCOEF + 1], s2 = cf[n * QHP_NCOEF + 2];
+        const double cs = __ldg(cf + n * QHP_NCOEF + 0), s1 = __ldg(cf + n * QHP_NCOEF + 1), s2 = __ldg(cf + n * QHP_NCOEF + 2);
         // A(dt/2): centroid translation / exact free ring-polymer rotation
         if (n == 0) q += a.hdt * p / m;
         else { const double qn = cs * q + s1 * p; p = s2 * q + cs * p; q = qn; }
         // O(dt)
         if (THERMO == 1) {
-          p = cf[n * QHP_NCOEF + 3] * p + cf[n * QHP_NCOEF + 4] * ft[n * TD + t];
+          p = __ldg(cf + n * QHP_NCOEF + 3) * p + __ldg(cf + n * QHP_NCOEF + 4) * ft[n * TD + t];
         } else if (THERMO == 2) {
           // classical BAOAB carrying the coloured force (Eq. 12, l.199; readings G14, G16)
           const long long k = dof * a.n_seg + a.n_loc;
@@ -360,7 +369,7 @@ template <int P>
 __global__ void __launch_bounds__(288) k_observe(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab) {
   extern __shared__ double sm[];
   const int TD = a.TD, t = threadIdx.x;
-  double *xt = sm, *ft = sm + P * TD, *scratch = ft + P * TD + a.nt * P * QHP_NCOEF;
+  double *xt = sm, *ft = sm + P * TD, *scratch = ft + P * TD;
   const qhp_tile tl = a.tiles[blockIdx.x];
   const bool active = t < 3 * (tl.a1 - tl.a0);
   const long long dof = 3LL * tl.a0 + t;
@@ -501,7 +510,7 @@ template <int P> static NmTab<P> make_tab(const std::vector<double> &T, int n) {
 
 static IntArgs make_args(qhp_system *s) {
   IntArgs a{};
-  a.N = s->N; a.Pc = s->Pc; a.nt = s->nt; a.TD = s->tile_threads; a.ND = 3LL * s->N;
+  a.N = s->N; a.Pc = s->Pc; a.nt = s->nt; a.TD = 3 * s->tile_atoms; a.ND = 3LL * s->N;
   a.tiles = s->dt_.tiles; a.Q = s->Q; a.Pm = s->Pm; a.coef = s->coef;
   a.type = s->dt_.type; a.molid = s->dt_.molid; a.mol_atom_start = s->dt_.mol_atom_start;
   a.mol_bond_start = s->dt_.mol_bond_start; a.mol_angle_start = s->dt_.mol_angle_start;
