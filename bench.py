@@ -40,11 +40,33 @@ if ROOT not in sys.path:
 
 from workloads import water as W  # noqa: E402
 
-# algorithmic work of the pair kernel per in-cutoff pair-bead (DESIGN.md "Rooflines"): minimum
+# algorithmic work of the pair kernel per in-cutoff pair-bead (SURVEY.md §8(d), DESIGN.md §6): minimum
 # image + distance 15 flop, DSF Coulomb (rsqrt, exp, erfc) + LJ + force accumulation 95 flop.
 FLOP_PER_PAIR_BEAD = 110.0
-# FP64 ALU peak derived from unit counts: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (max SM clock)
+# FP64 ALU peak derived from unit counts: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (max SM clock);
+# bench.py also measures it live with qhp_dfma_probe and reports both.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_staged<false> launch at C4, from the
+# `ncu --set full` capture summarised in profiles/r1b_summary.md (per launch, like `achieved`)
+NCU_TRAFFIC_BYTES = {("C4", "k_pair_staged"): 1.3636e9 + 2.33e7}
+
+
+def measure_dfma_peak() -> float:
+    """Dependent-FMA probe on every SM (8 chains per thread): measured FP64 FMA throughput, TFLOP/s."""
+    import torch
+    import paper_2212_03137_b200 as qhp
+    grid, block, iters = 148 * 8, 256, 1 << 16
+    qhp.qhp_dfma_probe(grid, block, iters)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best = float("inf")
+    for _ in range(3):
+        e0.record()
+        qhp.qhp_dfma_probe(grid, block, iters)
+        e1.record()
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    return 2.0 * grid * block * iters / (best * 1e-3) / 1e12
 
 
 def workload(name: str) -> dict:
@@ -106,6 +128,24 @@ class ClockSampler:
         if not sm:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
         return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+
+
+def max_over_ranks(x: float, world: int, device: str = "cuda") -> float:
+    """Replicas only: every rank times its own replica; the job's time is the slowest
+    rank's.  One all-reduce(MAX) of a scalar on the job's process group (nccl on GPUs, gloo in the
+    CPU tests)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(world: int, n_atoms: int, P: int, steps: int, seconds: float) -> float:
+    """bead-atom-steps/s of the whole job: all ranks' replicas over the slowest rank's time (weak scaling)."""
+    return world * n_atoms * P * steps / seconds
 
 
 def build_system(cfg: dict):
@@ -232,11 +272,8 @@ def main():
     sysg.profile(False)
     c1 = sysg.counters()
     launches = c1["launches"] - c0["launches"]          # kernels the library launched inside the timed region
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * N * P * K / (ms * 1e-3)
+    ms = max_over_ranks(ms, world)
+    value = job_throughput(world, N, P, K, ms * 1e-3)
     ns_day = K * cfg["dt_fs"] * 1e-6 / (ms * 1e-3) * 86400.0
 
     # ---- roofline of the dominant kernel (pair forces) ------------------------------------------
@@ -246,12 +283,16 @@ def main():
     flops_algo = 0.5 * pair_beads * FLOP_PER_PAIR_BEAD  # algorithmic: every unordered pair-bead once
     ach = flops_algo / (pair_ms * 1e-3) / 1e12 if pair_ms > 0 else 0.0
     pk = peaks()
-    roofline = dict(kernel="k_pair", bound="alu", achieved=ach, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
-                    frac=ach / FP64_PEAK_TFLOPS, traffic=None,
+    kname = "k_pair_staged" if c1.get("staged") else "k_pair"
+    dfma_tf = measure_dfma_peak()
+    roofline = dict(kernel=kname, bound="alu", achieved=ach, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
+                    frac=ach / FP64_PEAK_TFLOPS, traffic=NCU_TRAFFIC_BYTES.get((cfg["name"], kname)),
                     peak_source="derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz",
+                    peak_measured=dfma_tf, frac_of_measured=ach / dfma_tf if dfma_tf > 0 else None,
                     executed_tflops=2.0 * ach, ms_per_launch=pair_ms,
                     note="achieved counts each unordered in-cutoff pair-bead once (110 flop); the kernel "
-                         "evaluates both directions (full list, no atomics), see executed_tflops")
+                         "evaluates both directions (full list, no atomics), see executed_tflops; "
+                         "peak_measured = live qhp_dfma_probe")
     # second kernel: fused integrator pass, HBM-bound: 4 x 8 B per (DOF, bead) + 2 x 24 B * P'/P ... per atom-bead
     int_bytes = 4.0 * 8 * 3 * N * P + (32.0 + 24.0) * N * cfg["P_contract"]
     int_gbs = int_bytes / (int_ms * 1e-3) / 1e9 if int_ms > 0 else 0.0
@@ -259,7 +300,8 @@ def main():
                                     frac=int_gbs / pk["hbm_gbs"], peak_source=pk["source"]),
                    rebuild_chain=dict(ms_per_step=prof["rebuild"]["ms"] / max(prof["rebuild"]["n"], 1),
                                       rebuilds=c1["rebuilds"] - c0["rebuilds"]),
-                   qtb_segment=dict(ms_total=prof["qtb"]["ms"], n=prof["qtb"]["n"]))
+                   qtb_generate=dict(ms_per_segment=prof["qtb_generate"]["ms"] / max(prof["qtb_generate"]["n"], 1), n=prof["qtb_generate"]["n"]),
+                   qtb_adapt=dict(ms_per_segment=prof["qtb_adapt"]["ms"] / max(prof["qtb_adapt"]["n"], 1), n=prof["qtb_adapt"]["n"]))
 
     # ---- e2e through the host entry points ----------------------------------------------------------
     e2e = None
@@ -278,12 +320,9 @@ def main():
         obs = sysg.observables_host()
         torch.cuda.synchronize()
         t_e2e = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([t_e2e], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_e2e = float(t.item())
+        t_e2e = max_over_ranks(t_e2e, world)
         nbytes = xh.numel() * 8
-        e2e = dict(value=world * N * P * K / t_e2e, unit="bead-atom-steps/s",
+        e2e = dict(value=job_throughput(world, N, P, K, t_e2e), unit="bead-atom-steps/s",
                    h2d_bytes_per_step=2 * nbytes / K, d2h_bytes_per_step=(2 * nbytes + 32) / K,
                    ms_total=1e3 * t_e2e, what="set_state_host + qhp_step(K) + get_state_host + observables_host",
                    observables=[float(v) for v in obs])

@@ -134,14 +134,17 @@ int qhp_adqtb_gamma(qhp_system *sys, double *gamma);
 int qhp_adqtb_segment(qhp_system *sys, double *Fc, double *vseg);
 /* Counters for measurement: out_host[0] = neighbour-list rebuilds so far, [1] = list entries,
  * [2] = pair-bead interactions inside r_cut at the current positions (full list, both
- * directions), [3] = list capacity, [4] = kernels launched so far, [5] = error flags (bit 0 list overflow, bit 1 skin < 2 x bead spread).
- * n_out <= 6.  HOST pointer; synchronises. */
+ * directions), [3] = list capacity, [4] = kernels launched so far, [5] = error flags (bit 0 list
+ * overflow, bit 1 skin < 2 x bead spread, bit 2 staged neighbourhood outgrew shared memory),
+ * [6] = 1 if the shared-memory staged pair kernel serves this system (0: generic kernel),
+ * [7] = warps per CTA of the staged kernel.  n_out <= 8.  HOST pointer; synchronises. */
 int qhp_counters(qhp_system *sys, int64_t *out_host, int n_out);
 /* Per-phase device timing with CUDA events recorded on the library stream inside qhp_step:
  * qhp_profile(sys, 1) starts recording (and clears the sums), qhp_profile(sys, 0) stops.
- * qhp_profile_read synchronises and writes ms_host[0..3] = summed milliseconds of
- * {integrator pass, neighbour rebuild chain, pair forces, adQTB segment work} and
- * n_host[0..3] = number of timed intervals of each.  HOST pointers. */
+ * qhp_profile_read synchronises and writes ms_host[0..4] = summed milliseconds of
+ * {integrator pass, neighbour rebuild chain, pair forces, adQTB segment generation (Q2-Q4),
+ * adQTB spectra + adaptation (Q5-Q7)} and n_host[0..4] = number of timed intervals of each.
+ * HOST pointers. */
 int qhp_profile(qhp_system *sys, int enable);
 int qhp_profile_read(qhp_system *sys, double *ms_host, int64_t *n_host);
 /* Synchronise the stream and report sticky CUDA / overflow errors. */

@@ -250,9 +250,10 @@ class System:
         return Fc, v
 
     def counters(self) -> dict:
-        out = (C.c_int64 * 6)()
-        self._ok(self._L.qhp_counters(self._h, out, 6))
-        keys = ["rebuilds", "list_entries", "pair_beads_in_cutoff", "list_capacity", "launches", "overflow"]
+        out = (C.c_int64 * 8)()
+        self._ok(self._L.qhp_counters(self._h, out, 8))
+        keys = ["rebuilds", "list_entries", "pair_beads_in_cutoff", "list_capacity", "launches", "overflow",
+                "staged", "staged_warps"]
         return dict(zip(keys, [int(v) for v in out]))
 
     def check(self):
@@ -262,9 +263,9 @@ class System:
         self._ok(self._L.qhp_profile(self._h, int(bool(enable))))
 
     def profile_read(self) -> dict:
-        ms, n = (C.c_double * 4)(), (C.c_int64 * 4)()
+        ms, n = (C.c_double * 5)(), (C.c_int64 * 5)()
         self._ok(self._L.qhp_profile_read(self._h, ms, n))
-        keys = ["integrate", "rebuild", "pair", "qtb"]
+        keys = ["integrate", "rebuild", "pair", "qtb_generate", "qtb_adapt"]
         return {k: dict(ms=float(ms[i]), n=int(n[i])) for i, k in enumerate(keys)}
 
 

@@ -391,7 +391,7 @@ extern "C" int qhp_profile(qhp_system *s, int enable) {
   if (enable) {
     int rc = prof_drain(s);
     if (rc) return rc;
-    for (int k = 0; k < 4; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
+    for (int k = 0; k < 5; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
   }
   s->prof = enable != 0;
   return QHP_OK;
@@ -401,7 +401,7 @@ extern "C" int qhp_profile_read(qhp_system *s, double *ms_host, int64_t *n_host)
   if (!s) return QHP_EINVAL;
   int rc = prof_drain(s);
   if (rc) return rc;
-  for (int k = 0; k < 4; ++k) { if (ms_host) ms_host[k] = s->prof_ms[k]; if (n_host) n_host[k] = s->prof_n[k]; }
+  for (int k = 0; k < 5; ++k) { if (ms_host) ms_host[k] = s->prof_ms[k]; if (n_host) n_host[k] = s->prof_n[k]; }
   return QHP_OK;
 }
 
@@ -435,7 +435,7 @@ extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
     }
     s->step = st + 1;
     if (adqtb && s->step % s->n_seg == 0) {
-      prof_scope ps(s, 3);
+      prof_scope ps(s, 4);
       rc = qhp_qtb_adapt(s);                              // Q5-Q7 at the end of a segment
       if (rc) return rc;
     }
@@ -535,8 +535,9 @@ extern "C" int qhp_counters(qhp_system *s, int64_t *out_host, int n_out) {
   QHP_CUDA_OK(s, cudaMemcpyAsync(c, s->counters, sizeof(c), cudaMemcpyDeviceToHost, s->stream));
   QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
   s->n_launch = launches;
-  const int64_t v[6] = {c[0], total, c[3], s->nbr_stride * s->N, launches, c[1] | (c[6] << 1)};
-  for (int k = 0; k < std::min(n_out, 6); ++k) out_host[k] = v[k];
+  const int64_t v[8] = {c[0], total, c[3], s->nbr_stride * s->N, launches, c[1] | (c[6] << 1) | (c[7] << 2),
+                        s->staged ? 1 : 0, s->staged ? s->staged_warps : 0};
+  for (int k = 0; k < std::min(n_out, 8); ++k) out_host[k] = v[k];
   return QHP_OK;
 }
 

@@ -119,8 +119,8 @@ struct qhp_system {
   bool prof = false;
   std::vector<cudaEvent_t> prof_ev;      // flat list of (begin, end) pairs
   std::vector<int> prof_kind;            // phase of each pair
-  double prof_ms[4] = {0, 0, 0, 0};
-  int64_t prof_n[4] = {0, 0, 0, 0};
+  double prof_ms[5] = {0, 0, 0, 0, 0};
+  int64_t prof_n[5] = {0, 0, 0, 0, 0};
 
   // ---- run state (host) ----
   bool have_state = false;
