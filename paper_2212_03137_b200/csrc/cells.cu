@@ -19,6 +19,7 @@
 struct CellArgs {
   int N, nc[3], ncell;
   double box[3], inv_box[3], rl2;
+  float boxf[3], inv_boxf[3], rl2_lo, rl2_hi;   // fp32 pre-test: d2f < lo surely inside, >= hi surely outside
   const unsigned long long *flag;
   double thresh2;
 };
@@ -94,6 +95,28 @@ __global__ void k_cells_rank(const CellArgs a, const int32_t *__restrict__ cell_
   rank[i] = b + cnt;
 }
 
+// Is slot k a list neighbour of the slot whose centroid is ci / fi?  The decision is the canonical
+// fp64 one (O4); an fp32 pre-test on wrapped single-precision copies settles every pair that is not
+// within the fp32 error of r_list, so only a thin shell pays for the fp64 arithmetic.
+__device__ __forceinline__ bool list_hit(const CellArgs &a, const double *__restrict__ cent4, const float4 *__restrict__ centf,
+                                         const double4 &ci, const float4 &fi, int k) {
+  const float4 fj = centf[k];
+  if (__float_as_int(fj.w) == __float_as_int(fi.w)) return false;          // same molecule
+  float fx = fi.x - fj.x, fy = fi.y - fj.y, fz = fi.z - fj.z;
+  fx = fmaf(-a.boxf[0], rintf(fx * a.inv_boxf[0]), fx);
+  fy = fmaf(-a.boxf[1], rintf(fy * a.inv_boxf[1]), fy);
+  fz = fmaf(-a.boxf[2], rintf(fz * a.inv_boxf[2]), fz);
+  const float d2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
+  if (d2f < a.rl2_lo) return true;
+  if (d2f >= a.rl2_hi) return false;
+  const double4 cj = reinterpret_cast<const double4 *>(cent4)[k];
+  double dx = __dsub_rn(ci.x, cj.x), dy = __dsub_rn(ci.y, cj.y), dz = __dsub_rn(ci.z, cj.z);
+  dx = __fma_rn(-a.box[0], rint(__dmul_rn(dx, a.inv_box[0])), dx);
+  dy = __fma_rn(-a.box[1], rint(__dmul_rn(dy, a.inv_box[1])), dy);
+  dz = __fma_rn(-a.box[2], rint(__dmul_rn(dz, a.inv_box[2])), dz);
+  return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx))) < a.rl2;
+}
+
 // one warp per slot; nbr == NULL: count only
 __global__ void __launch_bounds__(256) k_list_build(const CellArgs a, const double *__restrict__ cent4,
                                                     const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
@@ -104,8 +127,9 @@ __global__ void __launch_bounds__(256) k_list_build(const CellArgs a, const doub
   const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (i >= a.N) return;
   if (i == 0 && lane == 0 && nbr) counters[0] += 1;
+  const float4 *centf = reinterpret_cast<const float4 *>(cent4 + 4LL * a.N);   // fp32 copies live behind cent4
   const double4 ci = reinterpret_cast<const double4 *>(cent4)[i];
-  const long long mi = __double_as_longlong(ci.w);
+  const float4 fi = centf[i];
   const int cell = cell_of[order[i]];
   const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
   const int nox = min(a.nc[0], 3), noy = min(a.nc[1], 3), noz = min(a.nc[2], 3);
@@ -122,17 +146,7 @@ __global__ void __launch_bounds__(256) k_list_build(const CellArgs a, const doub
         for (int k0 = b; k0 < e; k0 += 32) {
           const int k = k0 + lane;
           bool hit = false;
-          if (k < e && k != i) {
-            const double4 cj = reinterpret_cast<const double4 *>(cent4)[k];
-            if (__double_as_longlong(cj.w) != mi) {
-              double dx = __dsub_rn(ci.x, cj.x), dy = __dsub_rn(ci.y, cj.y), dz = __dsub_rn(ci.z, cj.z);
-              dx = __fma_rn(-a.box[0], rint(__dmul_rn(dx, a.inv_box[0])), dx);
-              dy = __fma_rn(-a.box[1], rint(__dmul_rn(dy, a.inv_box[1])), dy);
-              dz = __fma_rn(-a.box[2], rint(__dmul_rn(dz, a.inv_box[2])), dz);
-              const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-              hit = d2 < a.rl2;
-            }
-          }
+          if (k < e && k != i) hit = list_hit(a, cent4, centf, ci, fi, k);
           const unsigned mask = __ballot_sync(0xffffffffu, hit);
           if (hit && nbr) {
             const int pos = cnt + __popc(mask & lt);
@@ -164,8 +178,9 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
   const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (i >= a.N) return;
   if (i == 0 && lane == 0 && nbr) counters[0] += 1;
+  const float4 *centf = reinterpret_cast<const float4 *>(cent4 + 4LL * a.N);   // fp32 copies live behind cent4
   const double4 ci = reinterpret_cast<const double4 *>(cent4)[i];
-  const long long mi = __double_as_longlong(ci.w);
+  const float4 fi = centf[i];
   const int cell = cell_of[order[i]];
   const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
   const unsigned lt = (1u << lane) - 1u;
@@ -180,17 +195,7 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
         for (int k0 = b; k0 < e; k0 += 32) {
           const int k = k0 + lane;
           bool hit = false;
-          if (k < e && k != i) {
-            const double4 cj = reinterpret_cast<const double4 *>(cent4)[k];
-            if (__double_as_longlong(cj.w) != mi) {
-              double dx = __dsub_rn(ci.x, cj.x), dy = __dsub_rn(ci.y, cj.y), dz = __dsub_rn(ci.z, cj.z);
-              dx = __fma_rn(-a.box[0], rint(__dmul_rn(dx, a.inv_box[0])), dx);
-              dy = __fma_rn(-a.box[1], rint(__dmul_rn(dy, a.inv_box[1])), dy);
-              dz = __fma_rn(-a.box[2], rint(__dmul_rn(dz, a.inv_box[2])), dz);
-              const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-              hit = d2 < a.rl2;
-            }
-          }
+          if (k < e && k != i) hit = list_hit(a, cent4, centf, ci, fi, k);
           const unsigned mask = __ballot_sync(0xffffffffu, hit);
           if (hit && nbr) {
             const int pos = cnt + __popc(mask & lt);
@@ -274,6 +279,16 @@ static CellArgs cell_args(qhp_system *s, bool force) {
   const double rl = s->r_cut + s->skin;
   for (int d = 0; d < 3; ++d) { a.nc[d] = s->nc[d]; a.box[d] = s->box[d]; a.inv_box[d] = s->inv_box[d]; }
   a.rl2 = rl * rl;
+  {
+    // bound on the fp32 error of d2: coordinates wrapped into [0, L) and the box edge are rounded to
+    // fp32 (2^-24 relative each), the image count is at most 1; 4x safety
+    double Lmax = 0.0;
+    for (int d = 0; d < 3; ++d) { Lmax = fmax(Lmax, s->box[d]); a.boxf[d] = (float)s->box[d]; a.inv_boxf[d] = (float)s->inv_box[d]; }
+    const double e = (5.0 * Lmax + rl) * ldexp(1.0, -24);
+    const double m = 4.0 * (2.0 * sqrt(3.0) * rl * e + 4.0 * ldexp(1.0, -24) * a.rl2);
+    a.rl2_lo = (float)(a.rl2 - m) * (1.0f - 1.2e-7f);
+    a.rl2_hi = (float)(a.rl2 + m) * (1.0f + 1.2e-7f);
+  }
   a.flag = force ? nullptr : &s->d2max[s->flag_idx];
   const double th = 0.5 * s->skin;
   a.thresh2 = th * th;

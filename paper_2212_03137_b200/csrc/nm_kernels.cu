@@ -465,7 +465,8 @@ __global__ void k_to_beads(const double *__restrict__ Q, const double *__restric
 // mode 1: write xc_out [Pc][N][3] in atom order (parity hook).
 // `need` (may be NULL): device flag words; the kernel returns at once unless forced or the
 // list-validity statistic exceeds the threshold.
-__global__ void k_contract(const double *__restrict__ Q, int N, int Pc, const double *__restrict__ Tc,
+struct BoxArg { double box[3], inv_box[3]; };
+__global__ void k_contract(const BoxArg bx, const double *__restrict__ Q, int N, int Pc, const double *__restrict__ Tc,
                            const int32_t *__restrict__ rank, const int32_t *__restrict__ type,
                            const int32_t *__restrict__ molid, double *pos4, double *cent4, double *cref,
                            double *xc_out, int mode, const unsigned long long *d2max, double thresh2,
@@ -494,6 +495,10 @@ __global__ void k_contract(const double *__restrict__ Q, int N, int Pc, const do
     const double q0 = Q[d];
     cent4[slot * 4 + c] = q0;
     if (c == 0) reinterpret_cast<long long *>(cent4)[slot * 4 + 3] = molid[atom];
+    // single-precision copy, wrapped into [0, L), for the pre-test of the list build (cells.cu)
+    float *centf = reinterpret_cast<float *>(cent4 + 4LL * N);
+    centf[slot * 4 + c] = (float)(q0 - bx.box[c] * floor(q0 * bx.inv_box[c]));
+    if (c == 0) reinterpret_cast<int *>(centf)[slot * 4 + 3] = molid[atom];
     cref[d] = q0;
   }
 }
@@ -644,7 +649,9 @@ int qhp_nm_contract(qhp_system *s, bool rebuild_mode, bool force) {
   const double th = 0.5 * s->skin;
   // in rebuild mode the kernel reads the statistic written by the last integrator pass
   const unsigned long long *flag = (rebuild_mode && !force) ? &s->d2max[s->flag_idx] : nullptr;
-  k_contract<<<grid, tb, 0, s->stream>>>(s->Q, s->N, s->Pc, s->d_Tc, s->rank, s->dt_.type, s->dt_.molid,
+  BoxArg bx;
+  for (int d = 0; d < 3; ++d) { bx.box[d] = s->box[d]; bx.inv_box[d] = s->inv_box[d]; }
+  k_contract<<<grid, tb, 0, s->stream>>>(bx, s->Q, s->N, s->Pc, s->d_Tc, s->rank, s->dt_.type, s->dt_.molid,
                                         s->pos4, rebuild_mode ? s->cent4 : nullptr, s->cref, nullptr, 0,
                                         flag, th * th, (long long *)s->counters);
   QHP_LAUNCH_OK(s);
@@ -655,7 +662,7 @@ int qhp_nm_contracted_out(qhp_system *s, double *xc) {
   const long long ND = 3LL * s->N;
   const int tb = 256;
   const unsigned grid = (unsigned)((ND + tb - 1) / tb);
-  k_contract<<<grid, tb, 0, s->stream>>>(s->Q, s->N, s->Pc, s->d_Tc, nullptr, s->dt_.type, s->dt_.molid,
+  k_contract<<<grid, tb, 0, s->stream>>>(BoxArg{}, s->Q, s->N, s->Pc, s->d_Tc, nullptr, s->dt_.type, s->dt_.molid,
                                         nullptr, nullptr, nullptr, xc, 1, nullptr, 0.0, nullptr);
   QHP_LAUNCH_OK(s);
   return QHP_OK;

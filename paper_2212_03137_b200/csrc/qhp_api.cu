@@ -230,7 +230,7 @@ extern "C" int qhp_create(const qhp_topology *top, int P, int P_contract, double
   CREATE_CUDA(cudaMalloc(&s->Pm, sizeof(double) * ND * P));
   CREATE_CUDA(cudaMalloc(&s->pos4, sizeof(double) * 4 * (size_t)N * s->Pc));
   CREATE_CUDA(cudaMalloc(&s->Fs, sizeof(double) * ND * s->Pc));
-  CREATE_CUDA(cudaMalloc(&s->cent4, sizeof(double) * 4 * (size_t)N));
+  CREATE_CUDA(cudaMalloc(&s->cent4, (sizeof(double) + sizeof(float)) * 4 * (size_t)N));   // double4 + float4 copies
   CREATE_CUDA(cudaMalloc(&s->cref, sizeof(double) * ND));
   CREATE_CUDA(cudaMemset(s->Fs, 0, sizeof(double) * ND * s->Pc));
 
