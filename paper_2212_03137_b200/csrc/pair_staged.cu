@@ -126,7 +126,8 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
 
   const int h0 = off[13], nh = off[14] - off[13], slot0 = cbeg[13];
   uint32_t *ql = queue + warp * STG_QUEUE + lane;          // this lane's view of the warp's queue
-  const unsigned lt = (1u << lane) - 1u;
+  unsigned lt = (1u << lane) - 1u;
+  asm volatile("" : "+l"(ql), "+r"(lt));                   // keep both in registers (ptxas would recompute them per use)
   double U = 0.0;
   unsigned long long hits = 0;
 

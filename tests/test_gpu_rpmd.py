@@ -174,3 +174,33 @@ def test_harmonic_oscillators_single_atom_molecules():
     assert np.abs(x1.cpu().numpy() - xr).max() < 1e-10
     obs = sysg.observables().cpu().numpy()
     assert np.abs(obs - ref.observables()).max() < 1e-9 * np.abs(ref.observables()).max()
+
+
+def test_staged_pair_kernel_mid_size():
+    """5832 waters (17,496 atoms, 5 x 5 x 5 cells): the smallest water box the shared-memory staged pair
+    kernel serves (>= 4 cells per dimension and the 27-cell neighbourhood fits); lists, forces,
+    energy variant (observables) and 20 steps against the oracle."""
+    import oracle as O
+    top = W.water_box(5832)
+    sysg, ref, x0, p0 = make_pair(top, 4, 2, 0.25, "pile", sigma_bead=0.05)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    c = sysg.counters()
+    assert c["staged"] == 1 and c["overflow"] == 0
+    ref.set_state(x0, p0, 0)
+    otop, cent = _lists_check(sysg, top, x0)
+    count, i, j = _pairs_from_gpu(sysg)
+    for a in (0, 1, 7777, top["n_atoms"] - 1):
+        assert np.array_equal(np.sort(j[i == a]), np.sort(O.neighbours_of(otop, cent, a)))
+    assert (i < j).sum() * 2 == i.size
+    G = sysg.forces().cpu().numpy()
+    Gref = ref.forces()
+    assert np.abs(G - Gref).max() < FTOL * np.abs(Gref).max()
+    obs = sysg.observables().cpu().numpy()
+    oref = ref.observables()
+    assert np.abs(obs - oref).max() < 1e-10 * np.abs(oref).max()
+    sysg.step(20)
+    ref.step(20)
+    x1, _, _ = sysg.get_state()
+    xr, _ = ref.get_state()
+    assert np.abs(x1.cpu().numpy() - xr).max() < XTOL
+    sysg.check()
