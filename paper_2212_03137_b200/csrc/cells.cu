@@ -19,7 +19,7 @@
 struct CellArgs {
   int N, nc[3], ncell;
   double box[3], inv_box[3], rl2;
-  float boxf[3], inv_boxf[3], rl2_lo, rl2_hi;   // fp32 pre-test: d2f < lo surely inside, >= hi surely outside
+  float boxf[3], inv_boxf[3], edgef[3], rl2_lo, rl2_hi;   // fp32 pre-test: d2f < lo surely inside, >= hi surely outside
   const unsigned long long *flag;
   double thresh2;
 };
@@ -98,6 +98,14 @@ __global__ void k_cells_rank(const CellArgs a, const int32_t *__restrict__ cell_
 // Is slot k a list neighbour of the slot whose centroid is ci / fi?  The decision is the canonical
 // fp64 one (O4); an fp32 pre-test on wrapped single-precision copies settles every pair that is not
 // within the fp32 error of r_list, so only a thin shell pays for the fp64 arithmetic.
+__device__ __forceinline__ bool list_hit_exact(const CellArgs &a, const double *__restrict__ cent4, const double4 &ci, int k) {
+  const double4 cj = reinterpret_cast<const double4 *>(cent4)[k];
+  double dx = __dsub_rn(ci.x, cj.x), dy = __dsub_rn(ci.y, cj.y), dz = __dsub_rn(ci.z, cj.z);
+  dx = __fma_rn(-a.box[0], rint(__dmul_rn(dx, a.inv_box[0])), dx);
+  dy = __fma_rn(-a.box[1], rint(__dmul_rn(dy, a.inv_box[1])), dy);
+  dz = __fma_rn(-a.box[2], rint(__dmul_rn(dz, a.inv_box[2])), dz);
+  return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx))) < a.rl2;
+}
 __device__ __forceinline__ bool list_hit(const CellArgs &a, const double *__restrict__ cent4, const float4 *__restrict__ centf,
                                          const double4 &ci, const float4 &fi, int k) {
   const float4 fj = centf[k];
@@ -109,12 +117,7 @@ __device__ __forceinline__ bool list_hit(const CellArgs &a, const double *__rest
   const float d2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
   if (d2f < a.rl2_lo) return true;
   if (d2f >= a.rl2_hi) return false;
-  const double4 cj = reinterpret_cast<const double4 *>(cent4)[k];
-  double dx = __dsub_rn(ci.x, cj.x), dy = __dsub_rn(ci.y, cj.y), dz = __dsub_rn(ci.z, cj.z);
-  dx = __fma_rn(-a.box[0], rint(__dmul_rn(dx, a.inv_box[0])), dx);
-  dy = __fma_rn(-a.box[1], rint(__dmul_rn(dy, a.inv_box[1])), dy);
-  dz = __fma_rn(-a.box[2], rint(__dmul_rn(dz, a.inv_box[2])), dz);
-  return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx))) < a.rl2;
+  return list_hit_exact(a, cent4, ci, k);
 }
 
 // one warp per slot; nbr == NULL: count only
@@ -192,16 +195,36 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
                   qz = (cz - 1 + oz + a.nc[2]) % a.nc[2];
         const int c2 = (qx * a.nc[1] + qy) * a.nc[2] + qz;
         const int b = cell_start[c2], e = cell_start[c2 + 1];
-        for (int k0 = b; k0 < e; k0 += 32) {
-          const int k = k0 + lane;
-          bool hit = false;
-          if (k < e && k != i) hit = list_hit(a, cent4, centf, ci, fi, k);
-          const unsigned mask = __ballot_sync(0xffffffffu, hit);
-          if (hit && nbr) {
-            const int pos = cnt + __popc(mask & lt);
-            if (pos < stride) nbr[i * stride + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)(off + k - b);
+        // distance from this centroid to the neighbour cell's box (wrapped coordinates): a cell out of
+        // reach is skipped as a whole (the margin of rl2_hi covers the fp32 rounding of both)
+        const float gx = ox == 0 ? fi.x - cx * a.edgef[0] : (ox == 2 ? (cx + 1) * a.edgef[0] - fi.x : 0.f);
+        const float gy = oy == 0 ? fi.y - cy * a.edgef[1] : (oy == 2 ? (cy + 1) * a.edgef[1] - fi.y : 0.f);
+        const float gz = oz == 0 ? fi.z - cz * a.edgef[2] : (oz == 2 ? (cz + 1) * a.edgef[2] - fi.z : 0.f);
+        const float hx = fmaxf(gx, 0.f), hy = fmaxf(gy, 0.f), hz = fmaxf(gz, 0.f);
+        if (fmaf(hz, hz, fmaf(hy, hy, hx * hx)) < a.rl2_hi) {
+          // the image of the neighbour cell next to the home cell is known per cell: with >= 4 cells per
+          // dimension it is the minimum image of every pair within r_list, so the pre-test needs no rint
+          const float sx = cx - 1 + ox < 0 ? -a.boxf[0] : (cx - 1 + ox >= a.nc[0] ? a.boxf[0] : 0.f);
+          const float sy = cy - 1 + oy < 0 ? -a.boxf[1] : (cy - 1 + oy >= a.nc[1] ? a.boxf[1] : 0.f);
+          const float sz = cz - 1 + oz < 0 ? -a.boxf[2] : (cz - 1 + oz >= a.nc[2] ? a.boxf[2] : 0.f);
+          const float px = fi.x - sx, py = fi.y - sy, pz = fi.z - sz;
+          for (int k0 = b; k0 < e; k0 += 32) {
+            const int k = k0 + lane;
+            bool hit = false;
+            if (k < e && k != i) {
+              const float4 fj = centf[k];
+              const float dxf = px - fj.x, dyf = py - fj.y, dzf = pz - fj.z;
+              const float d2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
+              if (__float_as_int(fj.w) != __float_as_int(fi.w) && d2f < a.rl2_hi)
+                hit = d2f < a.rl2_lo || list_hit_exact(a, cent4, ci, k);
+            }
+            const unsigned mask = __ballot_sync(0xffffffffu, hit);
+            if (hit && nbr) {
+              const int pos = cnt + __popc(mask & lt);
+              if (pos < stride) nbr[i * stride + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)(off + k - b);
+            }
+            cnt += __popc(mask);
           }
-          cnt += __popc(mask);
         }
         off += e - b;
       }
@@ -283,7 +306,7 @@ static CellArgs cell_args(qhp_system *s, bool force) {
     // bound on the fp32 error of d2: coordinates wrapped into [0, L) and the box edge are rounded to
     // fp32 (2^-24 relative each), the image count is at most 1; 4x safety
     double Lmax = 0.0;
-    for (int d = 0; d < 3; ++d) { Lmax = fmax(Lmax, s->box[d]); a.boxf[d] = (float)s->box[d]; a.inv_boxf[d] = (float)s->inv_box[d]; }
+    for (int d = 0; d < 3; ++d) { Lmax = fmax(Lmax, s->box[d]); a.boxf[d] = (float)s->box[d]; a.inv_boxf[d] = (float)s->inv_box[d]; a.edgef[d] = (float)(s->box[d] / s->nc[d]); }
     const double e = (5.0 * Lmax + rl) * ldexp(1.0, -24);
     const double m = 4.0 * (2.0 * sqrt(3.0) * rl * e + 4.0 * ldexp(1.0, -24) * a.rl2);
     a.rl2_lo = (float)(a.rl2 - m) * (1.0f - 1.2e-7f);
