@@ -228,6 +228,21 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
   const int atom = tl.a0 + t / 3, c = t % 3;
   if (blockIdx.x == 0 && t == 0 && a.do_step) a.d2max[(a.step + 1) & 1] = 0ull;
 
+  // loads that do not depend on the tile exchange are issued first, so that their latency overlaps
+  // phases 1-3 (the P <= 8 kernels are latency-bound: one short dependent chain per CTA)
+  constexpr int PF = P < 8 ? P : 8;                    // momenta in flight
+  double pl[PF];
+  double fc_early = 0.0;
+  int ty = 0;
+  if (active) {
+    ty = a.type[atom];
+    if (P <= 8) {
+#pragma unroll
+      for (int k = 0; k < PF; ++k) pl[k] = a.Pm[k * a.ND + dof];
+    }
+    if (THERMO == 2 && a.do_step) fc_early = a.Fc[dof * a.n_seg + a.n_loc];
+  }
+
   // ---- phase 1: Q -> bead positions (shared tile), V_f per (molecule, bead) -------------------------
   {
     double Qr[P];
@@ -264,7 +279,6 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
   // ---- phase 4: B A O A per mode, contraction of the new positions -----------------------------------------
   double d2 = 0.0;
   if (active) {
-    const int ty = a.type[atom];
     const double m = a.mass[ty];
     const double *cf = a.coef + ty * P * QHP_NCOEF;   // read-only, L1-resident (two types x P x 6 doubles)
     double xc[PCM];                     // contracted beads (first Pc entries used)
@@ -272,11 +286,9 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
     for (int j = 0; j < PCM; ++j) xc[j] = 0.0;
     // momenta are fetched eight modes ahead of their use: the stores of one mode must not
     // serialise the loads of the next (Q and Pm may alias as far as the compiler knows)
-    constexpr int PF = P < 8 ? P : 8;
-    double pl[PF];
 #pragma unroll
     for (int n = 0; n < P; ++n) {
-      if (n % PF == 0) {
+      if (n % PF == 0 && P > 8) {
 #pragma unroll
         for (int k = 0; k < PF; ++k)
           if (n + k < P) pl[k] = a.Pm[(n + k) * a.ND + dof];
@@ -296,7 +308,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
         } else if (THERMO == 2) {
           // classical BAOAB carrying the coloured force (Eq. 12, l.199; readings G14, G16)
           const long long k = dof * a.n_seg + a.n_loc;
-          const double pn = a.qa * p + a.qbA * a.Fc[k];
+          const double pn = a.qa * p + a.qbA * fc_early;
           a.vseg[k] = (p + pn) / (2.0 * m);
           p = pn;
         }
