@@ -299,6 +299,43 @@ class Rpmd:
         return observables(self.top, self.P, self.Pc, self.T, self.Q, self.Pm, self.uc)
 
 
+def nm_forces_split(top: Topology, P: int, Pc: int, Q: np.ndarray, cells: bool | None = None):
+    """Normal-mode forces of V_f and V_s separately (Eq. 18; used by the RESPA stepper)."""
+    Q = _f64(Q)
+    ff, fs = np.empty_like(Q), np.empty_like(Q)
+    uc = top.use_cells if cells is None else int(cells)
+    lib().qo_nm_forces_split(top.ref, C.c_int(P), C.c_int(Pc), _p(Q), _p(ff), _p(fs), C.c_int(uc))
+    return ff, fs
+
+
+class RpmdRespa(Rpmd):
+    """BAOAB-RESPA (Eq. 19): `step(n)` advances n INNER steps of dt, n a multiple of
+    n_alt; V_s (on the Pc contracted beads) kicks with n_alt*dt/2 around every n_alt inner steps."""
+
+    def __init__(self, top, P, Pc, dt_ps, T_K, thermo, gamma0, seed, n_alt: int, cells=None):
+        super().__init__(top, P, Pc, dt_ps, T_K, thermo, gamma0, seed, cells)
+        self.n_alt = int(n_alt)
+
+    def set_state(self, x_beads, p_beads, step0: int = 0):
+        self.Q = beads_to_nm(x_beads)
+        self.Pm = beads_to_nm(p_beads)
+        self.ff, self.fs = nm_forces_split(self.top, self.P, self.Pc, self.Q, self.uc)
+        self.step_index = step0
+
+    @property
+    def f(self):
+        return self.ff + self.fs
+
+    def step(self, n: int):
+        assert n % self.n_alt == 0
+        lib().qo_rpmd_respa_steps(self.top.ref, C.c_int(self.P), C.c_int(self.Pc), C.c_double(self.dt),
+                                  C.c_double(self.T), C.c_int(self.thermo), C.c_double(self.gamma0),
+                                  C.c_uint64(self.seed), C.c_int64(self.step_index), C.c_int64(n // self.n_alt),
+                                  C.c_int(self.n_alt), _p(self.Q), _p(self.Pm), _p(self.ff), _p(self.fs),
+                                  C.c_int(self.uc))
+        self.step_index += n
+
+
 # ---------------------------------------------------------------- adQTB (O9-O11)
 def theta(omega, T_K: float):
     return np.vectorize(lambda w: lib().qo_theta(float(w), float(T_K)))(omega)

@@ -438,52 +438,114 @@ void qo_observables(const qo_topology *t, int P, int Pc, double T_K, const doubl
  * Pins: A block conserves each mode's energy; c1^2 + c2^2 = 1; P = 1 == classical BAOAB;
  * harmonic <q^2> closed form (statistical).
  * ------------------------------------------------------------------------------------------ */
-void qo_rpmd_steps(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
-                   double gamma0, uint64_t seed, int64_t step0, int64_t nsteps,
-                   double *Q, double *Pm, double *f, int use_cells) {
+/* A(dt/2) O(dt) A(dt/2) of one step (O5 items 2-4), shared by qo_rpmd_steps and qo_rpmd_respa_steps */
+static void qo_aoa(const qo_topology *t, int P, double dt, double T_K, int thermo, double gamma0,
+                   uint64_t seed, int64_t step, const double *om, double *Q, double *Pm) {
   int N = t->n_atoms;
   int64_t nd = 3 * (int64_t)N;
-  double *om = (double *)malloc(sizeof(double) * P);
-  qo_nm_freq(P, T_K, om);
-  for (int64_t s = 0; s < nsteps; ++s) {
-    int64_t step = step0 + s;
-    /* 1. B(dt/2) */
-    for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * f[k];
-    for (int half = 0; half < 2; ++half) {
-      /* 2./4. A(dt/2): centroid translation, exact harmonic rotation of the fluctuation modes */
-      for (int n = 0; n < P; ++n) for (int a = 0; a < N; ++a) {
-        double m = t->mass[t->type[a]];
-        for (int c = 0; c < 3; ++c) {
-          int64_t k = n * nd + 3 * a + c;
-          if (n == 0) { Q[k] += 0.5 * dt * Pm[k] / m; }
-          else {
-            double w = om[n], cs = cos(w * 0.5 * dt), sn = sin(w * 0.5 * dt);
-            double q = Q[k], p = Pm[k];
-            Q[k]  = cs * q + sn / (m * w) * p;
-            Pm[k] = -m * w * sn * q + cs * p;
+  for (int half = 0; half < 2; ++half) {
+    /* 2./4. A(dt/2): centroid translation, exact harmonic rotation of the fluctuation modes */
+    for (int n = 0; n < P; ++n) for (int a = 0; a < N; ++a) {
+      double m = t->mass[t->type[a]];
+      for (int c = 0; c < 3; ++c) {
+        int64_t k = n * nd + 3 * a + c;
+        if (n == 0) { Q[k] += 0.5 * dt * Pm[k] / m; }
+        else {
+          double w = om[n], cs = cos(w * 0.5 * dt), sn = sin(w * 0.5 * dt);
+          double q = Q[k], p = Pm[k];
+          Q[k]  = cs * q + sn / (m * w) * p;
+          Pm[k] = -m * w * sn * q + cs * p;
+        }
+      }
+    }
+    /* 3. O(dt) between the two A half-steps */
+    if (half == 0 && thermo == 1)
+      for (int n = 0; n < P; ++n) {
+        double g = (n == 0) ? gamma0 : (gamma0 > om[n] ? gamma0 : om[n]);
+        double c1 = exp(-g * dt), c2 = sqrt(1.0 - c1 * c1);
+        for (int a = 0; a < N; ++a) {
+          double z[3];
+          qo_normals3(seed, (uint32_t)a, (uint32_t)n, 3u, (uint64_t)step, z);
+          double sg = sqrt(t->mass[t->type[a]] * QO_KB * T_K * QO_ACC);
+          for (int c = 0; c < 3; ++c) {
+            int64_t k = n * nd + 3 * a + c;
+            Pm[k] = c1 * Pm[k] + sg * c2 * z[c];
           }
         }
       }
-      /* 3. O(dt) between the two A half-steps */
-      if (half == 0 && thermo == 1)
-        for (int n = 0; n < P; ++n) {
-          double g = (n == 0) ? gamma0 : (gamma0 > om[n] ? gamma0 : om[n]);
-          double c1 = exp(-g * dt), c2 = sqrt(1.0 - c1 * c1);
-          for (int a = 0; a < N; ++a) {
-            double z[3];
-            qo_normals3(seed, (uint32_t)a, (uint32_t)n, 3u, (uint64_t)step, z);
-            double sg = sqrt(t->mass[t->type[a]] * QO_KB * T_K * QO_ACC);
-            for (int c = 0; c < 3; ++c) {
-              int64_t k = n * nd + 3 * a + c;
-              Pm[k] = c1 * Pm[k] + sg * c2 * z[c];
-            }
-          }
-        }
-    }
+  }
+}
+
+void qo_rpmd_steps(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
+                   double gamma0, uint64_t seed, int64_t step0, int64_t nsteps,
+                   double *Q, double *Pm, double *f, int use_cells) {
+  int64_t nd = 3 * (int64_t)t->n_atoms;
+  double *om = (double *)malloc(sizeof(double) * P);
+  qo_nm_freq(P, T_K, om);
+  for (int64_t s = 0; s < nsteps; ++s) {
+    /* 1. B(dt/2) */
+    for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * f[k];
+    qo_aoa(t, P, dt, T_K, thermo, gamma0, seed, step0 + s, om, Q, Pm);
     /* 5.-7. forces at the new positions */
     qo_nm_forces(t, P, Pc, Q, f, NULL, use_cells);
     /* 8. B(dt/2) */
     for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * f[k];
+  }
+  free(om);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * NEXT-1  BAOAB-RESPA (Eq. 19): V = V_s + V_f (Eq. 18),
+ *   Bs(n_alt dt/2) [ Bf(dt/2) A(dt/2) O(dt) A(dt/2) Bf(dt/2) ]^{n_alt} Bs(n_alt dt/2)
+ * with V_f on all P beads and V_s on the Pc contracted beads (Eq. 20).
+ * ff, fs: normal-mode forces of V_f and V_s at the current Q (both valid on entry and on exit).
+ * `step0` counts INNER steps (one Philox step index per O block); n_outer outer steps are taken.
+ * Pins (tests/test_oracle_respa.py): n_alt = 1 reproduces qo_rpmd_steps; V_s = 0 reproduces plain
+ * BAOAB with dt; time reversal; second-order convergence to the single-step trajectory;
+ * conservation of the ring-polymer Hamiltonian without thermostat.
+ * ------------------------------------------------------------------------------------------ */
+void qo_nm_forces_split(const qo_topology *t, int P, int Pc, const double *Q, double *ff, double *fs,
+                        int use_cells) {
+  int64_t nd = 3 * (int64_t)t->n_atoms;
+  double *x = (double *)malloc(sizeof(double) * P * nd);
+  double *Ff = (double *)calloc((size_t)(P * nd), sizeof(double));
+  double *xc = (double *)malloc(sizeof(double) * Pc * nd);
+  double *Fc = (double *)calloc((size_t)(Pc * nd), sizeof(double));
+  if (ff) {
+    qo_nm_to_beads(P, nd, Q, x);
+    for (int i = 0; i < P; ++i) qo_force_fast(t, x + i * nd, Ff + i * nd);
+    qo_beads_to_nm(P, nd, Ff, ff);
+  }
+  if (fs) {
+    qo_contract(P, Pc, nd, Q, xc);
+    for (int j = 0; j < Pc; ++j) {
+      if (use_cells) qo_force_slow_cells(t, xc + j * nd, Fc + j * nd);
+      else qo_force_slow_brute(t, xc + j * nd, Fc + j * nd);
+    }
+    qo_expand_force(P, Pc, nd, Fc, fs);
+  }
+  free(x); free(Ff); free(xc); free(Fc);
+}
+
+void qo_rpmd_respa_steps(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
+                         double gamma0, uint64_t seed, int64_t step0, int64_t n_outer, int n_alt,
+                         double *Q, double *Pm, double *ff, double *fs, int use_cells) {
+  int64_t nd = 3 * (int64_t)t->n_atoms;
+  double *om = (double *)malloc(sizeof(double) * P);
+  qo_nm_freq(P, T_K, om);
+  for (int64_t o = 0; o < n_outer; ++o) {
+    /* Bs(n_alt dt/2) */
+    for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * n_alt * dt * QO_ACC * fs[k];
+    for (int j = 0; j < n_alt; ++j) {
+      /* Bf(dt/2) A O A Bf(dt/2) */
+      for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * ff[k];
+      qo_aoa(t, P, dt, T_K, thermo, gamma0, seed, step0 + o * n_alt + j, om, Q, Pm);
+      qo_nm_forces_split(t, P, Pc, Q, ff, NULL, use_cells);
+      for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * ff[k];
+    }
+    /* Bs(n_alt dt/2) with V_s at the new positions */
+    qo_nm_forces_split(t, P, Pc, Q, NULL, fs, use_cells);
+    for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * n_alt * dt * QO_ACC * fs[k];
   }
   free(om);
 }
