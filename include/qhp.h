@@ -105,6 +105,13 @@ int qhp_get_state_host(qhp_system *sys, double *x_beads, double *p_beads, int64_
  * boundaries. */
 int qhp_step(qhp_system *sys, int64_t nsteps);
 
+/* BAOAB-RESPA (Eq. 19): Bs(n_alt dt/2) [Bf(dt/2) A O A Bf(dt/2)]^n_alt Bs(n_alt dt/2)
+ * with V_f (bonds, angles, tethers; all P beads) in Bf and V_s (LJ + DSF Coulomb; P_contract beads) in
+ * Bs.  qhp_step keeps counting INNER steps of dt (one Philox index per O block) and then accepts
+ * multiples of n_alt only; V_s and the neighbour objects are evaluated once per n_alt inner steps.
+ * n_alt = 1 (default) is plain B A O A B.  Call it at a multiple of n_alt steps; not with adQTB. */
+int qhp_set_respa(qhp_system *sys, int n_alt);
+
 /* Bead-space forces at the current positions, device [P][n_atoms][3]:
  * G_i = -grad V_f(x_i) + (P/P') sum_j C_ji (-grad V_s(xc_j))  (Eq. 10-11 and chain rule on Eq. 20). */
 int qhp_forces(qhp_system *sys, double *f_beads);

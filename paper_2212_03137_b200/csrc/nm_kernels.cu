@@ -31,10 +31,11 @@ struct IntArgs {
   const double *Fs;
   const double *cref;
   unsigned long long *d2max;
-  int kick_prev, do_step;
+  int do_step;
+  double w_fast, w_slow;   // kick weights (dt/2 * 418.4 units) of V_f and V_s in this pass
   long long step;
   unsigned long long seed;
-  double hA, hdt;
+  double hdt;
   // adQTB (P = 1)
   const double *Fc;
   double *vseg;
@@ -121,9 +122,12 @@ __device__ __forceinline__ void modes_to_beads_tile(const NmTab<P> &tab, const d
 }
 
 // fr[n] = (1/sqrt P) sum_i T_in F^f_i (Eq. 10-11) + (1/sqrt P') sum_j T'_jn Fs_j (n < P'), one DOF
+// wf, ws: weights of the fast (V_f) and slow (V_s) parts: 1, 1 for the total force; the integrator
+// passes the kick weights of the two parts, which differ under BAOAB-RESPA (Eq. 19).
 template <int P>
 __device__ __forceinline__ void project_forces_tile(const IntArgs &a, const NmTab<P> &tab, const NmTab<P> &ctab,
-                                                    const double *ft, int TD, int t, int atom, int c, double (&fr)[P]) {
+                                                    const double *ft, int TD, int t, int atom, int c, double (&fr)[P],
+                                                    double wf = 1.0, double ws = 1.0) {
 #pragma unroll
   for (int n = 0; n < P; ++n) fr[n] = 0.0;
 #pragma unroll 1
@@ -132,12 +136,12 @@ __device__ __forceinline__ void project_forces_tile(const IntArgs &a, const NmTa
 #pragma unroll
     for (int n = 0; n < P; ++n) fr[n] = fma(tab.T[i * P + n], Fi, fr[n]);
   }
-  const double isp = 1.0 / sqrt((double)P);
+  const double isp = wf / sqrt((double)P);
 #pragma unroll
   for (int n = 0; n < P; ++n) fr[n] *= isp;
   // slow forces of the contracted beads, chain rule on Eq. 20
   const int Pc = a.Pc;
-  const double ispc = 1.0 / sqrt((double)Pc);
+  const double ispc = ws / sqrt((double)Pc);
   const long long slot = a.rank[atom];
   for (int j = 0; j < Pc; ++j) {
     const double Fj = a.Fs[((long long)j * a.N + slot) * 3 + c] * ispc;
@@ -262,7 +266,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
   }
   // ---- phase 2: normal-mode forces of this DOF ---------------------------------------------------------
   double fr[P];
-  if (active) project_forces_tile<P>(a, tab, ctab, ft, TD, t, atom, c, fr);
+  if (active) project_forces_tile<P>(a, tab, ctab, ft, TD, t, atom, c, fr, a.w_fast, a.w_slow);   // fr = momentum kick
   // ---- phase 3 (PILE): one Philox call per (atom, mode) gives the three Cartesian normals; they are
   //      exchanged through the force tile, which is dead once every thread has its fr ---------------------
   if (THERMO == 1 && a.do_step) {
@@ -295,9 +299,8 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
       }
       double q = xt[n * TD + t];
       double p = pl[n % PF];
-      if (a.kick_prev) p += a.hA * fr[n];
+      p += fr[n];                       // B: pending half kick of the last step + first half kick of this one
       if (a.do_step) {
-        p += a.hA * fr[n];
         const double cs = __ldg(cf + n * QHP_NCOEF + 0), s1 = __ldg(cf + n * QHP_NCOEF + 1), s2 = __ldg(cf + n * QHP_NCOEF + 2);
         // A(dt/2): centroid translation / exact free ring-polymer rotation
         if (n == 0) q += a.hdt * p / m;
@@ -535,7 +538,7 @@ static IntArgs make_args(qhp_system *s) {
   a.bond_k = s->dt_.bond_k; a.bond_r0 = s->dt_.bond_r0; a.angle_k = s->dt_.angle_k; a.angle_th0 = s->dt_.angle_th0;
   a.tether_k = s->has_tether ? s->dt_.tether_k : nullptr; a.mass = s->dt_.mass;
   a.rank = s->rank; a.pos4 = s->pos4; a.Fs = s->Fs; a.cref = s->cref; a.d2max = s->d2max;
-  a.seed = s->th.seed; a.hdt = 0.5 * s->dt; a.hA = 0.5 * s->dt * QHP_ACC;
+  a.seed = s->th.seed; a.hdt = 0.5 * s->dt; a.w_fast = 1.0; a.w_slow = 1.0;
   a.Fc = s->Fc; a.vseg = s->vseg; a.n_seg = s->n_seg;
   a.kT = QHP_KB * s->T;
   return a;
@@ -561,9 +564,16 @@ template <typename K> static cudaError_t set_smem(K kern, size_t bytes) {
   return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
+// kick_prev: the second half kick of the previous step is still pending (forces at the current Q);
+// do_step: first half kick + A O A of step `step`.  Under RESPA (n_alt > 1, Eq. 19) V_s kicks
+// with n_alt dt/2 only around every n_alt-th inner step, V_f with dt/2 around every inner step.
 int qhp_nm_integrate(qhp_system *s, bool kick_prev, bool do_step, int64_t step) {
   IntArgs a = make_args(s);
-  a.kick_prev = kick_prev; a.do_step = do_step; a.step = step;
+  const double hA = 0.5 * s->dt * QHP_ACC;
+  const int na = s->n_alt;
+  a.do_step = do_step; a.step = step;
+  a.w_fast = (kick_prev ? hA : 0.0) + (do_step ? hA : 0.0);
+  a.w_slow = (kick_prev && step % na == 0 ? na * hA : 0.0) + (do_step && step % na == 0 ? na * hA : 0.0);
   if (do_step) s->flag_idx = (int)(step & 1);
   if (s->th.kind == QHP_THERMO_ADQTB) {
     a.n_loc = (int)(step % s->n_seg);

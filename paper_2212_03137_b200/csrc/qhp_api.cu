@@ -307,6 +307,7 @@ static int flush_kick(qhp_system *s) {
 
 extern "C" int qhp_set_state(qhp_system *s, const double *x_beads, const double *p_beads, int64_t step0) {
   if (!s || !x_beads || !p_beads || step0 < 0) { if (s) s->err = "null state pointer or negative step"; return QHP_EINVAL; }
+  if (step0 % s->n_alt != 0) { s->err = "step0 must be a multiple of n_alt"; return QHP_ESTATE; }
   if (s->th.kind == QHP_THERMO_ADQTB && step0 % s->n_seg != 0) { s->err = "adQTB state can only be set at a segment boundary"; return QHP_ESTATE; }
   int rc = qhp_nm_to_modes(s, x_beads, p_beads);
   if (rc) return rc;
@@ -408,6 +409,7 @@ extern "C" int qhp_profile_read(qhp_system *s, double *ms_host, int64_t *n_host)
 extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
   if (!s || nsteps < 0) return QHP_EINVAL;
   if (!s->have_state) { s->err = "qhp_step before qhp_set_state"; return QHP_ESTATE; }
+  if (nsteps % s->n_alt != 0) { s->err = "nsteps must be a multiple of n_alt (qhp_set_respa)"; return QHP_EINVAL; }
   const bool adqtb = s->th.kind == QHP_THERMO_ADQTB;
   for (int64_t k = 0; k < nsteps; ++k) {
     const int64_t st = s->step;
@@ -423,15 +425,17 @@ extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
       if (rc) return rc;
     }
     s->pending_kick = true;
-    {
-      prof_scope ps(s, 1);
-      rc = qhp_cells_rebuild(s, false);                   // R7 (returns at once on the device unless needed)
-      if (rc) return rc;
-    }
-    {
-      prof_scope ps(s, 2);
-      rc = qhp_pair_forces(s, false);                     // R8
-      if (rc) return rc;
+    if ((st + 1) % s->n_alt == 0) {                       // RESPA: V_s only after the last inner step (Eq. 19)
+      {
+        prof_scope ps(s, 1);
+        rc = qhp_cells_rebuild(s, false);                 // R7 (returns at once on the device unless needed)
+        if (rc) return rc;
+      }
+      {
+        prof_scope ps(s, 2);
+        rc = qhp_pair_forces(s, false);                   // R8
+        if (rc) return rc;
+      }
     }
     s->step = st + 1;
     if (adqtb && s->step % s->n_seg == 0) {
@@ -440,6 +444,15 @@ extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
       if (rc) return rc;
     }
   }
+  return QHP_OK;
+}
+
+extern "C" int qhp_set_respa(qhp_system *s, int n_alt) {
+  if (!s) return QHP_EINVAL;
+  if (n_alt < 1) { s->err = "n_alt must be >= 1"; return QHP_EINVAL; }
+  if (s->th.kind == QHP_THERMO_ADQTB && n_alt != 1) { s->err = "RESPA is not available with adQTB"; return QHP_EINVAL; }
+  if (s->have_state && s->step % n_alt != 0) { s->err = "n_alt must divide the current step index"; return QHP_ESTATE; }
+  s->n_alt = n_alt;
   return QHP_OK;
 }
 

@@ -50,6 +50,7 @@ struct qhp_system {
   // ---- configuration (host) ----
   int N = 0, nt = 0, n_mol = 0, n_bonds = 0, n_angles = 0;
   int P = 1, Pc = 1;
+  int n_alt = 1;                           // BAOAB-RESPA: inner steps per V_s kick (Eq. 19); 1 = plain BAOAB
   double dt = 0, T = 0;
   qhp_thermostat th{};
   double box[3]{}, inv_box[3]{};
