@@ -422,13 +422,24 @@ def qtb_adapt(top: Topology, n_seg: int, gamma0: float, a_gamma: float, gmin_fra
     return g
 
 
+def qtb_adapt_ratio(top: Topology, n_seg: int, gamma0: float, gmin_frac: float, dt: float, tau, first: bool,
+                    Cvv, CvF, avv, avf, gamma):
+    """RATIO adaptation (Eq. 24-26) of the types with tau[z] > 0; returns (gamma, avv, avf) copies."""
+    g, av, af = _f64(gamma).copy(), _f64(avv).copy(), _f64(avf).copy()
+    Cvv, CvF, tau = _f64(Cvv), _f64(CvF), _f64(tau)
+    lib().qo_qtb_adapt_ratio(C.c_int(top.n_types), C.c_int(n_seg), _p(top.mass), C.c_double(gamma0),
+                             C.c_double(gmin_frac), C.c_double(dt), _p(tau), C.c_int(int(first)), _p(Cvv), _p(CvF),
+                             _p(av), _p(af), _p(g))
+    return g, av, af
+
+
 class Adqtb:
     """adQTB driver: segments of n_seg steps, noise generated at segment start
     (l.203-209), spectra + SIMPLE adaptation at segment end (l.213-232, 248)."""
 
     def __init__(self, top: Topology, dt_ps: float, T_K: float, gamma0: float, seed: int,
                  n_seg: int, a_gamma: float, gmin_frac: float = 0.01, classical: bool = False,
-                 direct: bool = False, cells: bool | None = None):
+                 direct: bool = False, cells: bool | None = None, ratio_tau=None):
         self.top, self.dt, self.T, self.gamma0, self.seed = top, dt_ps, T_K, gamma0, seed
         self.n_seg, self.a_gamma, self.gmin_frac = n_seg, a_gamma, gmin_frac
         self.classical, self.direct = classical, direct
@@ -438,6 +449,11 @@ class Adqtb:
         self.Fc = None
         self.vseg = np.zeros((3 * top.n_atoms, n_seg))
         self.history = []           # (Cvv, CvF, gamma_after) per finished segment
+        # RATIO adaptation (Eq. 24-26) for the types with ratio_tau[z] > 0 ps, SIMPLE (Eq. 23) for the others
+        self.ratio_tau = None if ratio_tau is None else np.asarray(ratio_tau, float)
+        self.avv = np.zeros((top.n_types, n_seg + 1))
+        self.avf = np.zeros((top.n_types, n_seg + 1))
+        self.ratio_started = False
 
     def set_state(self, x, p, step0: int = 0):
         assert step0 % self.n_seg == 0
@@ -473,8 +489,17 @@ class Adqtb:
             if self.step_index % self.n_seg == 0:
                 fn = qtb_spectra_direct if self.direct else qtb_spectra_fft
                 Cvv, CvF = fn(self.top, self.n_seg, self.dt, self.vseg, self.Fc)
-                self.gamma = qtb_adapt(self.top, self.n_seg, self.gamma0, self.a_gamma,
-                                       self.gmin_frac, Cvv, CvF, self.gamma)
+                g_simple = qtb_adapt(self.top, self.n_seg, self.gamma0, self.a_gamma,
+                                     self.gmin_frac, Cvv, CvF, self.gamma)
+                if self.ratio_tau is not None and (self.ratio_tau > 0).any():
+                    g_ratio, self.avv, self.avf = qtb_adapt_ratio(
+                        self.top, self.n_seg, self.gamma0, self.gmin_frac, self.dt, self.ratio_tau,
+                        not self.ratio_started, Cvv, CvF, self.avv, self.avf, self.gamma)
+                    self.ratio_started = True
+                    for z in range(self.top.n_types):
+                        if self.ratio_tau[z] > 0:
+                            g_simple[z] = g_ratio[z]
+                self.gamma = g_simple
                 self.history.append((Cvv, CvF, self.gamma.copy()))
 
     def get_state(self):

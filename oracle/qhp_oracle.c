@@ -728,3 +728,37 @@ void qo_qtb_adapt(int n_types, int n_seg, const double *mass_amu, double gamma0,
   }
   free(dl);
 }
+
+/* ------------------------------------------------------------------------------------------
+ * NEXT-2  RATIO adaptation (Eq. 24-26) for the types with tau[z] > 0:
+ *   <C>_tau^(k) = <C>_tau^(k-1) w + C^(k) (1 - w),  w = exp(-N_seg dt / tau_z)          (Eq. 26)
+ *   gamma_z(omega_j) = Re<C_vF,z>(omega_j) / (m_z <C_vv,z>(omega_j))                    (Eq. 25)
+ *   gamma_z <- max(gamma_min, gamma_z)                                                  (l.248)
+ * avv, avf: the running averages [n_types][n_seg+1], in/out.  Reading G24 (paper silent on k = 1):
+ * the first segment initialises the averages with its own spectra (`first` != 0).  A bin whose
+ * averaged C_vv is not positive keeps its gamma.  m_z in kcal/mol ps^2/A^2 as in O10/O11.
+ * Types with tau[z] <= 0 are left untouched (SIMPLE, qo_qtb_adapt, handles them).
+ * Pins (tests/test_oracle_ratio.py): closed form of the window recursion; Eq. 24 (a gamma with
+ * Delta_FDT = 0 under the SIMPLE definition is a fixed point); the free-particle ratio (1 - a)/b.
+ * ------------------------------------------------------------------------------------------ */
+void qo_qtb_adapt_ratio(int n_types, int n_seg, const double *mass_amu, double gamma0, double gmin_frac,
+                        double dt, const double *tau, int first, const double *Cvv, const double *CvF,
+                        double *avv, double *avf, double *gamma) {
+  int nf = n_seg + 1;
+  double gmin = gmin_frac * gamma0;
+  for (int z = 0; z < n_types; ++z) {
+    if (!(tau[z] > 0.0)) continue;
+    double w = first ? 0.0 : exp(-(double)n_seg * dt / tau[z]);
+    for (int j = 0; j < nf; ++j) {
+      int k = z * nf + j;
+      avv[k] = avv[k] * w + Cvv[k] * (1.0 - w);
+      avf[k] = avf[k] * w + CvF[k] * (1.0 - w);
+      double den = mass_amu[z] / QO_ACC * avv[k];
+      if (den > 0.0) {
+        double g = avf[k] / den;
+        gamma[k] = g > gmin ? g : gmin;
+      }
+    }
+  }
+}
+
