@@ -138,6 +138,12 @@ int qhp_contracted(qhp_system *sys, double *xc);
 /* adQTB: gamma_z(omega_j) [n_types][n_seg+1]; coloured force segment Fc and recorded
  * velocities vseg, both [3 n_atoms][n_seg] (NULL to skip). */
 int qhp_adqtb_gamma(qhp_system *sys, double *gamma);
+/* adQTB: RATIO adaptation (Eq. 24-26) for the atom types with tau_ps[z] > 0:
+ * gamma_z = Re<C_vF,z> / (m_z <C_vv,z>) from exponential-window averages of the segment spectra with
+ * time constant tau_ps[z] (the first segment after this call initialises them); the other types keep
+ * the SIMPLE rule (Eq. 23, thermostat a_gamma).  tau_ps: HOST pointer [n_types], or NULL for SIMPLE on
+ * every type.  Synchronises. */
+int qhp_adqtb_ratio(qhp_system *sys, const double *tau_ps);
 int qhp_adqtb_segment(qhp_system *sys, double *Fc, double *vseg);
 /* Counters for measurement: out_host[0] = neighbour-list rebuilds so far, [1] = list entries,
  * [2] = pair-bead interactions inside r_cut at the current positions (full list, both

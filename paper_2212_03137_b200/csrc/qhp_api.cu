@@ -282,7 +282,7 @@ extern "C" int qhp_destroy(qhp_system *s) {
                   s->d_Tc, s->pos4, s->Fs, s->cent4, s->cref, s->pair_tab, s->cell_of, s->cell_count, s->cell_start,
                   s->cell_cursor, s->cell_tmp, s->order, s->rank, s->nbr, s->nbr16, s->nbr_count, s->d2max, s->counters,
                   s->red, s->obs, s->gamma, s->Hf, s->hk, s->H4, s->Fc, s->vseg, s->tw, s->atoms_by_type,
-                  s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p};
+                  s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p, s->ratio_tau, s->ratio_avv, s->ratio_avf};
   for (void *p : ptrs) if (p) cudaFree(p);
   delete s;
   return QHP_OK;
@@ -523,6 +523,25 @@ extern "C" int qhp_adqtb_gamma(qhp_system *s, double *gamma) {
   if (!s || !gamma) return QHP_EINVAL;
   if (s->th.kind != QHP_THERMO_ADQTB) { s->err = "not an adQTB system"; return QHP_ESTATE; }
   QHP_CUDA_OK(s, cudaMemcpyAsync(gamma, s->gamma, sizeof(double) * s->nt * (s->n_seg + 1), cudaMemcpyDeviceToDevice, s->stream));
+  return QHP_OK;
+}
+
+extern "C" int qhp_adqtb_ratio(qhp_system *s, const double *tau_ps) {
+  if (!s) return QHP_EINVAL;
+  if (s->th.kind != QHP_THERMO_ADQTB) { s->err = "not an adQTB system"; return QHP_ESTATE; }
+  const size_t nf = (size_t)s->n_seg + 1;
+  if (!tau_ps) {                                        // back to SIMPLE for every type
+    if (s->ratio_tau) { cudaStreamSynchronize(s->stream); cudaFree(s->ratio_tau); s->ratio_tau = nullptr; }
+    return QHP_OK;
+  }
+  if (!s->ratio_tau) QHP_CUDA_OK(s, cudaMalloc(&s->ratio_tau, sizeof(double) * s->nt));
+  if (!s->ratio_avv) QHP_CUDA_OK(s, cudaMalloc(&s->ratio_avv, sizeof(double) * s->nt * nf));
+  if (!s->ratio_avf) QHP_CUDA_OK(s, cudaMalloc(&s->ratio_avf, sizeof(double) * s->nt * nf));
+  QHP_CUDA_OK(s, cudaMemcpyAsync(s->ratio_tau, tau_ps, sizeof(double) * s->nt, cudaMemcpyHostToDevice, s->stream));
+  QHP_CUDA_OK(s, cudaMemsetAsync(s->ratio_avv, 0, sizeof(double) * s->nt * nf, s->stream));
+  QHP_CUDA_OK(s, cudaMemsetAsync(s->ratio_avf, 0, sizeof(double) * s->nt * nf, s->stream));
+  QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));     // tau_ps is the caller's host buffer
+  s->ratio_started = false;
   return QHP_OK;
 }
 

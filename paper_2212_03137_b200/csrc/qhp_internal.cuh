@@ -115,6 +115,9 @@ struct qhp_system {
   double *spec_part = nullptr;     // [n_spec_cta][2][n_seg+1]
   double *Cvv = nullptr, *CvF = nullptr; // [nt][n_seg+1]
   int64_t fc_segment = -1;
+  double *ratio_tau = nullptr;             // [nt] ps, > 0: RATIO adaptation of that type (Eq. 24-26); NULL: SIMPLE for all
+  double *ratio_avv = nullptr, *ratio_avf = nullptr;   // [nt][n_seg+1] exponential-window averages (Eq. 26)
+  bool ratio_started = false;
 
   // ---- per-phase profiling (qhp_profile) ----
   bool prof = false;

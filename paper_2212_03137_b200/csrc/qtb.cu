@@ -268,10 +268,12 @@ __global__ void k_qtb_reduce(int nt, int n_seg, int n_cta, const int32_t *__rest
 
 // Q7: one CTA per type
 __global__ void k_qtb_adapt(int n_seg, const double *__restrict__ mass, double gamma0, double a_gamma, double gmin_frac,
-                            const double *__restrict__ Cvv, const double *__restrict__ CvF, double *gamma) {
+                            const double *__restrict__ Cvv, const double *__restrict__ CvF, double *gamma,
+                            const double *__restrict__ tau) {
   __shared__ double scratch[32];
   __shared__ double nrm_s;
   const int z = blockIdx.x, nf = n_seg + 1, t = threadIdx.x;
+  if (tau && tau[z] > 0.0) return;              // a RATIO type (k_qtb_adapt_ratio)
   const double mz = mass[z] / QHP_ACC;
   double s = 0.0;
   for (int j = t; j < nf; j += blockDim.x) {
@@ -296,6 +298,28 @@ __global__ void k_qtb_adapt(int n_seg, const double *__restrict__ mass, double g
     const double dl = mz * gamma[z * nf + j] * Cvv[z * nf + j] - CvF[z * nf + j];
     const double g = gamma[z * nf + j] - a_gamma * gamma0 * dl / nrm;
     gamma[z * nf + j] = g > gmin ? g : gmin;
+  }
+}
+
+// RATIO adaptation (Eq. 24-26) for the types with tau[z] > 0: exponential-window
+// averages of the per-type spectra (Eq. 26; the first segment initialises them, reading G24), then
+// gamma_z = Re<C_vF> / (m_z <C_vv>) (Eq. 25) with the lower bound of l.248.  Runs after k_qtb_adapt,
+// which leaves these types alone.
+__global__ void k_qtb_adapt_ratio(int nt, int n_seg, const double *__restrict__ mass, double gamma0, double gmin_frac,
+                                  double dt, const double *__restrict__ tau, int first, const double *__restrict__ Cvv,
+                                  const double *__restrict__ CvF, double *avv, double *avf, double *gamma) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nf = n_seg + 1;
+  if (idx >= nt * nf) return;
+  const int z = idx / nf;
+  if (!(tau[z] > 0.0)) return;
+  const double w = first ? 0.0 : exp(-(double)n_seg * dt / tau[z]);
+  const double av = avv[idx] * w + Cvv[idx] * (1.0 - w), af = avf[idx] * w + CvF[idx] * (1.0 - w);
+  avv[idx] = av; avf[idx] = af;
+  const double den = mass[z] / QHP_ACC * av;
+  if (den > 0.0) {
+    const double g = af / den, gmin = gmin_frac * gamma0;
+    gamma[idx] = g > gmin ? g : gmin;
   }
 }
 
@@ -388,8 +412,16 @@ int qhp_qtb_adapt(qhp_system *s) {
                                                            s->spec_part + (size_t)s->n_spec_cta * 2 * nf, s->dt, s->Cvv, s->CvF);
   QHP_LAUNCH_OK(s);
   if (s->th.a_gamma != 0.0) {
-    k_qtb_adapt<<<nt, 256, 0, s->stream>>>(ns, s->dt_.mass, s->th.gamma0, s->th.a_gamma, s->th.gamma_min_frac, s->Cvv, s->CvF, s->gamma);
+    k_qtb_adapt<<<nt, 256, 0, s->stream>>>(ns, s->dt_.mass, s->th.gamma0, s->th.a_gamma, s->th.gamma_min_frac, s->Cvv, s->CvF, s->gamma,
+                                           s->ratio_tau);
     QHP_LAUNCH_OK(s);
+  }
+  if (s->ratio_tau) {
+    k_qtb_adapt_ratio<<<(nt * nf + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->dt_.mass, s->th.gamma0, s->th.gamma_min_frac, s->dt,
+                                                                    s->ratio_tau, s->ratio_started ? 0 : 1, s->Cvv, s->CvF,
+                                                                    s->ratio_avv, s->ratio_avf, s->gamma);
+    QHP_LAUNCH_OK(s);
+    s->ratio_started = true;
   }
   return QHP_OK;
 }

@@ -85,3 +85,29 @@ def test_c1_first_segment_and_boundary():
     assert dv < 1e-4
     assert np.abs(g - ref.gamma).max() < max(1e-9, 100 * dv) * ref.gamma.max()
     sysg.check()
+
+
+@pytest.mark.parametrize("tau", [[0.05, -1.0], [0.02, 0.1]])
+def test_ratio_adaptation_matches_oracle(tau):
+    """RATIO adaptation (Eq. 24-26) for the types with tau > 0, SIMPLE (Eq. 23) for the others:
+    gamma_z(omega) after each of four segments, and the trajectory they drive."""
+    top = W.water_box(216)
+    n_seg = 64
+    sysg, ref, x0, p0 = make_pair(top, 1, 1, 0.5, "adqtb", gamma0=20.0, n_seg=n_seg, a_gamma=0.5)
+    ref.ratio_tau = np.asarray(tau, float)
+    sysg.adqtb_ratio(tau)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    for seg in range(4):
+        sysg.step(n_seg)
+        ref.step(n_seg)
+        g = sysg.adqtb_gamma().cpu().numpy()
+        assert np.abs(g - ref.gamma).max() < 1e-8 * np.abs(ref.gamma).max(), seg
+    x1, _, _ = sysg.get_state()
+    assert np.abs(x1.cpu().numpy() - ref.get_state()[0]).max() < 1e-7
+    sysg.adqtb_ratio(None)                      # back to SIMPLE for every type
+    sysg.step(n_seg)
+    ref.ratio_tau = None
+    ref.step(n_seg)
+    assert np.abs(sysg.adqtb_gamma().cpu().numpy() - ref.gamma).max() < 1e-7 * np.abs(ref.gamma).max()
+    sysg.check()
