@@ -27,7 +27,7 @@
 #include "qhp_internal.cuh"
 
 #ifndef STG_THREADS
-#define STG_THREADS 768           // largest CTA; the host launches fewer warps when shared memory is short
+#define STG_THREADS 896           // largest CTA (28 warps, 68 registers); the host launches fewer warps when shared memory is short
 #endif
 #define STG_MAX_WARPS (STG_THREADS / 32)
 #define STG_BLOCK 256             // list entries per row block (8 per lane)
@@ -346,7 +346,7 @@ int qhp_pair_staged_partials(const qhp_system *s) { return s->ncell * 8 * s->Pc;
 // Largest CTA (in warps) whose queues leave room for `region` staged atoms (+ 1/16 for drift between
 // list builds); sets staged_warps / staged_cap.  False: the neighbourhood does not fit at all.
 bool qhp_pair_staged_fit(qhp_system *s, long long region) {
-  static const int tries[] = {STG_MAX_WARPS, 16, 12, 8};
+  static const int tries[] = {STG_MAX_WARPS, 24, 16, 12, 8};
   const long long need = region + region / 16 + 32;
   for (int w : tries) {
     if (w > STG_MAX_WARPS) continue;
