@@ -355,6 +355,105 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// P = 1 (classical BAOAB, adQTB) with molecules of at most 4 atoms: one THREAD per molecule.  With a
+// single bead there is no normal-mode transform, so the tile exchange of k_integrate only served the
+// bonded terms; a thread that owns a whole molecule needs no shared memory and no barrier, and the
+// kernel is no longer a chain of short latency-bound phases (C3: 0.09 -> see profiles).
+// Forces are accumulated in registers through predicated adds (static indices, no local memory).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void acc4(double (&f)[4][3], int ai, double gx, double gy, double gz) {
+#pragma unroll
+  for (int k = 0; k < 4; ++k)
+    if (ai == k) { f[k][0] += gx; f[k][1] += gy; f[k][2] += gz; }
+}
+
+template <int THERMO>
+__global__ void __launch_bounds__(128) k_integrate_mol1(const IntArgs a, int n_mol) {
+  __shared__ double scratch[32];
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (blockIdx.x == 0 && threadIdx.x == 0 && a.do_step) a.d2max[(a.step + 1) & 1] = 0ull;
+  double d2 = 0.0;
+  if (m < n_mol) {
+    const int s0 = a.mol_atom_start[m], na = a.mol_atom_start[m + 1] - s0;
+    const double *x = a.Q + 3LL * s0;                 // P = 1: bead positions are Q_0
+    double f[4][3];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) f[k][0] = f[k][1] = f[k][2] = 0.0;
+    for (int b = a.mol_bond_start[m]; b < a.mol_bond_start[m + 1]; ++b) {
+      const int ai = a.bond_idx[2 * b] - s0, aj = a.bond_idx[2 * b + 1] - s0;
+      const double dx = x[3 * ai] - x[3 * aj], dy = x[3 * ai + 1] - x[3 * aj + 1], dz = x[3 * ai + 2] - x[3 * aj + 2];
+      const double r = sqrt(dx * dx + dy * dy + dz * dz);
+      const double g = -a.bond_k[b] * (r - a.bond_r0[b]) / r;
+      acc4(f, ai, g * dx, g * dy, g * dz);
+      acc4(f, aj, -g * dx, -g * dy, -g * dz);
+    }
+    for (int g = a.mol_angle_start[m]; g < a.mol_angle_start[m + 1]; ++g) {
+      const int ai = a.angle_idx[3 * g] - s0, aj = a.angle_idx[3 * g + 1] - s0, ak = a.angle_idx[3 * g + 2] - s0;   // aj = centre
+      const double ux = x[3 * ai] - x[3 * aj], uy = x[3 * ai + 1] - x[3 * aj + 1], uz = x[3 * ai + 2] - x[3 * aj + 2];
+      const double vx = x[3 * ak] - x[3 * aj], vy = x[3 * ak + 1] - x[3 * aj + 1], vz = x[3 * ak + 2] - x[3 * aj + 2];
+      const double ru = sqrt(ux * ux + uy * uy + uz * uz), rv = sqrt(vx * vx + vy * vy + vz * vz);
+      const double iruv = 1.0 / (ru * rv);
+      double cs = (ux * vx + uy * vy + uz * vz) * iruv;
+      cs = fmin(1.0, fmax(-1.0, cs));
+      const double dth = acos(cs) - a.angle_th0[g];
+      const double gg = a.angle_k[g] * dth / sqrt(1.0 - cs * cs);
+      const double cu = cs / (ru * ru), cv = cs / (rv * rv);
+      const double fix = gg * (vx * iruv - cu * ux), fiy = gg * (vy * iruv - cu * uy), fiz = gg * (vz * iruv - cu * uz);
+      const double fkx = gg * (ux * iruv - cv * vx), fky = gg * (uy * iruv - cv * vy), fkz = gg * (uz * iruv - cv * vz);
+      acc4(f, ai, fix, fiy, fiz);
+      acc4(f, ak, fkx, fky, fkz);
+      acc4(f, aj, -(fix + fkx), -(fiy + fky), -(fiz + fkz));
+    }
+    if (a.tether_k)
+      for (int al = 0; al < na; ++al) {
+        const double k = a.tether_k[a.type[s0 + al]];
+        acc4(f, al, -k * x[3 * al], -k * x[3 * al + 1], -k * x[3 * al + 2]);
+      }
+    // every position of the molecule has been read: update its atoms in place
+#pragma unroll
+    for (int al = 0; al < 4; ++al) {
+      if (al >= na) break;
+      const int atom = s0 + al;
+      const int ty = a.type[atom];
+      const double mass = a.mass[ty];
+      const long long slot = a.rank[atom];
+      const double *cf = a.coef + ty * QHP_NCOEF;
+      double z[3] = {0.0, 0.0, 0.0};
+      if (THERMO == 1 && a.do_step) qhp_normals3(a.seed, (uint32_t)atom, 0u, QHP_TAG_PILE, (uint64_t)a.step, z);
+      double dsum = 0.0;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const long long dof = 3LL * atom + c;
+        double q = a.Q[dof], p = a.Pm[dof];
+        p += a.w_fast * f[al][c] + a.w_slow * a.Fs[slot * 3 + c];
+        if (a.do_step) {
+          q += a.hdt * p / mass;
+          if (THERMO == 1) {
+            p = __ldg(cf + 3) * p + __ldg(cf + 4) * z[c];
+          } else if (THERMO == 2) {
+            const long long k = dof * a.n_seg + a.n_loc;
+            const double pn = a.qa * p + a.qbA * a.Fc[k];
+            a.vseg[k] = (p + pn) / (2.0 * mass);
+            p = pn;
+          }
+          q += a.hdt * p / mass;
+          a.Q[dof] = q;
+          a.pos4[slot * 4 + c] = q;
+          const double dd = q - a.cref[dof];
+          dsum += dd * dd;
+        }
+        a.Pm[dof] = p;
+      }
+      d2 = fmax(d2, dsum);
+    }
+  }
+  if (a.do_step) {
+    d2 = block_max(d2, scratch);
+    if (threadIdx.x == 0) atomicMax(&a.d2max[a.step & 1], (unsigned long long)__double_as_longlong(d2));
+  }
+}
+
 // bead-space forces G_i = sqrt(P) sum_n T_in f_n (O7)
 template <int P>
 __global__ void __launch_bounds__(288) k_bead_forces(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab) {
@@ -582,6 +681,14 @@ int qhp_nm_integrate(qhp_system *s, bool kick_prev, bool do_step, int64_t step) 
   }
   const size_t smem = s->int_smem;
   const int thermo = s->th.kind;
+  if (s->P == 1 && s->int_mol1) {
+    const int tb = 128, grid = (s->n_mol + tb - 1) / tb;
+    if (thermo == QHP_THERMO_ADQTB) k_integrate_mol1<2><<<grid, tb, 0, s->stream>>>(a, s->n_mol);
+    else if (thermo == QHP_THERMO_PILE) k_integrate_mol1<1><<<grid, tb, 0, s->stream>>>(a, s->n_mol);
+    else k_integrate_mol1<0><<<grid, tb, 0, s->stream>>>(a, s->n_mol);
+    QHP_LAUNCH_OK(s);
+    return QHP_OK;
+  }
 #define LAUNCH_INT(PP, TH, PCM)                                                                  \
   {                                                                                              \
     QHP_CUDA_OK(s, set_smem(k_integrate<PP, TH, PCM>, smem));                                    \

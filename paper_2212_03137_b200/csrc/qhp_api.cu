@@ -160,6 +160,7 @@ extern "C" int qhp_create(const qhp_topology *top, int P, int P_contract, double
     if (cur.a1 > cur.a0) tiles.push_back(cur);
   }
   s->n_tiles = (int)tiles.size();
+  s->int_mol1 = P == 1 && max_mol <= 4;
   s->int_smem = sizeof(double) * (2 * (size_t)P * 3 * s->tile_atoms + 64);   // two [P][tile DOF] tiles + reduction scratch
 
   // ---- normal modes and per-(type, mode) coefficients of the A and O blocks ----------------------

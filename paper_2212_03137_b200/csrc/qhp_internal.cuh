@@ -69,6 +69,7 @@ struct qhp_system {
   qhp_dev_topology dt_{};
   int n_tiles = 0, tile_atoms = 0, tile_threads = 0;
   size_t int_smem = 0;
+  bool int_mol1 = false;                   // P = 1 and molecules of <= 4 atoms: thread-per-molecule integrator
   double *Q = nullptr, *Pm = nullptr;      // [P][3N] normal modes
   double *coef = nullptr;                  // [nt][P][QHP_NCOEF]
   double *d_Tc = nullptr;                  // [Pc][Pc] T^(Pc) on the device
