@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
 #pragma unroll
       for (int k = 0; k < PF; ++k) pl[k] = a.Pm[k * a.ND + dof];
     }
-    if (THERMO == 2 && a.do_step) fc_early = a.Fc[dof * a.n_seg + a.n_loc];
+    if (THERMO == 2 && a.do_step) fc_early = a.Fc[(long long)a.n_loc * a.ND + dof];
   }
 
   // ---- phase 1: Q -> bead positions (shared tile), V_f per (molecule, bead) -------------------------
@@ -310,7 +310,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
           p = __ldg(cf + n * QHP_NCOEF + 3) * p + __ldg(cf + n * QHP_NCOEF + 4) * ft[n * TD + t];
         } else if (THERMO == 2) {
           // classical BAOAB carrying the coloured force (Eq. 12, l.199; readings G14, G16)
-          const long long k = dof * a.n_seg + a.n_loc;
+          const long long k = (long long)a.n_loc * a.ND + dof;   // [n_seg][3N]: step-contiguous
           const double pn = a.qa * p + a.qbA * fc_early;
           a.vseg[k] = (p + pn) / (2.0 * m);
           p = pn;
@@ -432,7 +432,7 @@ __global__ void __launch_bounds__(128) k_integrate_mol1(const IntArgs a, int n_m
           if (THERMO == 1) {
             p = __ldg(cf + 3) * p + __ldg(cf + 4) * z[c];
           } else if (THERMO == 2) {
-            const long long k = dof * a.n_seg + a.n_loc;
+            const long long k = (long long)a.n_loc * a.ND + dof;   // [n_seg][3N]: step-contiguous
             const double pn = a.qa * p + a.qbA * a.Fc[k];
             a.vseg[k] = (p + pn) / (2.0 * mass);
             p = pn;

@@ -549,10 +549,11 @@ extern "C" int qhp_adqtb_ratio(qhp_system *s, const double *tau_ps) {
 extern "C" int qhp_adqtb_segment(qhp_system *s, double *Fc, double *vseg) {
   if (!s) return QHP_EINVAL;
   if (s->th.kind != QHP_THERMO_ADQTB) { s->err = "not an adQTB system"; return QHP_ESTATE; }
-  const size_t bytes = sizeof(double) * 3 * (size_t)s->N * s->n_seg;
-  if (Fc) QHP_CUDA_OK(s, cudaMemcpyAsync(Fc, s->Fc, bytes, cudaMemcpyDeviceToDevice, s->stream));
-  if (vseg) QHP_CUDA_OK(s, cudaMemcpyAsync(vseg, s->vseg, bytes, cudaMemcpyDeviceToDevice, s->stream));
-  return QHP_OK;
+  // internal layout is [n_seg][3N] (step-contiguous); the hook returns [3N][n_seg]
+  int rc = QHP_OK;
+  if (Fc) rc = qhp_qtb_export_segment(s, s->Fc, Fc);
+  if (!rc && vseg) rc = qhp_qtb_export_segment(s, s->vseg, vseg);
+  return rc;
 }
 
 extern "C" int qhp_counters(qhp_system *s, int64_t *out_host, int n_out) {

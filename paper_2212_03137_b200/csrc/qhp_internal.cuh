@@ -106,7 +106,7 @@ struct qhp_system {
   double *Hf = nullptr;      // [nt][n_seg+1] filter H_z
   double *hk = nullptr;      // [nt][2 n_seg] kernel h_z
   double *H4 = nullptr;      // [nt][4 n_seg][2] spectrum of the zero-padded shifted kernel
-  double *Fc = nullptr, *vseg = nullptr;  // [3N][n_seg]
+  double *Fc = nullptr, *vseg = nullptr;  // [n_seg][3N] (step-contiguous: the integrator reads/writes one row per step)
   double *tw = nullptr;      // twiddles exp(-2 pi i k / NT) [NT][2], NT = 4 n_seg
   int32_t *atoms_by_type = nullptr; // [N]
   std::vector<int> type_start;     // [nt+1] offsets into atoms_by_type
@@ -156,6 +156,7 @@ int qhp_pair_partials(const qhp_system *s);          // upper bound of per-CTA e
 int qhp_qtb_init(qhp_system *s);
 int qhp_qtb_generate(qhp_system *s, int64_t seg);
 int qhp_qtb_adapt(qhp_system *s);
+int qhp_qtb_export_segment(qhp_system *s, const double *in, double *out);   // [n_seg][3N] -> [3N][n_seg]
 int qhp_fft_launch(double *data, int n, int64_t batch, int sign, const double *tw, int tw_n, cudaStream_t st);
 
 #define QHP_CUDA_OK(s, call)                                                          \

@@ -178,7 +178,7 @@ __global__ void k_qtb_spectrum4(int nt, int n_seg, const double *__restrict__ hk
 // kernel h is real, so real and imaginary parts are filtered independently), z through a second.
 //   F_c[dof][n] = sum_k h_z[k] r(dof, seg*n_seg + n - k + n_seg),  n = 0..n_seg-1
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) k_qtb_noise(int n_seg, unsigned long long seed, long long seg, const int32_t *__restrict__ type,
+__global__ void __launch_bounds__(1024) k_qtb_noise(int n_seg, long long ND, unsigned long long seed, long long seg, const int32_t *__restrict__ type,
                             const double2 *__restrict__ H4, const double2 *__restrict__ tw, double *Fc) {
   extern __shared__ double2 nbuf[];
   const int nf = 4 * n_seg, nw = 3 * n_seg;
@@ -202,11 +202,11 @@ __global__ void __launch_bounds__(1024) k_qtb_noise(int n_seg, unsigned long lon
     for (int q = t; q < nf; q += blockDim.x) nbuf[q] = cmul(nbuf[q], Hz[q]);
     __syncthreads();
     fft_smem(nbuf, nf, +1, tw, nf);
-    double *out = Fc + (3LL * atom) * n_seg;
+    double *out = Fc + 3LL * atom;                        // Fc[n][dof]: step-contiguous for the integrator
     for (int n = t; n < n_seg; n += blockDim.x) {
       const double2 y = nbuf[n + 2 * n_seg];
-      if (pass == 0) { out[n] = y.x * inv; out[n_seg + n] = y.y * inv; }
-      else out[2LL * n_seg + n] = y.x * inv;
+      if (pass == 0) { out[n * ND] = y.x * inv; out[n * ND + 1] = y.y * inv; }
+      else out[n * ND + 2] = y.x * inv;
     }
     if (pass == 0) {
       __syncthreads();
@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(1024) k_qtb_noise(int n_seg, unsigned long lon
 // Q5 + Q6: spectra.  One CTA walks a run of atoms of one type; v and F_c of a DOF are the real and
 // imaginary part of one zero-padded N_k-point transform.  Per-CTA sums -> fixed-order reduction.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) k_qtb_spectra(int n_seg, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
+__global__ void __launch_bounds__(1024) k_qtb_spectra(int n_seg, long long ND, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
                               const double *__restrict__ vseg, const double *__restrict__ Fc,
                               const double2 *__restrict__ tw, int tw_n, double *part) {
   extern __shared__ double2 sbuf[];
@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(1024) k_qtb_spectra(int n_seg, const int32_t *
       const long long d = 3LL * atom + c;
       __syncthreads();
       for (int n = t; n < nk; n += blockDim.x)
-        sbuf[n] = (n < n_seg) ? make_double2(vseg[d * n_seg + n], Fc[d * n_seg + n]) : make_double2(0.0, 0.0);
+        sbuf[n] = (n < n_seg) ? make_double2(vseg[n * ND + d], Fc[n * ND + d]) : make_double2(0.0, 0.0);
       __syncthreads();
       fft_smem(sbuf, nk, -1, tw, tw_n);
       for (int j = t; j < nf; j += blockDim.x) {
@@ -323,6 +323,32 @@ __global__ void k_qtb_adapt_ratio(int nt, int n_seg, const double *__restrict__ 
   }
 }
 
+// parity hook: internal [n_seg][3N] -> documented [3N][n_seg]
+__global__ void k_seg_transpose(const double *__restrict__ in, double *__restrict__ out, long long ND, int n_seg) {
+  __shared__ double tile[32][33];
+  const long long d0 = (long long)blockIdx.x * 32;
+  const int n0 = blockIdx.y * 32;
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    const long long d = d0 + threadIdx.x;
+    const int n = n0 + r;
+    tile[r][threadIdx.x] = (d < ND && n < n_seg) ? in[n * ND + d] : 0.0;
+  }
+  __syncthreads();
+  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+    const long long d = d0 + r;
+    const int n = n0 + threadIdx.x;
+    if (d < ND && n < n_seg) out[d * n_seg + n] = tile[threadIdx.x][r];
+  }
+}
+
+int qhp_qtb_export_segment(qhp_system *s, const double *in, double *out) {
+  const long long ND = 3LL * s->N;
+  const dim3 grid((unsigned)((ND + 31) / 32), (unsigned)((s->n_seg + 31) / 32)), block(32, 8);
+  k_seg_transpose<<<grid, block, 0, s->stream>>>(in, out, ND, s->n_seg);
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
 __global__ void k_fill(double *p, long long n, double v) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) p[i] = v;
@@ -393,7 +419,7 @@ int qhp_qtb_generate(qhp_system *s, int64_t seg) {
   const int n4 = 4 * ns;
   const size_t smem = sizeof(double2) * n4 + sizeof(double) * 3 * ns;
   QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_noise, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_qtb_noise<<<s->N, fft_threads(n4), smem, s->stream>>>(ns, s->th.seed, seg, s->dt_.type, (const double2 *)s->H4,
+  k_qtb_noise<<<s->N, fft_threads(n4), smem, s->stream>>>(ns, 3LL * s->N, s->th.seed, seg, s->dt_.type, (const double2 *)s->H4,
                                                          (const double2 *)s->tw, s->Fc);
   QHP_LAUNCH_OK(s);
   s->fc_segment = seg;
@@ -405,7 +431,7 @@ int qhp_qtb_adapt(qhp_system *s) {
   const int ns = s->n_seg, nf = ns + 1, nt = s->nt, nk = 2 * ns;
   const size_t smem = sizeof(double2) * nk + sizeof(double) * 2 * nf;
   QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_spectra, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_qtb_spectra<<<s->n_spec_cta, fft_threads(nk), smem, s->stream>>>(ns, s->spec_cta, s->atoms_by_type, s->vseg, s->Fc,
+  k_qtb_spectra<<<s->n_spec_cta, fft_threads(nk), smem, s->stream>>>(ns, 3LL * s->N, s->spec_cta, s->atoms_by_type, s->vseg, s->Fc,
                                                                      (const double2 *)s->tw, 4 * ns, s->spec_part);
   QHP_LAUNCH_OK(s);
   k_qtb_reduce<<<(nt * nf + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->n_spec_cta, s->spec_cta, s->spec_part,
