@@ -196,17 +196,21 @@ __global__ void __launch_bounds__(1024) k_qtb_noise(int n_seg, long long ND, uns
     }
   }
   const double inv = 1.0 / (double)nf;
+  double fx = 0.0, fy = 0.0;              // blockDim.x >= n_seg: thread t owns output sample n = t
   for (int pass = 0; pass < 2; ++pass) {
     __syncthreads();
     fft_smem(nbuf, nf, -1, tw, nf);
     for (int q = t; q < nf; q += blockDim.x) nbuf[q] = cmul(nbuf[q], Hz[q]);
     __syncthreads();
     fft_smem(nbuf, nf, +1, tw, nf);
-    double *out = Fc + 3LL * atom;                        // Fc[n][dof]: step-contiguous for the integrator
-    for (int n = t; n < n_seg; n += blockDim.x) {
-      const double2 y = nbuf[n + 2 * n_seg];
-      if (pass == 0) { out[n * ND] = y.x * inv; out[n * ND + 1] = y.y * inv; }
-      else out[n * ND + 2] = y.x * inv;
+    if (t < n_seg) {
+      const double2 y = nbuf[t + 2 * n_seg];
+      if (pass == 0) { fx = y.x * inv; fy = y.y * inv; }
+      else {
+        // Fc[n][dof] (step-contiguous for the integrator): the three components of one sample together
+        double *out = Fc + (long long)t * ND + 3LL * atom;
+        out[0] = fx; out[1] = fy; out[2] = y.x * inv;
+      }
     }
     if (pass == 0) {
       __syncthreads();
@@ -227,13 +231,19 @@ __global__ void __launch_bounds__(1024) k_qtb_spectra(int n_seg, long long ND, c
   double *avv = reinterpret_cast<double *>(sbuf + nk), *avf = avv + nf;
   for (int j = t; j < nf; j += blockDim.x) { avv[j] = 0.0; avf[j] = 0.0; }
   const int b = cta_tab[3 * blockIdx.x + 1], e = cta_tab[3 * blockIdx.x + 2];
+  double2 *raw = reinterpret_cast<double2 *>(avf + nf);        // [3][n_seg] (v, F_c) of the atom's three DOFs
   for (int ia = b; ia < e; ++ia) {
     const int atom = atoms[ia];
+    __syncthreads();
+    for (int n = t; n < n_seg; n += blockDim.x) {               // one 24-byte piece per sample and array
+      const double *pv = vseg + (long long)n * ND + 3LL * atom, *pf = Fc + (long long)n * ND + 3LL * atom;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) raw[c * n_seg + n] = make_double2(pv[c], pf[c]);
+    }
     for (int c = 0; c < 3; ++c) {
-      const long long d = 3LL * atom + c;
       __syncthreads();
       for (int n = t; n < nk; n += blockDim.x)
-        sbuf[n] = (n < n_seg) ? make_double2(vseg[n * ND + d], Fc[n * ND + d]) : make_double2(0.0, 0.0);
+        sbuf[n] = (n < n_seg) ? raw[c * n_seg + n] : make_double2(0.0, 0.0);
       __syncthreads();
       fft_smem(sbuf, nk, -1, tw, tw_n);
       for (int j = t; j < nf; j += blockDim.x) {
@@ -429,7 +439,7 @@ int qhp_qtb_generate(qhp_system *s, int64_t seg) {
 // Q5-Q7 at the end of a segment
 int qhp_qtb_adapt(qhp_system *s) {
   const int ns = s->n_seg, nf = ns + 1, nt = s->nt, nk = 2 * ns;
-  const size_t smem = sizeof(double2) * nk + sizeof(double) * 2 * nf;
+  const size_t smem = sizeof(double2) * nk + sizeof(double) * 2 * (nf + 1) + sizeof(double2) * 3 * ns;
   QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_spectra, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   k_qtb_spectra<<<s->n_spec_cta, fft_threads(nk), smem, s->stream>>>(ns, 3LL * s->N, s->spec_cta, s->atoms_by_type, s->vseg, s->Fc,
                                                                      (const double2 *)s->tw, 4 * ns, s->spec_part);
