@@ -20,74 +20,114 @@ __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
   return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
 
-// tw[m] = exp(-2 pi i m / tw_n); returns exp(sign * 2 pi i * num / den), den | tw_n, 0 <= num < den
+// tw[m] = exp(-2 pi i m / tw_n); returns exp(sign * 2 pi i * num / den), den | tw_n (powers of two), 0 <= num < den
 __device__ __forceinline__ double2 twiddle(const double2 *__restrict__ tw, int tw_n, int num, int den, int sign) {
-  double2 w = tw[num * (tw_n / den)];
+  double2 w = tw[num * (tw_n >> (__ffs(den) - 1))];
   if (sign > 0) w.y = -w.y;
   return w;
 }
 
-// In-place Stockham FFT of buf[0..n) by blockDim.x >= n/4 threads (all threads of the CTA must call).
-// sign = -1 forward, +1 inverse (unnormalised).  Result in natural order.
-__device__ void fft_smem(double2 *buf, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
-  const int t = threadIdx.x;
-  for (int Ns = 1; Ns < n;) {
-    const int rem = n / Ns;
-    if ((rem & 3) == 0) {
-      const int nb = n >> 2;
-      double2 v0, v1, v2, v3;
-      int j0 = 0;
-      const bool on = t < nb;
-      if (on) {
-        const int k = t & (Ns - 1);
-        v0 = buf[t]; v1 = buf[t + nb]; v2 = buf[t + 2 * nb]; v3 = buf[t + 3 * nb];
+// 4-point DFT in place: (a, b, c, d) -> (X0, X1, X2, X3), X_v = sum_u x_u exp(SG 2 pi i u v / 4)
+template <int SG>
+__device__ __forceinline__ void dft4(double2 &a, double2 &b, double2 &c, double2 &d) {
+  const double2 t0 = make_double2(a.x + c.x, a.y + c.y), t1 = make_double2(a.x - c.x, a.y - c.y);
+  const double2 t2 = make_double2(b.x + d.x, b.y + d.y), e = make_double2(b.x - d.x, b.y - d.y);
+  const double2 t3 = (SG < 0) ? make_double2(e.y, -e.x) : make_double2(-e.y, e.x);   // (b - d) * (SG i)
+  a = make_double2(t0.x + t2.x, t0.y + t2.y); b = make_double2(t1.x + t3.x, t1.y + t3.y);
+  c = make_double2(t0.x - t2.x, t0.y - t2.y); d = make_double2(t1.x - t3.x, t1.y - t3.y);
+}
+
+// One Stockham pass of radix R (16, 4 or 2) at stride Ns over buf[0..n).  Every thread t < max(n/16, 1)
+// keeps 16 elements in registers: one radix-16 butterfly (two radix-4 layers without touching shared
+// memory in between: half the shared-memory traffic of two radix-4 passes, which bounded the first
+// version of the noise kernel), or 4 radix-4 / 8 radix-2 butterflies.  Reads are contiguous in t.
+// Input twiddles w^(k u) are successive powers of one table entry w^k (<= 15 products, ~1e-14 relative).
+template <int R, int SG>
+__device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const double2 *__restrict__ tw, int tw_n) {
+  constexpr int G = 16 / R;                       // butterflies per thread
+  const int nth = n >= 16 ? n >> 4 : 1, nb = n / R, t = threadIdx.x;
+  const bool on = t < nth;
+  double2 v[16];
+  int j0[G];
+  if (on) {
+#pragma unroll
+    for (int q = 0; q < G; ++q) {
+      const int j = t + q * nth;
+      j0[q] = -1;
+      if (j < nb) {
+        const int k = j & (Ns - 1);
+#pragma unroll
+        for (int u = 0; u < R; ++u) v[q * R + u] = buf[j + u * nb];
         if (k) {
-          v1 = cmul(v1, twiddle(tw, tw_n, k, Ns * 4, sign));
-          v2 = cmul(v2, twiddle(tw, tw_n, 2 * k, Ns * 4, sign));
-          v3 = cmul(v3, twiddle(tw, tw_n, 3 * k, Ns * 4, sign));
-        }
-        j0 = (t - k) * 4 + k;
-      }
-      __syncthreads();
-      if (on) {
-        const double2 t0 = make_double2(v0.x + v2.x, v0.y + v2.y), t1 = make_double2(v0.x - v2.x, v0.y - v2.y);
-        const double2 t2 = make_double2(v1.x + v3.x, v1.y + v3.y);
-        const double2 d = make_double2(v1.x - v3.x, v1.y - v3.y);
-        // (v1 - v3) * (sign * i)
-        const double2 t3 = (sign < 0) ? make_double2(d.y, -d.x) : make_double2(-d.y, d.x);
-        buf[j0] = make_double2(t0.x + t2.x, t0.y + t2.y);
-        buf[j0 + Ns] = make_double2(t1.x + t3.x, t1.y + t3.y);
-        buf[j0 + 2 * Ns] = make_double2(t0.x - t2.x, t0.y - t2.y);
-        buf[j0 + 3 * Ns] = make_double2(t1.x - t3.x, t1.y - t3.y);
-      }
-      __syncthreads();
-      Ns <<= 2;
-    } else {
-      const int nb = n >> 1;
-      double2 a[2], b[2];
-      int j0[2];
+          const double2 w1 = twiddle(tw, tw_n, k, Ns * R, SG);
+          double2 w = w1;
 #pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        const int j = t + u * (nb >> 1);
-        j0[u] = -1;
-        if (t < (nb >> 1) || (nb == 1 && t == 0 && u == 0)) {
-          const int k = j & (Ns - 1);
-          a[u] = buf[j]; b[u] = buf[j + nb];
-          if (k) b[u] = cmul(b[u], twiddle(tw, tw_n, k, Ns * 2, sign));
-          j0[u] = (j - k) * 2 + k;
+          for (int u = 1; u < R; ++u) {
+            v[q * R + u] = cmul(v[q * R + u], w);
+            if (u + 1 < R) w = cmul(w, w1);
+          }
         }
+        j0[q] = (j - k) * R + k;
       }
-      __syncthreads();
-#pragma unroll
-      for (int u = 0; u < 2; ++u)
-        if (j0[u] >= 0) {
-          buf[j0[u]] = make_double2(a[u].x + b[u].x, a[u].y + b[u].y);
-          buf[j0[u] + Ns] = make_double2(a[u].x - b[u].x, a[u].y - b[u].y);
-        }
-      __syncthreads();
-      Ns <<= 1;
     }
   }
+  __syncthreads();
+  if (on) {
+    if (R == 16) {
+      if (j0[0] >= 0) {
+        // u = 4 a + b: 4-point DFTs over a, twiddles w16^(b c), 4-point DFTs over b; X[c + 4 d] ends in v[4 c + d]
+#pragma unroll
+        for (int b = 0; b < 4; ++b) dft4<SG>(v[b], v[4 + b], v[8 + b], v[12 + b]);
+        const double c8 = 0.92387953251128673848, s8 = 0.38268343236508978178, r2 = 0.70710678118654752440;
+        const double sg = (SG < 0) ? -1.0 : 1.0;
+        // after the first layer v[4 c + b] = T[b][c]
+        v[5] = cmul(v[5], make_double2(c8, sg * s8));        // b c = 1
+        v[6] = cmul(v[6], make_double2(r2, sg * r2));        // 2
+        v[7] = cmul(v[7], make_double2(s8, sg * c8));        // 3
+        v[9] = cmul(v[9], make_double2(r2, sg * r2));        // 2
+        v[10] = make_double2(-sg * v[10].y, sg * v[10].x);   // 4: multiply by (SG i)
+        v[11] = cmul(v[11], make_double2(-r2, sg * r2));     // 6
+        v[13] = cmul(v[13], make_double2(s8, sg * c8));      // 3
+        v[14] = cmul(v[14], make_double2(-r2, sg * r2));     // 6
+        v[15] = cmul(v[15], make_double2(-c8, -sg * s8));    // 9
+#pragma unroll
+        for (int c = 0; c < 4; ++c) dft4<SG>(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+          for (int d = 0; d < 4; ++d) buf[j0[0] + (c + 4 * d) * Ns] = v[4 * c + d];
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < G; ++q)
+        if (j0[q] >= 0) {
+          if (R == 4) {
+            dft4<SG>(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) buf[j0[q] + u * Ns] = v[4 * q + u];
+          } else {
+            const double2 x0 = v[2 * q], x1 = v[2 * q + 1];
+            buf[j0[q]] = make_double2(x0.x + x1.x, x0.y + x1.y);
+            buf[j0[q] + Ns] = make_double2(x0.x - x1.x, x0.y - x1.y);
+          }
+        }
+    }
+  }
+  __syncthreads();
+}
+
+// In-place Stockham FFT of buf[0..n) by blockDim.x >= max(n/16, 1) threads (all threads of the CTA
+// must call).  sign = -1 forward, +1 inverse (unnormalised).  Result in natural order.
+template <int SG>
+__device__ __forceinline__ void fft_smem_sg(double2 *buf, int n, const double2 *__restrict__ tw, int tw_n) {
+  int Ns = 1;
+  while (n / Ns >= 16 && ((n / Ns) & 15) == 0) { fft_pass<16, SG>(buf, n, Ns, tw, tw_n); Ns <<= 4; }
+  while (((n / Ns) & 3) == 0 && Ns < n) { fft_pass<4, SG>(buf, n, Ns, tw, tw_n); Ns <<= 2; }
+  while (Ns < n) { fft_pass<2, SG>(buf, n, Ns, tw, tw_n); Ns <<= 1; }
+}
+__device__ __noinline__ void fft_smem(double2 *buf, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
+  if (sign < 0) fft_smem_sg<-1>(buf, n, tw, tw_n);
+  else fft_smem_sg<1>(buf, n, tw, tw_n);
 }
 
 __global__ void k_twiddle(double2 *tw, int n) {
@@ -98,7 +138,7 @@ __global__ void k_twiddle(double2 *tw, int n) {
   tw[m] = make_double2(c, s);
 }
 
-__global__ void __launch_bounds__(1024) k_fft_batch(double2 *data, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
+__global__ void __launch_bounds__(512) k_fft_batch(double2 *data, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
   extern __shared__ double2 fbuf[];
   double2 *d = data + (long long)blockIdx.x * n;
   for (int k = threadIdx.x; k < n; k += blockDim.x) fbuf[k] = d[k];
@@ -107,7 +147,7 @@ __global__ void __launch_bounds__(1024) k_fft_batch(double2 *data, int n, int si
   for (int k = threadIdx.x; k < n; k += blockDim.x) d[k] = fbuf[k];
 }
 
-static int fft_threads(int n) { return n / 4 < 32 ? 32 : n / 4; }
+static int fft_threads(int n) { return n / 16 < 32 ? 32 : n / 16; }
 
 int qhp_fft_launch(double *data, int n, int64_t batch, int sign, const double *tw, int tw_n, cudaStream_t st) {
   const size_t smem = sizeof(double2) * (size_t)n;
@@ -178,7 +218,7 @@ __global__ void k_qtb_spectrum4(int nt, int n_seg, const double *__restrict__ hk
 // kernel h is real, so real and imaginary parts are filtered independently), z through a second.
 //   F_c[dof][n] = sum_k h_z[k] r(dof, seg*n_seg + n - k + n_seg),  n = 0..n_seg-1
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) k_qtb_noise(int n_seg, long long ND, unsigned long long seed, long long seg, const int32_t *__restrict__ type,
+__global__ void __launch_bounds__(256, 2) k_qtb_noise(int n_seg, long long ND, unsigned long long seed, long long seg, const int32_t *__restrict__ type,
                             const double2 *__restrict__ H4, const double2 *__restrict__ tw, double *Fc) {
   extern __shared__ double2 nbuf[];
   const int nf = 4 * n_seg, nw = 3 * n_seg;
@@ -196,20 +236,24 @@ __global__ void __launch_bounds__(1024) k_qtb_noise(int n_seg, long long ND, uns
     }
   }
   const double inv = 1.0 / (double)nf;
-  double fx = 0.0, fy = 0.0;              // blockDim.x >= n_seg: thread t owns output sample n = t
+  double fx[4] = {0.0, 0.0, 0.0, 0.0}, fy[4] = {0.0, 0.0, 0.0, 0.0};   // 4 blockDim.x >= n_seg: samples n = t + u blockDim.x
   for (int pass = 0; pass < 2; ++pass) {
     __syncthreads();
     fft_smem(nbuf, nf, -1, tw, nf);
     for (int q = t; q < nf; q += blockDim.x) nbuf[q] = cmul(nbuf[q], Hz[q]);
     __syncthreads();
     fft_smem(nbuf, nf, +1, tw, nf);
-    if (t < n_seg) {
-      const double2 y = nbuf[t + 2 * n_seg];
-      if (pass == 0) { fx = y.x * inv; fy = y.y * inv; }
-      else {
-        // Fc[n][dof] (step-contiguous for the integrator): the three components of one sample together
-        double *out = Fc + (long long)t * ND + 3LL * atom;
-        out[0] = fx; out[1] = fy; out[2] = y.x * inv;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int n = t + u * blockDim.x;
+      if (n < n_seg) {
+        const double2 y = nbuf[n + 2 * n_seg];
+        if (pass == 0) { fx[u] = y.x * inv; fy[u] = y.y * inv; }
+        else {
+          // Fc[n][dof] (step-contiguous for the integrator): the three components of one sample together
+          double *out = Fc + (long long)n * ND + 3LL * atom;
+          out[0] = fx[u]; out[1] = fy[u]; out[2] = y.x * inv;
+        }
       }
     }
     if (pass == 0) {
@@ -223,7 +267,7 @@ __global__ void __launch_bounds__(1024) k_qtb_noise(int n_seg, long long ND, uns
 // Q5 + Q6: spectra.  One CTA walks a run of atoms of one type; v and F_c of a DOF are the real and
 // imaginary part of one zero-padded N_k-point transform.  Per-CTA sums -> fixed-order reduction.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) k_qtb_spectra(int n_seg, long long ND, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
+__global__ void __launch_bounds__(256, 2) k_qtb_spectra(int n_seg, long long ND, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
                               const double *__restrict__ vseg, const double *__restrict__ Fc,
                               const double2 *__restrict__ tw, int tw_n, double *part) {
   extern __shared__ double2 sbuf[];
