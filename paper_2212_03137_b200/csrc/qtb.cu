@@ -43,9 +43,9 @@ __device__ __forceinline__ void dft4(double2 &a, double2 &b, double2 &c, double2
 // version of the noise kernel), or 4 radix-4 / 8 radix-2 butterflies.  Reads are contiguous in t.
 // Input twiddles w^(k u) are successive powers of one table entry w^k (<= 15 products, ~1e-14 relative).
 template <int R, int SG>
-__device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const double2 *__restrict__ tw, int tw_n) {
+__device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const double2 *__restrict__ tw, int tw_n, int t) {
   constexpr int G = 16 / R;                       // butterflies per thread
-  const int nth = n >= 16 ? n >> 4 : 1, nb = n / R, t = threadIdx.x;
+  const int nth = n >= 16 ? n >> 4 : 1, nb = n / R;
   const bool on = t < nth;
   double2 v[16];
   int j0[G];
@@ -119,15 +119,17 @@ __device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const doub
 // In-place Stockham FFT of buf[0..n) by blockDim.x >= max(n/16, 1) threads (all threads of the CTA
 // must call).  sign = -1 forward, +1 inverse (unnormalised).  Result in natural order.
 template <int SG>
-__device__ __forceinline__ void fft_smem_sg(double2 *buf, int n, const double2 *__restrict__ tw, int tw_n) {
+__device__ __forceinline__ void fft_smem_sg(double2 *buf, int n, const double2 *__restrict__ tw, int tw_n, int t) {
   int Ns = 1;
-  while (n / Ns >= 16 && ((n / Ns) & 15) == 0) { fft_pass<16, SG>(buf, n, Ns, tw, tw_n); Ns <<= 4; }
-  while (((n / Ns) & 3) == 0 && Ns < n) { fft_pass<4, SG>(buf, n, Ns, tw, tw_n); Ns <<= 2; }
-  while (Ns < n) { fft_pass<2, SG>(buf, n, Ns, tw, tw_n); Ns <<= 1; }
+  while (n / Ns >= 16 && ((n / Ns) & 15) == 0) { fft_pass<16, SG>(buf, n, Ns, tw, tw_n, t); Ns <<= 4; }
+  while (((n / Ns) & 3) == 0 && Ns < n) { fft_pass<4, SG>(buf, n, Ns, tw, tw_n, t); Ns <<= 2; }
+  while (Ns < n) { fft_pass<2, SG>(buf, n, Ns, tw, tw_n, t); Ns <<= 1; }
 }
-__device__ __noinline__ void fft_smem(double2 *buf, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
-  if (sign < 0) fft_smem_sg<-1>(buf, n, tw, tw_n);
-  else fft_smem_sg<1>(buf, n, tw, tw_n);
+// t: index of the calling thread inside its FFT (threads t >= max(n/16, 1) only take part in the barriers);
+// several FFTs of the same length can run side by side in one CTA on different buffers.
+__device__ __noinline__ void fft_smem(double2 *buf, int n, int sign, const double2 *__restrict__ tw, int tw_n, int t) {
+  if (sign < 0) fft_smem_sg<-1>(buf, n, tw, tw_n, t);
+  else fft_smem_sg<1>(buf, n, tw, tw_n, t);
 }
 
 __global__ void k_twiddle(double2 *tw, int n) {
@@ -143,7 +145,7 @@ __global__ void __launch_bounds__(512) k_fft_batch(double2 *data, int n, int sig
   double2 *d = data + (long long)blockIdx.x * n;
   for (int k = threadIdx.x; k < n; k += blockDim.x) fbuf[k] = d[k];
   __syncthreads();
-  fft_smem(fbuf, n, sign, tw, tw_n);
+  fft_smem(fbuf, n, sign, tw, tw_n, threadIdx.x);
   for (int k = threadIdx.x; k < n; k += blockDim.x) d[k] = fbuf[k];
 }
 
@@ -239,10 +241,10 @@ __global__ void __launch_bounds__(256, 2) k_qtb_noise(int n_seg, long long ND, u
   double fx[4] = {0.0, 0.0, 0.0, 0.0}, fy[4] = {0.0, 0.0, 0.0, 0.0};   // 4 blockDim.x >= n_seg: samples n = t + u blockDim.x
   for (int pass = 0; pass < 2; ++pass) {
     __syncthreads();
-    fft_smem(nbuf, nf, -1, tw, nf);
+    fft_smem(nbuf, nf, -1, tw, nf, t);
     for (int q = t; q < nf; q += blockDim.x) nbuf[q] = cmul(nbuf[q], Hz[q]);
     __syncthreads();
-    fft_smem(nbuf, nf, +1, tw, nf);
+    fft_smem(nbuf, nf, +1, tw, nf, t);
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const int n = t + u * blockDim.x;
@@ -267,41 +269,54 @@ __global__ void __launch_bounds__(256, 2) k_qtb_noise(int n_seg, long long ND, u
 // Q5 + Q6: spectra.  One CTA walks a run of atoms of one type; v and F_c of a DOF are the real and
 // imaginary part of one zero-padded N_k-point transform.  Per-CTA sums -> fixed-order reduction.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256, 2) k_qtb_spectra(int n_seg, long long ND, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
+// One CTA = 3 groups of max(n_k/16, 32) threads; group c transforms DOF c of the current atom (v and
+// F_c as real and imaginary part of one zero-padded n_k-point FFT).  Every thread accumulates its own
+// frequency bins in registers over all atoms of the CTA's run; the three groups are combined once at
+// the end in a fixed order.  SPEC_BINS bounds (n_seg + 1) / group size (n_seg <= 1024: 1025 / 128).
+#define SPEC_BINS 9
+__global__ void __launch_bounds__(384, 2) k_qtb_spectra(int n_seg, long long ND, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
                               const double *__restrict__ vseg, const double *__restrict__ Fc,
                               const double2 *__restrict__ tw, int tw_n, double *part) {
-  extern __shared__ double2 sbuf[];
-  const int nk = 2 * n_seg, nf = n_seg + 1, t = threadIdx.x;
-  double *avv = reinterpret_cast<double *>(sbuf + nk), *avf = avv + nf;
-  for (int j = t; j < nf; j += blockDim.x) { avv[j] = 0.0; avf[j] = 0.0; }
-  const int b = cta_tab[3 * blockIdx.x + 1], e = cta_tab[3 * blockIdx.x + 2];
-  double2 *raw = reinterpret_cast<double2 *>(avf + nf);        // [3][n_seg] (v, F_c) of the atom's three DOFs
-  for (int ia = b; ia < e; ++ia) {
-    const int atom = atoms[ia];
-    __syncthreads();
-    for (int n = t; n < n_seg; n += blockDim.x) {               // one 24-byte piece per sample and array
-      const double *pv = vseg + (long long)n * ND + 3LL * atom, *pf = Fc + (long long)n * ND + 3LL * atom;
+  extern __shared__ double2 sbuf_all[];
+  const int nk = 2 * n_seg, nf = n_seg + 1, gsz = blockDim.x / 3;
+  const int c = threadIdx.x / gsz, t = threadIdx.x - c * gsz;
+  double2 *sbuf = sbuf_all + (size_t)c * nk;
+  double avv[SPEC_BINS], avf[SPEC_BINS];
 #pragma unroll
-      for (int c = 0; c < 3; ++c) raw[c * n_seg + n] = make_double2(pv[c], pf[c]);
-    }
-    for (int c = 0; c < 3; ++c) {
-      __syncthreads();
-      for (int n = t; n < nk; n += blockDim.x)
-        sbuf[n] = (n < n_seg) ? raw[c * n_seg + n] : make_double2(0.0, 0.0);
-      __syncthreads();
-      fft_smem(sbuf, nk, -1, tw, tw_n);
-      for (int j = t; j < nf; j += blockDim.x) {
+  for (int m = 0; m < SPEC_BINS; ++m) { avv[m] = 0.0; avf[m] = 0.0; }
+  const int b = cta_tab[3 * blockIdx.x + 1], e = cta_tab[3 * blockIdx.x + 2];
+  for (int ia = b; ia < e; ++ia) {
+    const long long d = 3LL * atoms[ia] + c;
+    for (int n = t; n < nk; n += gsz)
+      sbuf[n] = (n < n_seg) ? make_double2(vseg[(long long)n * ND + d], Fc[(long long)n * ND + d]) : make_double2(0.0, 0.0);
+    __syncthreads();
+    fft_smem(sbuf, nk, -1, tw, tw_n, t);
+#pragma unroll
+    for (int m = 0; m < SPEC_BINS; ++m) {
+      const int j = t + m * gsz;
+      if (j < nf) {
         const double2 A = sbuf[j], Zm = sbuf[(nk - j) & (nk - 1)];
         const double vx = 0.5 * (A.x + Zm.x), vy = 0.5 * (A.y - Zm.y);     // V_j
         const double px = 0.5 * (A.y + Zm.y), py = -0.5 * (A.x - Zm.x);    // Phi_j
-        avv[j] += vx * vx + vy * vy;
-        avf[j] += vx * px + vy * py;
+        avv[m] += vx * vx + vy * vy;
+        avf[m] += vx * px + vy * py;
       }
     }
+    __syncthreads();
+  }
+  // combine the three groups: (x + y) + z per bin
+  double *red = reinterpret_cast<double *>(sbuf_all);          // [3][2][nf]
+#pragma unroll
+  for (int m = 0; m < SPEC_BINS; ++m) {
+    const int j = t + m * gsz;
+    if (j < nf) { red[(c * 2) * nf + j] = avv[m]; red[(c * 2 + 1) * nf + j] = avf[m]; }
   }
   __syncthreads();
   double *o = part + (long long)blockIdx.x * 2 * nf;
-  for (int j = t; j < nf; j += blockDim.x) { o[j] = avv[j]; o[nf + j] = avf[j]; }
+  for (int j = threadIdx.x; j < nf; j += blockDim.x) {
+    o[j] = (red[j] + red[2 * nf + j]) + red[4 * nf + j];
+    o[nf + j] = (red[nf + j] + red[3 * nf + j]) + red[5 * nf + j];
+  }
 }
 
 __global__ void k_qtb_reduce(int nt, int n_seg, int n_cta, const int32_t *__restrict__ cta_tab, const double *__restrict__ part,
@@ -483,10 +498,10 @@ int qhp_qtb_generate(qhp_system *s, int64_t seg) {
 // Q5-Q7 at the end of a segment
 int qhp_qtb_adapt(qhp_system *s) {
   const int ns = s->n_seg, nf = ns + 1, nt = s->nt, nk = 2 * ns;
-  const size_t smem = sizeof(double2) * nk + sizeof(double) * 2 * (nf + 1) + sizeof(double2) * 3 * ns;
+  const size_t smem = sizeof(double2) * 3 * nk;
   QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_spectra, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_qtb_spectra<<<s->n_spec_cta, fft_threads(nk), smem, s->stream>>>(ns, 3LL * s->N, s->spec_cta, s->atoms_by_type, s->vseg, s->Fc,
-                                                                     (const double2 *)s->tw, 4 * ns, s->spec_part);
+  k_qtb_spectra<<<s->n_spec_cta, 3 * fft_threads(nk), smem, s->stream>>>(ns, 3LL * s->N, s->spec_cta, s->atoms_by_type, s->vseg, s->Fc,
+                                                                        (const double2 *)s->tw, 4 * ns, s->spec_part);
   QHP_LAUNCH_OK(s);
   k_qtb_reduce<<<(nt * nf + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->n_spec_cta, s->spec_cta, s->spec_part,
                                                            s->spec_part + (size_t)s->n_spec_cta * 2 * nf, s->dt, s->Cvv, s->CvF);
