@@ -47,8 +47,8 @@ FLOP_PER_PAIR_BEAD = 110.0
 # bench.py also measures it live with qhp_dfma_probe and reports both.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_staged<false> launch at C4, from the
-# `ncu --set full` capture summarised in profiles/r1b_summary.md (per launch, like `achieved`)
-NCU_TRAFFIC_BYTES = {("C4", "k_pair_staged"): 1.3636e9 + 2.33e7}
+# `ncu --set full` capture summarised in profiles/r1c_summary.md (per launch, like `achieved`)
+NCU_TRAFFIC_BYTES = {("C4", "k_pair_staged"): 1.3636e9 + 2.36e7}
 
 
 def measure_dfma_peak() -> float:
