@@ -204,3 +204,32 @@ def test_staged_pair_kernel_mid_size():
     xr, _ = ref.get_state()
     assert np.abs(x1.cpu().numpy() - xr).max() < XTOL
     sysg.check()
+
+
+def test_orthorhombic_box_staged_kernel():
+    """Non-cubic box (6 x 5 x 4 cells, different cell edges per dimension): cell indexing, the staged
+    neighbourhood and the per-cell image shifts must not rely on a cubic box."""
+    import oracle as O
+    top = W.water_box(5832)
+    scale = np.array([1.2, 1.0, 1.0 / 1.2])
+    pos = top["positions"].reshape(-1, 3, 3)
+    centre = pos[:, :1, :]
+    top["positions"] = np.ascontiguousarray((centre * scale + (pos - centre)).reshape(-1, 3))
+    top["box"] = top["box"] * scale
+    sysg, ref, x0, p0 = make_pair(top, 2, 2, 0.25, "pile", sigma_bead=0.03)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    assert sysg.counters()["staged"] == 1
+    ref.set_state(x0, p0, 0)
+    otop, cent = _lists_check(sysg, top, x0)
+    assert tuple(sysg.neighbor_lists()[0].cpu().numpy()) == (6, 5, 4)
+    count, i, j = _pairs_from_gpu(sysg)
+    for a in (0, 5, 9000, top["n_atoms"] - 1):
+        assert np.array_equal(np.sort(j[i == a]), np.sort(O.neighbours_of(otop, cent, a)))
+    G = sysg.forces().cpu().numpy()
+    Gref = ref.forces()
+    assert np.abs(G - Gref).max() < FTOL * np.abs(Gref).max()
+    sysg.step(10)
+    ref.step(10)
+    x1, _, _ = sysg.get_state()
+    assert np.abs(x1.cpu().numpy() - ref.get_state()[0]).max() < XTOL
+    sysg.check()
