@@ -72,12 +72,15 @@ __device__ __forceinline__ double poly17(const double *c, double u) {
 // row sits at (pos / 256) * 256 + (pos % 32) * 8 + (pos % 256) / 32, i.e. one 16-byte load per lane
 // brings entries pos = 256 m + 32 j + lane, j = 0..7; rows are padded with index 0 up to a multiple
 // of 256 entries.
-template <bool ENERGY>
+// F32: with the float4 copy for the fp32 pre-test (40 B per staged atom).  !F32: neighbourhoods too
+// large for that stage fp64 positions + an int type only (28 B per atom) and pre-test in fp64.
+template <bool ENERGY, bool F32>
 __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double *sp = reinterpret_cast<double *>(smem_raw);                  // [cap][3] fp64, cell-centred
-  float4 *sf = reinterpret_cast<float4 *>(sp + 3 * (size_t)a.cap);    // [cap] fp32 copy + type bits
-  double *tab = reinterpret_cast<double *>(sf + a.cap);
+  float4 *sf = reinterpret_cast<float4 *>(sp + 3 * (size_t)a.cap);    // F32: [cap] fp32 copy + type bits
+  int *st = reinterpret_cast<int *>(sp + 3 * (size_t)a.cap);          // !F32: [cap] types
+  double *tab = F32 ? reinterpret_cast<double *>(sf + a.cap) : reinterpret_cast<double *>(st + a.cap);
   uint32_t *queue = reinterpret_cast<uint32_t *>(tab + QHP_MAX_TYPES * QHP_MAX_TYPES * 4);
   __shared__ int off[28], cbeg[27], next_atom;
   __shared__ double su[STG_MAX_WARPS];
@@ -120,7 +123,8 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
     ly = fma(-a.box[1], rint(ly * a.inv_box[1]), ly);
     lz = fma(-a.box[2], rint(lz * a.inv_box[2]), lz);
     sp[3 * g] = lx; sp[3 * g + 1] = ly; sp[3 * g + 2] = lz;
-    sf[g] = make_float4((float)lx, (float)ly, (float)lz, __int_as_float((int)__double_as_longlong(p.w)));
+    if (F32) sf[g] = make_float4((float)lx, (float)ly, (float)lz, __int_as_float((int)__double_as_longlong(p.w)));
+    else st[g] = (int)__double_as_longlong(p.w);
   }
   __syncthreads();
 
@@ -154,9 +158,9 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   while (ii < nh) {
     const int ei = h0 + ii;
     const long long slot = slot0 + ii;
-    const float4 fi = sf[ei];
+    const float4 fi = F32 ? sf[ei] : make_float4(0.f, 0.f, 0.f, 0.f);
     const double xi = sp[3 * ei], yi = sp[3 * ei + 1], zi = sp[3 * ei + 2];
-    const double *tab_i = tab + __float_as_int(fi.w) * a.nt * 4;
+    const double *tab_i = tab + (F32 ? __float_as_int(fi.w) : st[ei]) * a.nt * 4;
     double Fx = 0.0, Fy = 0.0, Fz = 0.0;
     int qn = 0;
 
@@ -198,12 +202,22 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       for (int j = 0; j < 8; ++j) {
         if (32 * j >= n - STG_BLOCK * m) break;            // warp-uniform: the row ends before this step
         const uint32_t e = (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
-        const float4 pj = sf[e];
-        const float dxf = fi.x - pj.x, dyf = fi.y - pj.y, dzf = fi.z - pj.z;
-        const float r2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
-        const bool hit = (32 * j < left) && r2f < a.rc2f;
+        bool hit;
+        uint32_t tj;
+        if (F32) {
+          const float4 pj = sf[e];
+          const float dxf = fi.x - pj.x, dyf = fi.y - pj.y, dzf = fi.z - pj.z;
+          const float r2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
+          hit = (32 * j < left) && r2f < a.rc2f;
+          tj = (uint32_t)__float_as_int(pj.w);
+        } else {
+          const double *pj = sp + 3 * e;
+          const double dx = xi - pj[0], dy = yi - pj[1], dz = zi - pj[2];
+          hit = (32 * j < left) && fma(dz, dz, fma(dy, dy, dx * dx)) < a.rc2;
+          tj = (uint32_t)st[e];
+        }
         const unsigned mask = __ballot_sync(0xffffffffu, hit);
-        if (hit) ql[qn + __popc(mask & lt) - lane] = e | ((uint32_t)__float_as_int(pj.w) << 16);
+        if (hit) ql[qn + __popc(mask & lt) - lane] = e | (tj << 16);
         qn += __popc(mask);
       }
       __syncwarp();
@@ -306,8 +320,9 @@ static long double fit_poly(int which, long double wmax, long double scale, doub
   return worst;
 }
 
-static size_t staged_smem_bytes(int cap, int warps) {
-  return (size_t)cap * (3 * sizeof(double) + sizeof(float4)) + sizeof(double) * QHP_MAX_TYPES * QHP_MAX_TYPES * 4 +
+static size_t staged_atom_bytes(bool f32) { return 3 * sizeof(double) + (f32 ? sizeof(float4) : sizeof(int)); }
+static size_t staged_smem_bytes(int cap, int warps, bool f32) {
+  return (size_t)cap * staged_atom_bytes(f32) + 16 + sizeof(double) * QHP_MAX_TYPES * QHP_MAX_TYPES * 4 +
          sizeof(uint32_t) * (size_t)warps * STG_QUEUE;
 }
 
@@ -325,8 +340,10 @@ int qhp_pair_setup(qhp_system *s) {
   QHP_CUDA_OK(s, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device));
   s->staged_smem_max = max_smem - 1024;                                // room for the static shared variables
   if (s->staged_smem_max < 64 * 1024) return QHP_OK;
-  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->staged_smem_max));
-  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->staged_smem_max));
+  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->staged_smem_max));
+  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->staged_smem_max));
+  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->staged_smem_max));
+  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_staged<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->staged_smem_max));
   // CTAs per (cell, bead): aim at >= 6 waves of one CTA per SM, keep >= one atom per warp
   int sms = 148;
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device);
@@ -346,16 +363,19 @@ int qhp_pair_staged_partials(const qhp_system *s) { return s->ncell * 8 * s->Pc;
 // Largest CTA (in warps) whose queues leave room for `region` staged atoms (+ 1/16 for drift between
 // list builds); sets staged_warps / staged_cap.  False: the neighbourhood does not fit at all.
 bool qhp_pair_staged_fit(qhp_system *s, long long region) {
-  static const int tries[] = {STG_MAX_WARPS, 24, 16, 12, 8};
+  static const int tries[] = {STG_MAX_WARPS, 24, 16};
   const long long need = region + region / 16 + 32;
-  for (int w : tries) {
-    if (w > STG_MAX_WARPS) continue;
-    const long long room = (long long)s->staged_smem_max - (long long)staged_smem_bytes(0, w);
-    long long cap = room / (long long)(3 * sizeof(double) + sizeof(float4));
-    if (cap > 65534) cap = 65534;                                      // 16-bit list entries
-    cap &= ~1LL;
-    if (cap >= need) { s->staged_warps = w; s->staged_cap = (int)cap; return true; }
-  }
+  // first choice: the fp32 pre-test copy with the largest CTA; then the same CTA sizes without the copy
+  for (int f32 = 1; f32 >= 0; --f32)
+    for (int w : tries) {
+      if (w > STG_MAX_WARPS) continue;
+      const long long room = (long long)s->staged_smem_max - (long long)staged_smem_bytes(0, w, f32 != 0);
+      long long cap = room / (long long)staged_atom_bytes(f32 != 0);
+      if (cap > 65534) cap = 65534;                                    // 16-bit list entries
+      cap &= ~3LL;                                                     // keeps the arrays behind the positions aligned
+      if (cap >= need) { s->staged_warps = w; s->staged_cap = (int)cap; s->staged_f32 = f32 != 0; return true; }
+      if (f32 && w == STG_MAX_WARPS) break;                            // a smaller CTA is worse than dropping the copy
+    }
   return false;
 }
 
@@ -383,10 +403,15 @@ int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned lo
   for (int k = 0; k < QHP_NPOLY; ++k) { a.cS[k] = s->polyS[k]; a.cE[k] = s->polyE[k]; }
   a.part = part; a.count = count; a.counters = (long long *)s->counters;
   const dim3 grid((unsigned)(s->ncell * s->staged_split), (unsigned)s->Pc);
-  const size_t smem = staged_smem_bytes(s->staged_cap, s->staged_warps);
+  const size_t smem = staged_smem_bytes(s->staged_cap, s->staged_warps, s->staged_f32);
   const int threads = 32 * s->staged_warps;
-  if (energy) k_pair_staged<true><<<grid, threads, smem, s->stream>>>(a);
-  else k_pair_staged<false><<<grid, threads, smem, s->stream>>>(a);
+  if (s->staged_f32) {
+    if (energy) k_pair_staged<true, true><<<grid, threads, smem, s->stream>>>(a);
+    else k_pair_staged<false, true><<<grid, threads, smem, s->stream>>>(a);
+  } else {
+    if (energy) k_pair_staged<true, false><<<grid, threads, smem, s->stream>>>(a);
+    else k_pair_staged<false, false><<<grid, threads, smem, s->stream>>>(a);
+  }
   QHP_LAUNCH_OK(s);
   return QHP_OK;
 }

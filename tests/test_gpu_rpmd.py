@@ -110,6 +110,7 @@ def test_c2_lists_forces_steps():
     top = W.water_box(4096)
     sysg, ref, x0, p0 = make_pair(top, 32, 4, 0.25, "pile")
     sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    assert sysg.counters()["staged"] == 1      # 5184-atom neighbourhoods: the staged kernel without its fp32 copy
     ref.set_state(x0, p0, 0)
     otop, cent = _lists_check(sysg, top, x0)
     count, i, j = _pairs_from_gpu(sysg)
