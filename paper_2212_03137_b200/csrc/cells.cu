@@ -188,46 +188,63 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
   const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
   const unsigned lt = (1u << lane) - 1u;
   int cnt = 0, off = 0;
-  for (int ox = 0; ox < 3; ++ox)
-    for (int oy = 0; oy < 3; ++oy)
+  // The 27 stencil cells are walked as 9 (x, y) columns.  The three cells of a column are adjacent in z,
+  // hence contiguous in slot order unless the column wraps around the box: they are scanned as one run
+  // (fewer ragged 32-candidate chunks, one set of per-run constants).  A cell whose box is out of reach
+  // of this centroid is dropped from its run (the margin of rl2_hi covers the fp32 rounding).  The
+  // image of a neighbour cell next to the home cell is known per cell: with >= 4 cells per dimension it
+  // is the minimum image of every pair within r_list, so the fp32 pre-test needs no rint.
+  const float gzl = fmaxf(fi.z - cz * a.edgef[2], 0.f), gzh = fmaxf((cz + 1) * a.edgef[2] - fi.z, 0.f);
+  for (int ox = 0; ox < 3; ++ox) {
+    const int ux = cx - 1 + ox, qx = ux < 0 ? ux + a.nc[0] : (ux >= a.nc[0] ? ux - a.nc[0] : ux);
+    const float px = fi.x - (ux < 0 ? -a.boxf[0] : (ux >= a.nc[0] ? a.boxf[0] : 0.f));
+    const float hx = ox == 0 ? fmaxf(fi.x - cx * a.edgef[0], 0.f) : (ox == 2 ? fmaxf((cx + 1) * a.edgef[0] - fi.x, 0.f) : 0.f);
+    for (int oy = 0; oy < 3; ++oy) {
+      const int uy = cy - 1 + oy, qy = uy < 0 ? uy + a.nc[1] : (uy >= a.nc[1] ? uy - a.nc[1] : uy);
+      const float py = fi.y - (uy < 0 ? -a.boxf[1] : (uy >= a.nc[1] ? a.boxf[1] : 0.f));
+      const float hy = oy == 0 ? fmaxf(fi.y - cy * a.edgef[1], 0.f) : (oy == 2 ? fmaxf((cy + 1) * a.edgef[1] - fi.y, 0.f) : 0.f);
+      const float gxy = fmaf(hy, hy, hx * hx);
+      const int cb = (qx * a.nc[1] + qy) * a.nc[2];
+      int bq[3], eq[3];
+      float sz[3];
+      bool reach[3];
+#pragma unroll
       for (int oz = 0; oz < 3; ++oz) {
-        const int qx = (cx - 1 + ox + a.nc[0]) % a.nc[0], qy = (cy - 1 + oy + a.nc[1]) % a.nc[1],
-                  qz = (cz - 1 + oz + a.nc[2]) % a.nc[2];
-        const int c2 = (qx * a.nc[1] + qy) * a.nc[2] + qz;
-        const int b = cell_start[c2], e = cell_start[c2 + 1];
-        // distance from this centroid to the neighbour cell's box (wrapped coordinates): a cell out of
-        // reach is skipped as a whole (the margin of rl2_hi covers the fp32 rounding of both)
-        const float gx = ox == 0 ? fi.x - cx * a.edgef[0] : (ox == 2 ? (cx + 1) * a.edgef[0] - fi.x : 0.f);
-        const float gy = oy == 0 ? fi.y - cy * a.edgef[1] : (oy == 2 ? (cy + 1) * a.edgef[1] - fi.y : 0.f);
-        const float gz = oz == 0 ? fi.z - cz * a.edgef[2] : (oz == 2 ? (cz + 1) * a.edgef[2] - fi.z : 0.f);
-        const float hx = fmaxf(gx, 0.f), hy = fmaxf(gy, 0.f), hz = fmaxf(gz, 0.f);
-        if (fmaf(hz, hz, fmaf(hy, hy, hx * hx)) < a.rl2_hi) {
-          // the image of the neighbour cell next to the home cell is known per cell: with >= 4 cells per
-          // dimension it is the minimum image of every pair within r_list, so the pre-test needs no rint
-          const float sx = cx - 1 + ox < 0 ? -a.boxf[0] : (cx - 1 + ox >= a.nc[0] ? a.boxf[0] : 0.f);
-          const float sy = cy - 1 + oy < 0 ? -a.boxf[1] : (cy - 1 + oy >= a.nc[1] ? a.boxf[1] : 0.f);
-          const float sz = cz - 1 + oz < 0 ? -a.boxf[2] : (cz - 1 + oz >= a.nc[2] ? a.boxf[2] : 0.f);
-          const float px = fi.x - sx, py = fi.y - sy, pz = fi.z - sz;
-          for (int k0 = b; k0 < e; k0 += 32) {
-            const int k = k0 + lane;
-            bool hit = false;
-            if (k < e && k != i) {
-              const float4 fj = centf[k];
-              const float dxf = px - fj.x, dyf = py - fj.y, dzf = pz - fj.z;
-              const float d2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
-              if (__float_as_int(fj.w) != __float_as_int(fi.w) && d2f < a.rl2_hi)
-                hit = d2f < a.rl2_lo || list_hit_exact(a, cent4, ci, k);
-            }
-            const unsigned mask = __ballot_sync(0xffffffffu, hit);
-            if (hit && nbr) {
-              const int pos = cnt + __popc(mask & lt);
-              if (pos < stride) nbr[i * stride + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)(off + k - b);
-            }
-            cnt += __popc(mask);
-          }
-        }
-        off += e - b;
+        const int uz = cz - 1 + oz, qz = uz < 0 ? uz + a.nc[2] : (uz >= a.nc[2] ? uz - a.nc[2] : uz);
+        bq[oz] = cell_start[cb + qz]; eq[oz] = cell_start[cb + qz + 1];
+        sz[oz] = uz < 0 ? -a.boxf[2] : (uz >= a.nc[2] ? a.boxf[2] : 0.f);
+        const float hz = oz == 0 ? gzl : (oz == 2 ? gzh : 0.f);
+        reach[oz] = fmaf(hz, hz, gxy) < a.rl2_hi;
       }
+      int oz = 0;
+      while (oz < 3) {
+        if (!reach[oz]) { off += eq[oz] - bq[oz]; ++oz; continue; }
+        const int b = bq[oz], run_off = off;
+        const float pz = fi.z - sz[oz];
+        int e = eq[oz], oz2 = oz + 1;
+        off += eq[oz] - bq[oz];
+        while (oz2 < 3 && reach[oz2] && bq[oz2] == e && sz[oz2] == sz[oz]) { e = eq[oz2]; off += eq[oz2] - bq[oz2]; ++oz2; }
+        for (int k0 = b; k0 < e; k0 += 32) {
+          const int k = k0 + lane;
+          bool hit = false;
+          if (k < e && k != i) {
+            const float4 fj = centf[k];
+            const float dxf = px - fj.x, dyf = py - fj.y, dzf = pz - fj.z;
+            const float d2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
+            if (__float_as_int(fj.w) != __float_as_int(fi.w) && d2f < a.rl2_hi)
+              hit = d2f < a.rl2_lo || list_hit_exact(a, cent4, ci, k);
+          }
+          const unsigned mask = __ballot_sync(0xffffffffu, hit);
+          if (hit && nbr) {
+            const int pos = cnt + __popc(mask & lt);
+            if (pos < stride) nbr[i * stride + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)(run_off + k - b);
+          }
+          cnt += __popc(mask);
+        }
+        oz = oz2;
+      }
+    }
+  }
   if (nbr) {
     // pad the last 256-entry block with index 0 (a valid staged index; the kernel masks these lanes)
     const int n = (int)min((long long)cnt, stride), end = (int)min((long long)((n + 255) & ~255), stride);
