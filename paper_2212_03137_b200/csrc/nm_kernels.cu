@@ -107,17 +107,38 @@ __device__ __forceinline__ double bonded_molecule(const IntArgs &a, int m, int a
 // warp-uniform, so the coefficients come through the constant bank / uniform registers) and the
 // mode sum runs in four independent partial sums; a fully unrolled P x P body overflowed the
 // instruction cache at P = 32.
+// The transfer matrix (O1) is a real DFT: columns n = 0, odd n (cos) and, for even P, n = P - 1 are
+// symmetric under i -> P - i, columns of even n >= 2 (sin) antisymmetric and zero at i = 0, P/2.
+// Beads i and P - i therefore share one cos sum A and one sin sum B (x_i = A + B, x_{P-i} = A - B),
+// which halves the multiply-adds of the dense P x P transforms.
+#define QHP_SIN_MODE(n) ((n) >= 2 && ((n) & 1) == 0)
 template <int P>
 __device__ __forceinline__ void modes_to_beads_tile(const NmTab<P> &tab, const double (&Qr)[P], double *xt, double *ft,
                                                     int TD, int t) {
   const double sp = sqrt((double)P);
-#pragma unroll 1
-  for (int i = 0; i < P; ++i) {
-    double s[4] = {0.0, 0.0, 0.0, 0.0};
+  constexpr int NP = (P - 1) / 2;                 // pairs (i, P - i), i = 1 .. NP
+  {                                               // i = 0 and, for even P, i = P/2: cos-type columns only
+    double s0 = 0.0, s1 = 0.0, h0 = 0.0, h1 = 0.0;
 #pragma unroll
-    for (int n = 0; n < P; ++n) s[n & 3] = fma(tab.T[i * P + n], Qr[n], s[n & 3]);
-    xt[i * TD + t] = sp * ((s[0] + s[1]) + (s[2] + s[3]));
-    ft[i * TD + t] = 0.0;
+    for (int n = 0; n < P; ++n)
+      if (!QHP_SIN_MODE(n)) {
+        if (n & 2) { s1 = fma(tab.T[n], Qr[n], s1); if (P % 2 == 0) h1 = fma(tab.T[(P / 2) * P + n], Qr[n], h1); }
+        else { s0 = fma(tab.T[n], Qr[n], s0); if (P % 2 == 0) h0 = fma(tab.T[(P / 2) * P + n], Qr[n], h0); }
+      }
+    xt[t] = sp * (s0 + s1); ft[t] = 0.0;
+    if (P % 2 == 0 && P > 1) { xt[(P / 2) * TD + t] = sp * (h0 + h1); ft[(P / 2) * TD + t] = 0.0; }
+  }
+#pragma unroll 1
+  for (int i = 1; i <= NP; ++i) {
+    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
+#pragma unroll
+    for (int n = 0; n < P; ++n) {
+      if (QHP_SIN_MODE(n)) { if (n & 2) b1 = fma(tab.T[i * P + n], Qr[n], b1); else b0 = fma(tab.T[i * P + n], Qr[n], b0); }
+      else { if (n & 2) a1 = fma(tab.T[i * P + n], Qr[n], a1); else a0 = fma(tab.T[i * P + n], Qr[n], a0); }
+    }
+    const double A = a0 + a1, B = b0 + b1;
+    xt[i * TD + t] = sp * (A + B); ft[i * TD + t] = 0.0;
+    xt[(P - i) * TD + t] = sp * (A - B); ft[(P - i) * TD + t] = 0.0;
   }
 }
 
@@ -128,13 +149,21 @@ template <int P>
 __device__ __forceinline__ void project_forces_tile(const IntArgs &a, const NmTab<P> &tab, const NmTab<P> &ctab,
                                                     const double *ft, int TD, int t, int atom, int c, double (&fr)[P],
                                                     double wf = 1.0, double ws = 1.0) {
+  constexpr int NP = (P - 1) / 2;
+  {
+    const double F0 = ft[t], Fh = (P % 2 == 0 && P > 1) ? ft[(P / 2) * TD + t] : 0.0;
 #pragma unroll
-  for (int n = 0; n < P; ++n) fr[n] = 0.0;
+    for (int n = 0; n < P; ++n) {
+      if (QHP_SIN_MODE(n)) fr[n] = 0.0;
+      else fr[n] = (P % 2 == 0 && P > 1) ? fma(tab.T[(P / 2) * P + n], Fh, tab.T[n] * F0) : tab.T[n] * F0;
+    }
+  }
 #pragma unroll 1
-  for (int i = 0; i < P; ++i) {
-    const double Fi = ft[i * TD + t];
+  for (int i = 1; i <= NP; ++i) {
+    const double Fi = ft[i * TD + t], Fm = ft[(P - i) * TD + t];
+    const double S = Fi + Fm, D = Fi - Fm;
 #pragma unroll
-    for (int n = 0; n < P; ++n) fr[n] = fma(tab.T[i * P + n], Fi, fr[n]);
+    for (int n = 0; n < P; ++n) fr[n] = fma(tab.T[i * P + n], QHP_SIN_MODE(n) ? D : S, fr[n]);
   }
   const double isp = wf / sqrt((double)P);
 #pragma unroll
