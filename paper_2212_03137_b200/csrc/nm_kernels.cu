@@ -12,10 +12,17 @@
 // two shared-memory tiles [P][TD] so that the bonded terms can be evaluated per (molecule, bead).
 // The P x P transform matrix is a kernel parameter, i.e. lives in the constant bank: with the
 // loops fully unrolled every FMA takes its coefficient as an immediate constant operand.
+#include <algorithm>
+
 #include "qhp_internal.cuh"
 #include "philox.cuh"
 
 template <int P> struct NmTab { double T[P * P]; };   // T[i*P+n], Eq. 2 eigenvectors
+// Mass-independent coefficients of the A and O blocks per mode (kernel-parameter bank: they reach the
+// FP64 instructions as constant operands, no loads): cs = cos(w dt/2), sw = sin(w dt/2)/w,
+// ws = w sin(w dt/2), c1 = exp(-gamma_n dt), c2k = sqrt(kB T 418.4 (1 - c1^2)).  With the mass m of the
+// DOF: s1 = sw/m, s2 = -m ws, noise amplitude = sqrt(m) c2k.
+template <int P> struct ModeCoef { double cs[P], sw[P], ws[P], c1[P], c2k[P]; };
 
 struct IntArgs {
   int N, Pc, nt, TD;
@@ -250,7 +257,8 @@ __device__ __forceinline__ double block_sum(double v, double *scratch) {
 // ---------------------------------------------------------------------------------------------
 // CTA size and residency: 48-atom tiles (160 threads, three CTAs per SM) for P >= 24, else 96-atom tiles
 template <int P, int THERMO, int PCM>   // PCM: compile-time bound on the contracted beads P'
-__global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integrate(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab) {
+__global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integrate(const IntArgs a, const NmTab<P> tab, const NmTab<P> ctab,
+                                                                                   const ModeCoef<P> mc) {
   extern __shared__ double sm[];
   const int TD = a.TD, t = threadIdx.x;
   double *xt = sm, *ft = sm + P * TD, *scratch = ft + P * TD;
@@ -312,8 +320,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
   // ---- phase 4: B A O A per mode, contraction of the new positions -----------------------------------------
   double d2 = 0.0;
   if (active) {
-    const double m = a.mass[ty];
-    const double *cf = a.coef + ty * P * QHP_NCOEF;   // read-only, L1-resident (two types x P x 6 doubles)
+    const double m = a.mass[ty], minv = 1.0 / m, sqm = sqrt(m);
     double xc[PCM];                     // contracted beads (first Pc entries used)
 #pragma unroll
     for (int j = 0; j < PCM; ++j) xc[j] = 0.0;
@@ -330,13 +337,13 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
       double p = pl[n % PF];
       p += fr[n];                       // B: pending half kick of the last step + first half kick of this one
       if (a.do_step) {
-        const double cs = __ldg(cf + n * QHP_NCOEF + 0), s1 = __ldg(cf + n * QHP_NCOEF + 1), s2 = __ldg(cf + n * QHP_NCOEF + 2);
+        const double cs = mc.cs[n], s1 = mc.sw[n] * minv, s2 = -(mc.ws[n] * m);
         // A(dt/2): centroid translation / exact free ring-polymer rotation
-        if (n == 0) q += a.hdt * p / m;
+        if (n == 0) q += a.hdt * p * minv;
         else { const double qn = cs * q + s1 * p; p = s2 * q + cs * p; q = qn; }
         // O(dt)
         if (THERMO == 1) {
-          p = __ldg(cf + n * QHP_NCOEF + 3) * p + __ldg(cf + n * QHP_NCOEF + 4) * ft[n * TD + t];
+          p = mc.c1[n] * p + (mc.c2k[n] * sqm) * ft[n * TD + t];
         } else if (THERMO == 2) {
           // classical BAOAB carrying the coloured force (Eq. 12, l.199; readings G14, G16)
           const long long k = (long long)a.n_loc * a.ND + dof;   // [n_seg][3N]: step-contiguous
@@ -345,7 +352,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
           p = pn;
         }
         // A(dt/2)
-        if (n == 0) q += a.hdt * p / m;
+        if (n == 0) q += a.hdt * p * minv;
         else { const double qn = cs * q + s1 * p; p = s2 * q + cs * p; q = qn; }
         a.Q[n * a.ND + dof] = q;
         // contraction of the new positions (Eq. 20): only the first Pc modes contribute
@@ -656,6 +663,21 @@ template <int P> static NmTab<P> make_tab(const std::vector<double> &T, int n) {
   return t;
 }
 
+template <int P> static ModeCoef<P> make_mode_coef(const qhp_system *s) {
+  ModeCoef<P> mc;
+  const double kTA = QHP_KB * s->T * QHP_ACC;
+  for (int n = 0; n < P; ++n) {
+    const double w = n < (int)s->omega.size() ? s->omega[n] : 0.0, h = 0.5 * s->dt;
+    mc.cs[n] = cos(w * h);
+    mc.sw[n] = n ? sin(w * h) / w : 0.0;
+    mc.ws[n] = n ? w * sin(w * h) : 0.0;
+    const double g = (n == 0) ? s->th.gamma0 : std::max(s->th.gamma0, w);
+    mc.c1[n] = exp(-g * s->dt);
+    mc.c2k[n] = sqrt(kTA * (1.0 - mc.c1[n] * mc.c1[n]));
+  }
+  return mc;
+}
+
 static IntArgs make_args(qhp_system *s) {
   IntArgs a{};
   a.N = s->N; a.Pc = s->Pc; a.nt = s->nt; a.TD = 3 * s->tile_atoms; a.ND = 3LL * s->N;
@@ -721,7 +743,8 @@ int qhp_nm_integrate(qhp_system *s, bool kick_prev, bool do_step, int64_t step) 
 #define LAUNCH_INT(PP, TH, PCM)                                                                  \
   {                                                                                              \
     QHP_CUDA_OK(s, set_smem(k_integrate<PP, TH, PCM>, smem));                                    \
-    k_integrate<PP, TH, PCM><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, make_tab<PP>(s->T_P, PP), make_tab<PP>(s->T_Pc, s->Pc)); \
+    k_integrate<PP, TH, PCM><<<s->n_tiles, s->tile_threads, smem, s->stream>>>(a, make_tab<PP>(s->T_P, PP), make_tab<PP>(s->T_Pc, s->Pc), \
+                                                                               make_mode_coef<PP>(s));                              \
   }
 #define FN(PP)                                                                                   \
   {                                                                                              \
