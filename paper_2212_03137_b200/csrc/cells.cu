@@ -14,6 +14,8 @@
 // one warp per slot scanning the 27-cell stencil with ballot compaction (deterministic order).
 // Every kernel of the rebuild chain returns at once unless the integrator's list-validity statistic
 // max |xc - cref|^2 reached (skin/2)^2, so the chain can be enqueued every step without a host sync.
+#include <cooperative_groups.h>
+
 #include "qhp_internal.cuh"
 
 struct CellArgs {
@@ -336,7 +338,78 @@ static CellArgs cell_args(qhp_system *s, bool force) {
 }
 
 // cells (assign, scan, fill, rank) of the current centroids Q_0
+// The four cell kernels as one cooperative kernel (grid-wide barriers between the phases): inside
+// qhp_step the chain is enqueued every step and returns at once unless a rebuild is due, so one launch
+// instead of four takes 3 kernel boundaries off every step (they dominate the small boxes).
+__global__ void __launch_bounds__(256) k_cells_fused(const CellArgs a, const double *__restrict__ Q0, int32_t *cell_of,
+                                                     int32_t *cell_count, int32_t *cell_start, int32_t *cursor,
+                                                     int32_t *tmp, int32_t *order, int32_t *rank) {
+  if (cells_skip(a)) return;                       // uniform over the grid: nobody reaches a barrier
+  namespace cg = cooperative_groups;
+  cg::grid_group grid = cg::this_grid();
+  const int nthreads = gridDim.x * blockDim.x, t0 = blockIdx.x * blockDim.x + threadIdx.x;
+  for (int i = t0; i < a.N; i += nthreads) {       // assign
+    int q[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      double sc = __dmul_rn(Q0[3LL * i + d], a.inv_box[d]);
+      sc = __dsub_rn(sc, floor(sc));
+      int v = (int)__dmul_rn(sc, (double)a.nc[d]);
+      if (v > a.nc[d] - 1) v = a.nc[d] - 1;
+      q[d] = v;
+    }
+    const int cell = (q[0] * a.nc[1] + q[1]) * a.nc[2] + q[2];
+    cell_of[i] = cell;
+    atomicAdd(&cell_count[cell], 1);
+  }
+  grid.sync();
+  if (blockIdx.x == 0) {                           // exclusive scan of the cell counts by one CTA
+    __shared__ int32_t part[256];
+    const int t = threadIdx.x, nt = blockDim.x, n = a.ncell;
+    const int len = (n + nt - 1) / nt;
+    const int b = min(n, t * len), e = min(n, b + len);
+    int32_t sum = 0;
+    for (int k = b; k < e; ++k) sum += cell_count[k];
+    part[t] = sum;
+    __syncthreads();
+    for (int o = 1; o < nt; o <<= 1) {
+      const int32_t v = (t >= o) ? part[t - o] : 0;
+      __syncthreads();
+      part[t] += v;
+      __syncthreads();
+    }
+    int32_t run = part[t] - sum;
+    for (int k = b; k < e; ++k) {
+      const int32_t v = cell_count[k];
+      cell_start[k] = run; cursor[k] = run; cell_count[k] = 0;
+      run += v;
+    }
+    if (t == nt - 1) { cell_start[n] = part[t]; cursor[n] = part[t]; }
+  }
+  grid.sync();
+  for (int i = t0; i < a.N; i += nthreads) tmp[atomicAdd(&cursor[cell_of[i]], 1)] = i;   // fill
+  grid.sync();
+  for (int i = t0; i < a.N; i += nthreads) {       // stable order inside each cell
+    const int c = cell_of[i], b = cell_start[c], e = cell_start[c + 1];
+    int cnt = 0;
+    for (int k = b; k < e; ++k) cnt += (tmp[k] < i);
+    order[b + cnt] = i;
+    rank[i] = b + cnt;
+  }
+}
+
 static int cells_only(qhp_system *s, const CellArgs &a) {
+  if (s->coop_blocks > 0) {
+    const int tb = 256;
+    int grid = (s->N + tb - 1) / tb;
+    if (grid > s->coop_blocks) grid = s->coop_blocks;
+    CellArgs ac = a;
+    const double *q0 = s->Q;
+    void *args[] = {&ac, &q0, &s->cell_of, &s->cell_count, &s->cell_start, &s->cell_cursor, &s->cell_tmp, &s->order, &s->rank};
+    QHP_CUDA_OK(s, cudaLaunchCooperativeKernel((const void *)k_cells_fused, dim3(grid), dim3(tb), args, 0, s->stream));
+    s->n_launch++;
+    return QHP_OK;
+  }
   const int tb = 256, grid = (s->N + tb - 1) / tb;
   k_cells_assign<<<grid, tb, 0, s->stream>>>(a, s->Q, s->cell_of, s->cell_count);
   QHP_LAUNCH_OK(s);
@@ -443,3 +516,16 @@ int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, i
   if (cnt_own) cudaFree(cnt_own);
   return QHP_OK;
 }
+
+// cooperative launches need all CTAs resident: how many k_cells_fused CTAs fit on the device (0: unsupported)
+int qhp_cells_setup(qhp_system *s) {
+  int coop = 0, per_sm = 0, sms = 0;
+  QHP_CUDA_OK(s, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, s->device));
+  QHP_CUDA_OK(s, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device));
+  s->coop_blocks = 0;
+  if (!coop) return QHP_OK;
+  QHP_CUDA_OK(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cells_fused, 256, 0));
+  s->coop_blocks = per_sm * sms;
+  return QHP_OK;
+}
+

@@ -258,7 +258,9 @@ extern "C" int qhp_create(const qhp_topology *top, int P, int P_contract, double
   CREATE_CUDA(cudaMemset(s->counters, 0, sizeof(int64_t) * 8));
   CREATE_CUDA(cudaMalloc(&s->obs, sizeof(double) * 8));
   {
-    const int rc = qhp_pair_setup(s);
+    int rc = qhp_cells_setup(s);
+    if (rc) CREATE_FAIL(rc, s->err);
+    rc = qhp_pair_setup(s);
     if (rc) CREATE_FAIL(rc, s->err);
     s->red_len = 4 * (size_t)s->n_tiles + (size_t)qhp_pair_partials(s) + 16;
     CREATE_CUDA(cudaMalloc(&s->red, sizeof(double) * s->red_len));
