@@ -269,8 +269,9 @@ class Rpmd:
     """State in normal modes; `step(n)` = n x B A O A B (Eq. 16-17)."""
 
     def __init__(self, top: Topology, P: int, Pc: int, dt_ps: float, T_K: float, thermo: str,
-                 gamma0: float, seed: int, cells: bool | None = None):
+                 gamma0: float, seed: int, cells: bool | None = None, a_block: str = "exact"):
         self.top, self.P, self.Pc, self.dt, self.T = top, P, Pc, dt_ps, T_K
+        self.a_block = {"exact": 0, "cayley": 1}[a_block]       # "cayley": BCOCB (PAPER.md:151)
         self.thermo = {"none": 0, "pile": 1}[thermo]
         self.gamma0, self.seed = gamma0, seed
         self.uc = top.use_cells if cells is None else int(cells)
@@ -283,10 +284,11 @@ class Rpmd:
         self.step_index = step0
 
     def step(self, n: int):
-        lib().qo_rpmd_steps(self.top.ref, C.c_int(self.P), C.c_int(self.Pc), C.c_double(self.dt),
-                            C.c_double(self.T), C.c_int(self.thermo), C.c_double(self.gamma0),
-                            C.c_uint64(self.seed), C.c_int64(self.step_index), C.c_int64(n),
-                            _p(self.Q), _p(self.Pm), _p(self.f), C.c_int(self.uc))
+        fn = lib().qo_rpmd_steps_bcocb if self.a_block else lib().qo_rpmd_steps
+        fn(self.top.ref, C.c_int(self.P), C.c_int(self.Pc), C.c_double(self.dt),
+           C.c_double(self.T), C.c_int(self.thermo), C.c_double(self.gamma0),
+           C.c_uint64(self.seed), C.c_int64(self.step_index), C.c_int64(n),
+           _p(self.Q), _p(self.Pm), _p(self.f), C.c_int(self.uc))
         self.step_index += n
 
     def get_state(self):

@@ -439,8 +439,14 @@ void qo_observables(const qo_topology *t, int P, int Pc, double T_K, const doubl
  * harmonic <q^2> closed form (statistical).
  * ------------------------------------------------------------------------------------------ */
 /* A(dt/2) O(dt) A(dt/2) of one step (O5 items 2-4), shared by qo_rpmd_steps and qo_rpmd_respa_steps */
+/* a_block = 0: exact harmonic A(dt/2) (Eq. 17).  a_block = 1: the BCOCB variant ("the exact
+ * integration of e^{iL_A dt/2} is replaced by a numerical scheme", ref. [66] of the paper): the half-step
+ * is the square root of the Cayley transform cay(dt A) = (1 - dt A/2)^-1 (1 + dt A/2) of the free
+ * ring-polymer generator A = [[0, 1/m], [-m w^2, 0]] of each mode, whose closed form is
+ *   cay(dt A)^(1/2) = (1 + (w dt/2)^2)^(-1/2) [[1, dt/(2m)], [-m w^2 dt/2, 1]]        (reading G25)
+ * (a rotation by atan(w dt/2) instead of w dt/2; the centroid, w = 0, is the same translation). */
 static void qo_aoa(const qo_topology *t, int P, double dt, double T_K, int thermo, double gamma0,
-                   uint64_t seed, int64_t step, const double *om, double *Q, double *Pm) {
+                   uint64_t seed, int64_t step, const double *om, double *Q, double *Pm, int a_block) {
   int N = t->n_atoms;
   int64_t nd = 3 * (int64_t)N;
   for (int half = 0; half < 2; ++half) {
@@ -450,6 +456,12 @@ static void qo_aoa(const qo_topology *t, int P, double dt, double T_K, int therm
       for (int c = 0; c < 3; ++c) {
         int64_t k = n * nd + 3 * a + c;
         if (n == 0) { Q[k] += 0.5 * dt * Pm[k] / m; }
+        else if (a_block == 1) {
+          double w = om[n], a = 0.5 * w * dt, nrm = 1.0 / sqrt(1.0 + a * a);
+          double q = Q[k], p = Pm[k];
+          Q[k]  = nrm * (q + 0.5 * dt / m * p);
+          Pm[k] = nrm * (-m * w * w * 0.5 * dt * q + p);
+        }
         else {
           double w = om[n], cs = cos(w * 0.5 * dt), sn = sin(w * 0.5 * dt);
           double q = Q[k], p = Pm[k];
@@ -476,22 +488,38 @@ static void qo_aoa(const qo_topology *t, int P, double dt, double T_K, int therm
   }
 }
 
-void qo_rpmd_steps(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
-                   double gamma0, uint64_t seed, int64_t step0, int64_t nsteps,
-                   double *Q, double *Pm, double *f, int use_cells) {
+static void qo_rpmd_steps_ab(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
+                             double gamma0, uint64_t seed, int64_t step0, int64_t nsteps,
+                             double *Q, double *Pm, double *f, int use_cells, int a_block) {
   int64_t nd = 3 * (int64_t)t->n_atoms;
   double *om = (double *)malloc(sizeof(double) * P);
   qo_nm_freq(P, T_K, om);
   for (int64_t s = 0; s < nsteps; ++s) {
     /* 1. B(dt/2) */
     for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * f[k];
-    qo_aoa(t, P, dt, T_K, thermo, gamma0, seed, step0 + s, om, Q, Pm);
+    qo_aoa(t, P, dt, T_K, thermo, gamma0, seed, step0 + s, om, Q, Pm, a_block);
     /* 5.-7. forces at the new positions */
     qo_nm_forces(t, P, Pc, Q, f, NULL, use_cells);
     /* 8. B(dt/2) */
     for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * f[k];
   }
   free(om);
+}
+
+void qo_rpmd_steps(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
+                   double gamma0, uint64_t seed, int64_t step0, int64_t nsteps,
+                   double *Q, double *Pm, double *f, int use_cells) {
+  qo_rpmd_steps_ab(t, P, Pc, dt, T_K, thermo, gamma0, seed, step0, nsteps, Q, Pm, f, use_cells, 0);
+}
+
+/* NEXT-3  BCOCB: B(dt/2) C(dt/2) O(dt) C(dt/2) B(dt/2), C = cay(dt A)^(1/2) (see qo_aoa).
+ * Pins (tests/test_oracle_bcocb.py): C^2 equals the Cayley matrix from a linear solve and C equals
+ * scipy's matrix square root of it; det C = 1; the mode's harmonic energy is conserved exactly; C agrees
+ * with the exact rotation to O((w dt)^3); time reversal; second order; w dt -> large stays bounded. */
+void qo_rpmd_steps_bcocb(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
+                         double gamma0, uint64_t seed, int64_t step0, int64_t nsteps,
+                         double *Q, double *Pm, double *f, int use_cells) {
+  qo_rpmd_steps_ab(t, P, Pc, dt, T_K, thermo, gamma0, seed, step0, nsteps, Q, Pm, f, use_cells, 1);
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -539,7 +567,7 @@ void qo_rpmd_respa_steps(const qo_topology *t, int P, int Pc, double dt, double 
     for (int j = 0; j < n_alt; ++j) {
       /* Bf(dt/2) A O A Bf(dt/2) */
       for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * ff[k];
-      qo_aoa(t, P, dt, T_K, thermo, gamma0, seed, step0 + o * n_alt + j, om, Q, Pm);
+      qo_aoa(t, P, dt, T_K, thermo, gamma0, seed, step0 + o * n_alt + j, om, Q, Pm, 0);
       qo_nm_forces_split(t, P, Pc, Q, ff, NULL, use_cells);
       for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * ff[k];
     }
