@@ -221,6 +221,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--workload", default="C4", choices=sorted(W.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--a-block", choices=["exact", "cayley"], default="exact", help="cayley = BCOCB (PAPER.md:151); exact = the BASELINE.json configs")
     ap.add_argument("--n-alt", type=int, default=1, help="BAOAB-RESPA inner steps per V_s evaluation (PAPER.md Eq. 19); 1 = the BASELINE.json configs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -249,6 +250,8 @@ def main():
     N, P, K = top["n_atoms"], cfg["P"], args.steps
     xd = torch.as_tensor(x0).cuda()
     pd = torch.as_tensor(p0).cuda()
+    if args.a_block != "exact":
+        sysg.set_a_block(args.a_block)
     if args.n_alt > 1:
         sysg.set_respa(args.n_alt)
         args.warmup = -(-args.warmup // args.n_alt) * args.n_alt
@@ -355,7 +358,7 @@ def main():
                 warmup=args.warmup, ms_per_step=ms / K, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f64", data="synthetic",
                 config=dict(workload=cfg["name"], n_atoms=N, P=P, P_contract=cfg["P_contract"], dt_fs=cfg["dt_fs"],
-                            thermostat=cfg["thermostat"], n_alt=args.n_alt, ns_per_day=ns_day, parallelism="replicas only" if world > 1 else "1 GPU",
+                            thermostat=cfg["thermostat"], n_alt=args.n_alt, a_block=args.a_block, ns_per_day=ns_day, parallelism="replicas only" if world > 1 else "1 GPU",
                             l2="inputs larger than L2 (state + neighbour table >> 126 MB)" if N > 100000 else "inputs smaller than L2",
                             pair_beads_in_cutoff=pair_beads, list_entries=c1["list_entries"]),
                 clocks=clk.summary(), e2e=e2e, gpu_launches=int(launches),

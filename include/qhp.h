@@ -112,6 +112,15 @@ int qhp_step(qhp_system *sys, int64_t nsteps);
  * n_alt = 1 (default) is plain B A O A B.  Call it at a multiple of n_alt steps; not with adQTB. */
 int qhp_set_respa(qhp_system *sys, int n_alt);
 
+/* A block of the splitting: QHP_ABLOCK_EXACT (default) = exact harmonic evolution of the
+ * fluctuation modes over dt/2 (Eq. 17); QHP_ABLOCK_CAYLEY = the BCOCB variant, whose half-step is the
+ * square root of the Cayley transform of the free ring-polymer generator,
+ *   (q, p) -> (1 + (w dt/2)^2)^(-1/2) (q + dt/(2m) p, p - m w^2 dt/2 q)      (reading G25),
+ * stable for any w dt.  The centroid and P = 1 are unchanged.  May be called at any step. */
+#define QHP_ABLOCK_EXACT 0
+#define QHP_ABLOCK_CAYLEY 1
+int qhp_set_a_block(qhp_system *sys, int kind);
+
 /* Bead-space forces at the current positions, device [P][n_atoms][3]:
  * G_i = -grad V_f(x_i) + (P/P') sum_j C_ji (-grad V_s(xc_j))  (Eq. 10-11 and chain rule on Eq. 20). */
 int qhp_forces(qhp_system *sys, double *f_beads);

@@ -314,8 +314,8 @@ class RpmdRespa(Rpmd):
     """BAOAB-RESPA (Eq. 19): `step(n)` advances n INNER steps of dt, n a multiple of
     n_alt; V_s (on the Pc contracted beads) kicks with n_alt*dt/2 around every n_alt inner steps."""
 
-    def __init__(self, top, P, Pc, dt_ps, T_K, thermo, gamma0, seed, n_alt: int, cells=None):
-        super().__init__(top, P, Pc, dt_ps, T_K, thermo, gamma0, seed, cells)
+    def __init__(self, top, P, Pc, dt_ps, T_K, thermo, gamma0, seed, n_alt: int, cells=None, a_block="exact"):
+        super().__init__(top, P, Pc, dt_ps, T_K, thermo, gamma0, seed, cells, a_block)
         self.n_alt = int(n_alt)
 
     def set_state(self, x_beads, p_beads, step0: int = 0):
@@ -330,11 +330,12 @@ class RpmdRespa(Rpmd):
 
     def step(self, n: int):
         assert n % self.n_alt == 0
-        lib().qo_rpmd_respa_steps(self.top.ref, C.c_int(self.P), C.c_int(self.Pc), C.c_double(self.dt),
-                                  C.c_double(self.T), C.c_int(self.thermo), C.c_double(self.gamma0),
-                                  C.c_uint64(self.seed), C.c_int64(self.step_index), C.c_int64(n // self.n_alt),
-                                  C.c_int(self.n_alt), _p(self.Q), _p(self.Pm), _p(self.ff), _p(self.fs),
-                                  C.c_int(self.uc))
+        fn = lib().qo_rpmd_respa_steps_bcocb if self.a_block else lib().qo_rpmd_respa_steps
+        fn(self.top.ref, C.c_int(self.P), C.c_int(self.Pc), C.c_double(self.dt),
+           C.c_double(self.T), C.c_int(self.thermo), C.c_double(self.gamma0),
+           C.c_uint64(self.seed), C.c_int64(self.step_index), C.c_int64(n // self.n_alt),
+           C.c_int(self.n_alt), _p(self.Q), _p(self.Pm), _p(self.ff), _p(self.fs),
+           C.c_int(self.uc))
         self.step_index += n
 
 

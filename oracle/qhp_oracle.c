@@ -555,9 +555,9 @@ void qo_nm_forces_split(const qo_topology *t, int P, int Pc, const double *Q, do
   free(x); free(Ff); free(xc); free(Fc);
 }
 
-void qo_rpmd_respa_steps(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
-                         double gamma0, uint64_t seed, int64_t step0, int64_t n_outer, int n_alt,
-                         double *Q, double *Pm, double *ff, double *fs, int use_cells) {
+static void qo_rpmd_respa_steps_ab(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
+                                   double gamma0, uint64_t seed, int64_t step0, int64_t n_outer, int n_alt,
+                                   double *Q, double *Pm, double *ff, double *fs, int use_cells, int a_block) {
   int64_t nd = 3 * (int64_t)t->n_atoms;
   double *om = (double *)malloc(sizeof(double) * P);
   qo_nm_freq(P, T_K, om);
@@ -567,7 +567,7 @@ void qo_rpmd_respa_steps(const qo_topology *t, int P, int Pc, double dt, double 
     for (int j = 0; j < n_alt; ++j) {
       /* Bf(dt/2) A O A Bf(dt/2) */
       for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * ff[k];
-      qo_aoa(t, P, dt, T_K, thermo, gamma0, seed, step0 + o * n_alt + j, om, Q, Pm, 0);
+      qo_aoa(t, P, dt, T_K, thermo, gamma0, seed, step0 + o * n_alt + j, om, Q, Pm, a_block);
       qo_nm_forces_split(t, P, Pc, Q, ff, NULL, use_cells);
       for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * dt * QO_ACC * ff[k];
     }
@@ -576,6 +576,20 @@ void qo_rpmd_respa_steps(const qo_topology *t, int P, int Pc, double dt, double 
     for (int64_t k = 0; k < P * nd; ++k) Pm[k] += 0.5 * n_alt * dt * QO_ACC * fs[k];
   }
   free(om);
+}
+
+void qo_rpmd_respa_steps(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
+                         double gamma0, uint64_t seed, int64_t step0, int64_t n_outer, int n_alt,
+                         double *Q, double *Pm, double *ff, double *fs, int use_cells) {
+  qo_rpmd_respa_steps_ab(t, P, Pc, dt, T_K, thermo, gamma0, seed, step0, n_outer, n_alt, Q, Pm, ff, fs, use_cells, 0);
+}
+
+/* RESPA with the BCOCB half-steps in the inner loop: Bs [Bf C O C Bf]^{n_alt} Bs (same pins as both parents:
+ * n_alt = 1 reproduces qo_rpmd_steps_bcocb, tests/test_oracle_bcocb.py) */
+void qo_rpmd_respa_steps_bcocb(const qo_topology *t, int P, int Pc, double dt, double T_K, int thermo,
+                               double gamma0, uint64_t seed, int64_t step0, int64_t n_outer, int n_alt,
+                               double *Q, double *Pm, double *ff, double *fs, int use_cells) {
+  qo_rpmd_respa_steps_ab(t, P, Pc, dt, T_K, thermo, gamma0, seed, step0, n_outer, n_alt, Q, Pm, ff, fs, use_cells, 1);
 }
 
 /* ------------------------------------------------------------------------------------------

@@ -668,9 +668,16 @@ template <int P> static ModeCoef<P> make_mode_coef(const qhp_system *s) {
   const double kTA = QHP_KB * s->T * QHP_ACC;
   for (int n = 0; n < P; ++n) {
     const double w = n < (int)s->omega.size() ? s->omega[n] : 0.0, h = 0.5 * s->dt;
-    mc.cs[n] = cos(w * h);
-    mc.sw[n] = n ? sin(w * h) / w : 0.0;
-    mc.ws[n] = n ? w * sin(w * h) : 0.0;
+    if (s->a_block == QHP_ABLOCK_CAYLEY) {           // BCOCB: rotation by atan(w h) instead of w h (G25)
+      const double nrm = 1.0 / sqrt(1.0 + (w * h) * (w * h));
+      mc.cs[n] = nrm;
+      mc.sw[n] = n ? nrm * h : 0.0;
+      mc.ws[n] = n ? nrm * w * w * h : 0.0;
+    } else {
+      mc.cs[n] = cos(w * h);
+      mc.sw[n] = n ? sin(w * h) / w : 0.0;
+      mc.ws[n] = n ? w * sin(w * h) : 0.0;
+    }
     const double g = (n == 0) ? s->th.gamma0 : std::max(s->th.gamma0, w);
     mc.c1[n] = exp(-g * s->dt);
     mc.c2k[n] = sqrt(kTA * (1.0 - mc.c1[n] * mc.c1[n]));

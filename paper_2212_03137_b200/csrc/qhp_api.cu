@@ -459,6 +459,13 @@ extern "C" int qhp_set_respa(qhp_system *s, int n_alt) {
   return QHP_OK;
 }
 
+extern "C" int qhp_set_a_block(qhp_system *s, int kind) {
+  if (!s) return QHP_EINVAL;
+  if (kind != QHP_ABLOCK_EXACT && kind != QHP_ABLOCK_CAYLEY) { s->err = "unknown A block"; return QHP_EINVAL; }
+  s->a_block = kind;
+  return QHP_OK;
+}
+
 extern "C" int qhp_forces(qhp_system *s, double *f_beads) {
   if (!s || !f_beads) return QHP_EINVAL;
   if (!s->have_state) { s->err = "no state"; return QHP_ESTATE; }

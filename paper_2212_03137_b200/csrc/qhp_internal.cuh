@@ -50,6 +50,7 @@ struct qhp_system {
   // ---- configuration (host) ----
   int N = 0, nt = 0, n_mol = 0, n_bonds = 0, n_angles = 0;
   int P = 1, Pc = 1;
+  int a_block = 0;                         // 0: exact A(dt/2); 1: BCOCB half-step sqrt(cay(dt A))
   int n_alt = 1;                           // BAOAB-RESPA: inner steps per V_s kick (Eq. 19); 1 = plain BAOAB
   double dt = 0, T = 0;
   qhp_thermostat th{};

@@ -127,3 +127,17 @@ def test_P1_is_unchanged_and_water_is_reversible_and_second_order():
         e.step(n); c.step(n)
         errs.append(np.abs(e.Q - c.Q).max())
     assert errs[0] > 1e-9 and 3.5 < errs[0] / errs[1] < 4.5
+
+
+def test_respa_with_n_alt_1_is_bcocb():
+    top = W.water_box(27)
+    top["box"] = np.array([20.0] * 3)
+    ot = O.Topology(top)
+    x0, p0 = W.initial_state(top, 4, T_K, sigma_bead=0.03)
+    a = O.Rpmd(ot, 4, 2, 0.25e-3, T_K, "pile", 1.0, 7, a_block="cayley")
+    b = O.RpmdRespa(ot, 4, 2, 0.25e-3, T_K, "pile", 1.0, 7, n_alt=1, a_block="cayley")
+    e = O.RpmdRespa(ot, 4, 2, 0.25e-3, T_K, "pile", 1.0, 7, n_alt=1)
+    for s in (a, b, e):
+        s.set_state(x0, p0, 3); s.step(12)
+    assert np.abs(a.Q - b.Q).max() < 1e-13 and np.abs(a.Pm - b.Pm).max() < 1e-11 * np.abs(a.Pm).max()
+    assert np.abs(a.Q - e.Q).max() > 1e-9                  # and it is not the exact-A stepper
