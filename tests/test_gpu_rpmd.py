@@ -234,3 +234,37 @@ def test_orthorhombic_box_staged_kernel():
     x1, _, _ = sysg.get_state()
     assert np.abs(x1.cpu().numpy() - ref.get_state()[0]).max() < XTOL
     sysg.check()
+
+
+@pytest.mark.parametrize("P,Pc", [(2, 1), (2, 2), (3, 3), (5, 3), (6, 3), (6, 6), (12, 5), (16, 16), (24, 12), (32, 1), (32, 32)])
+def test_every_supported_bead_count(P, Pc):
+    """All P the integrator is instantiated for, with odd / even / full / centroid-only contraction:
+    forces at the start and positions after 10 steps (216 waters, one cell)."""
+    import oracle as O
+    top = W.water_box(216)
+    sysg, ref, x0, p0 = make_pair(top, P, Pc, 0.25, "pile", sigma_bead=0.03)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    G = sysg.forces().cpu().numpy()
+    Gref = O.bead_forces(O.Topology(top), P, Pc, x0)
+    assert np.abs(G - Gref).max() < FTOL * np.abs(Gref).max()
+    sysg.step(10); ref.step(10)
+    assert np.abs(sysg.get_state()[0].cpu().numpy() - ref.get_state()[0]).max() < XTOL
+    sysg.check()
+
+
+def test_unsupported_arguments_are_rejected():
+    import paper_2212_03137_b200 as qhp
+    top = W.water_box(216)
+    for P, Pc in [(7, 7), (8, 9), (8, 0), (0, 0)]:
+        with pytest.raises(qhp.QhpError):
+            qhp.System(top, P, Pc, 0.25e-3, T_K, "pile", gamma0=1.0, seed=1)
+    with pytest.raises(qhp.QhpError):
+        qhp.System(top, 8, 8, -1.0, T_K, "pile", gamma0=1.0, seed=1)
+    sysg = qhp.System(top, 4, 2, 0.25e-3, T_K, "pile", gamma0=1.0, seed=1)
+    with pytest.raises(qhp.QhpError):
+        sysg.step(1)                                   # no state yet
+    x0, p0 = W.initial_state(top, 4, T_K)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    sysg.step(0)                                       # zero steps is a no-op
+    assert sysg.get_state()[2] == 0

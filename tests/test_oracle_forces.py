@@ -173,3 +173,30 @@ def test_bond_angle_equilibrium_and_values():
     x[2] = x[0] + b2
     u, _ = O.force_fast(t, x)
     assert abs(u - 0.5 * 75.90 * th ** 2) < 1e-10
+
+
+def test_ragged_molecules_four_types_finite_difference_and_cells():
+    """workloads.water.ionic_water_box: molecules of 1, 2 and 3 atoms, four types (ions with LJ + charge):
+    forces are minus the gradient of the energy, sum to zero, and the cell walk equals the double loop."""
+    top = W.ionic_water_box(729)
+    t = O.Topology(top)
+    sizes = np.bincount(top["mol"])
+    assert set(sizes) == {1, 2, 3}
+    rng = np.random.default_rng(6)
+    x = top["positions"] + 0.05 * rng.standard_normal(top["positions"].shape)
+    ub, Fb = O.force_slow(t, x, cells=False)
+    uc, Fc = O.force_slow(t, x, cells=True)
+    assert abs(ub - uc) < 1e-10 * abs(ub) and np.abs(Fb - Fc).max() < 1e-11 * np.abs(Fb).max()
+    _, F = O.force_total(t, x, cells=False)
+    assert np.abs(F.sum(0)).max() < 1e-9
+    first = np.concatenate([[0], np.cumsum(sizes)[:-1]])
+    picks = [first[sizes == 1][0], first[sizes == 1][1], first[sizes == 2][0], first[sizes == 2][0] + 1, first[sizes == 3][5] + 2]
+    h = 1e-4
+    for a, c in zip(picks, (0, 1, 2, 0, 1)):
+        xp, xm = x.copy(), x.copy()
+        xp[a, c] += h
+        xm[a, c] -= h
+        up, _ = O.force_total(t, xp, cells=False)
+        um, _ = O.force_total(t, xm, cells=False)
+        fd = -(up - um) / (2 * h)
+        assert abs(fd - F[a, c]) < 1e-6 * max(1.0, abs(F[a, c])), (a, c, fd, F[a, c])

@@ -122,6 +122,49 @@ def water_box(n_mol: int, seed: int = MASTER_SEED) -> dict:
     )
 
 
+def ionic_water_box(n_sites: int, ion_every: int = 7, seed: int = MASTER_SEED) -> dict:
+    """A water box in which every `ion_every`-th lattice site holds, in turn, a monatomic cation (one-atom
+    molecule), a monatomic anion, or a charged diatomic (two atoms, one bond, no angle) instead of a water:
+    molecules of 1, 2 and 3 atoms mixed in atom order, four atom types, net charge zero for n_sites a
+    multiple of 3 * ion_every.  Not a workload of the paper: the ragged-molecule parity case (tiles, bonded
+    ranges, exclusions and the per-type tables must not assume O,H,H triples)."""
+    w = water_box(n_sites, seed)
+    ff = WATER_FF
+    pos_w = w["positions"].reshape(n_sites, 3, 3)
+    typ, mol, pos, bonds, bk, br, angles, ak, at = [], [], [], [], [], [], [], [], []
+    kind = 0
+    for m in range(n_sites):
+        a0 = len(typ)
+        if m % ion_every == ion_every - 1:
+            k = kind % 3
+            kind += 1
+            if k == 0:                                  # cation, type 2
+                typ += [2]; pos += [pos_w[m, 0]]
+            elif k == 1:                                # anion, type 3
+                typ += [3]; pos += [pos_w[m, 0]]
+            else:                                       # diatomic O-H (types 0, 1), one bond; carries -0.42
+                typ += [0, 1]; pos += [pos_w[m, 0], pos_w[m, 1]]
+                bonds += [[a0, a0 + 1]]; bk += [ff["bond_k"]]; br += [ff["bond_r0"]]
+        else:
+            typ += [0, 1, 1]; pos += list(pos_w[m])
+            bonds += [[a0, a0 + 1], [a0, a0 + 2]]; bk += [ff["bond_k"]] * 2; br += [ff["bond_r0"]] * 2
+            angles += [[a0 + 1, a0, a0 + 2]]; ak += [ff["angle_k"]]; at += [np.deg2rad(ff["angle_th0_deg"])]
+        mol += [m] * (len(typ) - a0)
+    out = dict(w)
+    out.update(
+        n_atoms=len(typ), n_types=4, n_bonds=len(bonds), n_angles=len(angles),
+        type=np.array(typ, np.int32), mol=np.array(mol, np.int32),
+        mass=np.array([ff["m_O"], ff["m_H"], 22.99, 35.45]),
+        charge=np.array([ff["q_O"], ff["q_H"], 0.92, -0.50]),       # cation + anion + diatomic: 0.92 - 0.50 - 0.42 = 0
+        lj_eps=np.array([ff["lj_eps_O"], 0.0, 0.0874, 0.0356]),
+        lj_sigma=np.array([ff["lj_sigma_O"], 0.0, 2.439, 4.478]),
+        bond_idx=np.array(bonds, np.int32).reshape(-1, 2), bond_k=np.array(bk), bond_r0=np.array(br),
+        angle_idx=np.array(angles, np.int32).reshape(-1, 3), angle_k=np.array(ak), angle_th0=np.array(at),
+        positions=np.ascontiguousarray(np.array(pos)),
+    )
+    return out
+
+
 def oscillator_box(n_atoms: int, mass: float, k_tether: float, box: float = 1000.0,
                    seed: int = MASTER_SEED) -> dict:
     """`n_atoms` uncharged, non-interacting atoms tethered harmonically to the origin.
