@@ -19,7 +19,7 @@
 // The DSF radial function needs no erfc/exp: with w = (alpha r)^2,
 //   erfc(x) + (2x/sqrt(pi)) e^{-x^2} = 1 - x^3 S(w),   erfc(x)/x = 1/x - E(w),
 // S and E entire in w, so F/r = qq (1/r^3 - alpha^3 S(w) - fshift/r) with 1/r from one rsqrt and
-// alpha^3 S a degree-17 polynomial in u = 2 r^2/r_c^2 - 1 whose coefficients (fitted at create time
+// alpha^3 S a degree-15 polynomial in u = 2 r^2/r_c^2 - 1 whose coefficients (fitted at create time
 // from the Taylor series of S, qhp_pair_setup) sit in the kernel's constant bank.
 // Full list (each ordered pair evaluated from its own side): no atomics, fixed summation order.
 #include <math.h>
@@ -60,11 +60,12 @@ __device__ __forceinline__ double rsqrt_seeded(double s) {
 }
 
 // even/odd split Horner (two independent chains)
-__device__ __forceinline__ double poly17(const double *c, double u) {
+__device__ __forceinline__ double poly_eval(const double *c, double u) {
+  static_assert(QHP_NPOLY % 2 == 0, "even/odd split");
   const double v = u * u;
-  double a = c[16], b = c[17];
+  double a = c[QHP_NPOLY - 2], b = c[QHP_NPOLY - 1];
 #pragma unroll
-  for (int k = 14; k >= 0; k -= 2) { a = fma(a, v, c[k]); b = fma(b, v, c[k + 1]); }
+  for (int k = QHP_NPOLY - 4; k >= 0; k -= 2) { a = fma(a, v, c[k]); b = fma(b, v, c[k + 1]); }
   return fma(b, u, a);
 }
 
@@ -175,7 +176,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       const double qq = pt[0], eps4 = pt[1];
       const double y = rsqrt_seeded(r2s), y2 = y * y, y3 = y2 * y;
       const double u = fma(r2s, a.u_scale, -1.0);
-      double fr = qq * fma(-a.fshift, y, y3 - poly17(a.cS, u));
+      double fr = qq * fma(-a.fshift, y, y3 - poly_eval(a.cS, u));
       double s6 = 0.0;
       if (__any_sync(0xffffffffu, eps4 != 0.0)) {
         const double s2 = pt[2] * y2;
@@ -186,7 +187,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       Fx = fma(fr, dx, Fx); Fy = fma(fr, dy, Fy); Fz = fma(fr, dz, Fz);
       if (ENERGY) {
         const double r = r2s * y;
-        const double up = qq * (y - poly17(a.cE, u) - a.erfc_rc + a.fshift * (r - a.rc)) + eps4 * (s6 * s6 - s6) - pt[3];
+        const double up = qq * (y - poly_eval(a.cE, u) - a.erfc_rc + a.fshift * (r - a.rc)) + eps4 * (s6 * s6 - s6) - pt[3];
         U += in ? up : 0.0;
         hits += in ? 1ull : 0ull;
       }

@@ -17,7 +17,7 @@
 
 #define QHP_MAX_P 32
 #define QHP_MAX_TYPES 8
-#define QHP_NPOLY 18   // degree-17 polynomials of the damped Coulomb kernel (pair.cu)
+#define QHP_NPOLY 16   // degree-15 polynomials of the damped Coulomb kernel (pair_staged.cu): truncation ~1e-16 at alpha r_c = 1.8
 
 // Philox stream tags
 #define QHP_TAG_PILE 3u
