@@ -174,21 +174,26 @@ __global__ void __launch_bounds__(256) k_list_build(const CellArgs a, const doub
 // Same pair set, written as 16-bit indices into the staged array of the row's cell (pair_staged.cu):
 // index = (number of atoms in the stencil cells before this one, in the stencil order below) + (k - b).
 // Requires nc >= 4 in every dimension (27 distinct stencil cells).
+template <bool FILL>
 __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const double *__restrict__ cent4,
                                                       const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
                                                       const int32_t *__restrict__ cell_start, uint16_t *nbr,
-                                                      int32_t *nbr_count, long long stride, long long *counters) {
+                                                      int32_t *nbr_count, int stride, long long *counters) {
   if (cells_skip(a)) return;
   const int lane = threadIdx.x & 31;
-  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
   if (i >= a.N) return;
-  if (i == 0 && lane == 0 && nbr) counters[0] += 1;
+  if (i == 0 && lane == 0 && FILL) counters[0] += 1;
   const float4 *centf = reinterpret_cast<const float4 *>(cent4 + 4LL * a.N);   // fp32 copies live behind cent4
   const double4 ci = reinterpret_cast<const double4 *>(cent4)[i];
   const float4 fi = centf[i];
+  const int wi = __float_as_int(fi.w);
   const int cell = cell_of[order[i]];
   const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
-  const unsigned lt = (1u << lane) - 1u;
+  unsigned lt = (1u << lane) - 1u;
+  uint16_t *row = nbr + (long long)i * stride;
+  float lo = a.rl2_lo, hi = a.rl2_hi;
+  asm volatile("" : "+r"(lt), "+l"(row));
   int cnt = 0, off = 0;
   // The 27 stencil cells are walked as 9 (x, y) columns.  The three cells of a column are adjacent in z,
   // hence contiguous in slot order unless the column wraps around the box: they are scanned as one run
@@ -199,11 +204,11 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
   const float gzl = fmaxf(fi.z - cz * a.edgef[2], 0.f), gzh = fmaxf((cz + 1) * a.edgef[2] - fi.z, 0.f);
   for (int ox = 0; ox < 3; ++ox) {
     const int ux = cx - 1 + ox, qx = ux < 0 ? ux + a.nc[0] : (ux >= a.nc[0] ? ux - a.nc[0] : ux);
-    const float px = fi.x - (ux < 0 ? -a.boxf[0] : (ux >= a.nc[0] ? a.boxf[0] : 0.f));
+    const float px0 = fi.x - (ux < 0 ? -a.boxf[0] : (ux >= a.nc[0] ? a.boxf[0] : 0.f));
     const float hx = ox == 0 ? fmaxf(fi.x - cx * a.edgef[0], 0.f) : (ox == 2 ? fmaxf((cx + 1) * a.edgef[0] - fi.x, 0.f) : 0.f);
     for (int oy = 0; oy < 3; ++oy) {
       const int uy = cy - 1 + oy, qy = uy < 0 ? uy + a.nc[1] : (uy >= a.nc[1] ? uy - a.nc[1] : uy);
-      const float py = fi.y - (uy < 0 ? -a.boxf[1] : (uy >= a.nc[1] ? a.boxf[1] : 0.f));
+      const float py0 = fi.y - (uy < 0 ? -a.boxf[1] : (uy >= a.nc[1] ? a.boxf[1] : 0.f));
       const float hy = oy == 0 ? fmaxf(fi.y - cy * a.edgef[1], 0.f) : (oy == 2 ? fmaxf((cy + 1) * a.edgef[1] - fi.y, 0.f) : 0.f);
       const float gxy = fmaf(hy, hy, hx * hx);
       const int cb = (qx * a.nc[1] + qy) * a.nc[2];
@@ -221,25 +226,25 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
       int oz = 0;
       while (oz < 3) {
         if (!reach[oz]) { off += eq[oz] - bq[oz]; ++oz; continue; }
-        const int b = bq[oz], run_off = off;
-        const float pz = fi.z - sz[oz];
-        int e = eq[oz], oz2 = oz + 1;
+        const int b = bq[oz];
+        int e = eq[oz], oz2 = oz + 1, idx0 = off - b;           // staged index of slot k = idx0 + k
+        float px = px0, py = py0, pz = fi.z - sz[oz];
         off += eq[oz] - bq[oz];
         while (oz2 < 3 && reach[oz2] && bq[oz2] == e && sz[oz2] == sz[oz]) { e = eq[oz2]; off += eq[oz2] - bq[oz2]; ++oz2; }
-        for (int k0 = b; k0 < e; k0 += 32) {
-          const int k = k0 + lane;
-          bool hit = false;
-          if (k < e && k != i) {
-            const float4 fj = centf[k];
-            const float dxf = px - fj.x, dyf = py - fj.y, dzf = pz - fj.z;
-            const float d2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
-            if (__float_as_int(fj.w) != __float_as_int(fi.w) && d2f < a.rl2_hi)
-              hit = d2f < a.rl2_lo || list_hit_exact(a, cent4, ci, k);
-          }
+        // the inner loop decides the run time of a rebuild: keep its invariants in registers (ptxas
+        // otherwise re-derives the image shifts and reloads the thresholds every iteration)
+        asm volatile("" : "+f"(px), "+f"(py), "+f"(pz), "+f"(lo), "+f"(hi), "+r"(idx0), "+r"(e));
+        const int last = e - 1;
+        for (int k = b + lane; k - lane < e; k += 32) {
+          const float4 fj = centf[min(k, last)];
+          const float dxf = px - fj.x, dyf = py - fj.y, dzf = pz - fj.z;
+          const float d2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
+          bool hit = (k <= last) & (k != i) & (__float_as_int(fj.w) != wi) & (d2f < hi);
+          if (hit && !(d2f < lo)) hit = list_hit_exact(a, cent4, ci, k);      // the thin shell around r_list
           const unsigned mask = __ballot_sync(0xffffffffu, hit);
-          if (hit && nbr) {
+          if (FILL && hit) {
             const int pos = cnt + __popc(mask & lt);
-            if (pos < stride) nbr[i * stride + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)(run_off + k - b);
+            if (pos < stride) row[(pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)(idx0 + k);
           }
           cnt += __popc(mask);
         }
@@ -247,15 +252,15 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
       }
     }
   }
-  if (nbr) {
+  if (FILL) {
     // pad the last 256-entry block with index 0 (a valid staged index; the kernel masks these lanes)
-    const int n = (int)min((long long)cnt, stride), end = (int)min((long long)((n + 255) & ~255), stride);
+    const int n = min(cnt, stride), end = min((n + 255) & ~255, stride);
     for (int pos = n + lane; pos < end; pos += 32)
-      nbr[i * stride + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = 0;
+      row[(pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = 0;
   }
   if (lane == 0) {
-    if (nbr) {
-      nbr_count[i] = (int)min((long long)cnt, stride);
+    if (FILL) {
+      nbr_count[i] = min(cnt, stride);
       if (cnt > stride) counters[1] = 1;
     } else {
       nbr_count[i] = cnt;
@@ -426,10 +431,12 @@ static int list_build(qhp_system *s, const CellArgs &a, bool count_only) {
   const int tb = 256;
   const long long threads = 32LL * s->N;
   const unsigned grid = (unsigned)((threads + tb - 1) / tb);
-  if (s->staged)
-    k_list_build16<<<grid, tb, 0, s->stream>>>(a, s->cent4, s->cell_of, s->order, s->cell_start,
-                                              count_only ? nullptr : s->nbr16, s->nbr_count, s->nbr_stride,
-                                              (long long *)s->counters);
+  if (s->staged && count_only)
+    k_list_build16<false><<<grid, tb, 0, s->stream>>>(a, s->cent4, s->cell_of, s->order, s->cell_start, nullptr, s->nbr_count,
+                                                     (int)s->nbr_stride, (long long *)s->counters);
+  else if (s->staged)
+    k_list_build16<true><<<grid, tb, 0, s->stream>>>(a, s->cent4, s->cell_of, s->order, s->cell_start, s->nbr16, s->nbr_count,
+                                                    (int)s->nbr_stride, (long long *)s->counters);
   else
     k_list_build<<<grid, tb, 0, s->stream>>>(a, s->cent4, s->cell_of, s->order, s->cell_start,
                                             count_only ? nullptr : s->nbr, s->nbr_count, s->nbr_stride,
