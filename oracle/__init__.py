@@ -508,3 +508,16 @@ class Adqtb:
     def get_state(self):
         N = self.top.n_atoms
         return self.x.reshape(1, N, 3).copy(), self.p.reshape(1, N, 3).copy()
+
+
+# ---------------------------------------------------------------- PI-BAR (NEXT-5, Eq. 27-28)
+def pibar(wA, wB, beta: float, max_iter: int = 1000, tol: float = 1e-13):
+    """dF_AB = (1/beta) ln(Z_A/Z_B) from wA = U_B - U_A on samples of A and wB = U_A - U_B on samples of B
+    (Eq. 27-28, solved by fixed-point iteration).  Returns (dF, iterations)."""
+    wA, wB = _f64(wA), _f64(wB)
+    out = C.c_double(0.0)
+    fn = lib().qo_pibar
+    fn.restype = C.c_int
+    it = fn(_p(wA), C.c_int64(wA.size), _p(wB), C.c_int64(wB.size), C.c_double(beta), C.c_int(max_iter),
+            C.c_double(tol), C.byref(out))
+    return out.value, it

@@ -804,3 +804,39 @@ void qo_qtb_adapt_ratio(int n_types, int n_seg, const double *mass_amu, double g
   }
 }
 
+
+/* ------------------------------------------------------------------------------------------
+ * NEXT-5  PI-BAR free-energy estimator (Eq. 27-28).
+ *   dF_AB = beta^-1 ln(Z_A/Z_B) = C + beta^-1 ln( <f(U_A - U_B + C)>_B / <f(U_B - U_A - C)>_A ),   (27)
+ *   C = dF_AB + beta^-1 ln(n_B / n_A),   f(x) = 1 / (1 + exp(beta x)),                               (28)
+ * "a self-consistent set of equations that is solved iteratively" (l.304).
+ * Inputs are the stored series of bead-averaged potential differences (U of Eq. 3):
+ *   wA[i] = U_B - U_A on the n_A configurations sampled in state A,
+ *   wB[j] = U_A - U_B on the n_B configurations sampled in state B.
+ * Reading G26 (paper silent): start from dF = 0; one iteration = Eq. 28 then Eq. 27; stop when
+ * |dF_new - dF| <= tol or after max_iter iterations; returns the number of iterations done.
+ * With U = V on a single bead this is the estimator of Appendix A (Eq. A1); with P = 1 it is BAR.
+ * Pins (tests/test_oracle_pibar.py): U_B = U_A + c gives c exactly; the fixed point solves Bennett's
+ * implicit equation sum_A f = sum_B f (root found with scipy.optimize.brentq); dF_BA = -dF_AB;
+ * classical and finite-P quantum harmonic oscillators against their closed-form partition functions.
+ * ------------------------------------------------------------------------------------------ */
+static double qo_fermi(double beta, double x) { return 1.0 / (1.0 + exp(beta * x)); }
+
+int qo_pibar(const double *wA, int64_t nA, const double *wB, int64_t nB, double beta, int max_iter,
+             double tol, double *dF_out) {
+  double dF = 0.0;
+  int it = 0;
+  while (it < max_iter) {
+    double C = dF + log((double)nB / (double)nA) / beta;                /* Eq. 28 */
+    double sB = 0.0, sA = 0.0;
+    for (int64_t j = 0; j < nB; ++j) sB += qo_fermi(beta, wB[j] + C);   /* <f(U_A - U_B + C)>_B */
+    for (int64_t i = 0; i < nA; ++i) sA += qo_fermi(beta, wA[i] - C);   /* <f(U_B - U_A - C)>_A */
+    double dF_new = C + log((sB / (double)nB) / (sA / (double)nA)) / beta;   /* Eq. 27 */
+    double change = fabs(dF_new - dF);
+    dF = dF_new;
+    ++it;
+    if (change <= tol) break;
+  }
+  *dF_out = dF;
+  return it;
+}
