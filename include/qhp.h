@@ -186,6 +186,18 @@ int qhp_fft_c2c(double *data, int n, int64_t batch, int sign, void *cuda_stream)
  * writes one double per thread to sink (device, grid*block doubles). */
 int qhp_dfma_probe(double *sink, int grid, int block, int64_t iters, void *cuda_stream);
 
+/* ---- post-processing of stored potential-energy series ---------------------------------- */
+/* PI-BAR free-energy difference dF_AB = (1/beta) ln(Z_A/Z_B) (Eq. 27-28):
+ *   dF = C + (1/beta) ln( <f(U_A - U_B + C)>_B / <f(U_B - U_A - C)>_A ),  C = dF + (1/beta) ln(n_B/n_A),
+ *   f(x) = 1/(1 + exp(beta x)), iterated from dF = 0 until |change| <= tol or max_iter iterations (G26).
+ * wA (device, n_A doubles) = U_B - U_A on the configurations sampled in state A, wB (device, n_B) =
+ * U_A - U_B on those sampled in state B, U the bead-averaged potential of Eq. 3 (qhp_observables out[1]);
+ * with a single bead's V it is the estimator of Appendix A, with P = 1 classical BAR.  beta in mol/kcal.
+ * Runs on cuda_stream and synchronises it; dF_host (kcal/mol) and iters_host (may be NULL) are host
+ * pointers.  The inputs are not modified.  QHP_EINVAL for empty series or beta <= 0. */
+int qhp_pibar(const double *wA, int64_t n_A, const double *wB, int64_t n_B, double beta, int max_iter,
+              double tol, void *cuda_stream, double *dF_host, int *iters_host);
+
 #ifdef __cplusplus
 }
 #endif

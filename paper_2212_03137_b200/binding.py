@@ -18,7 +18,7 @@ SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_respa", "qhp_set_a_block", "qhp
            "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
            "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma", "qhp_adqtb_ratio",
            "qhp_adqtb_segment", "qhp_counters", "qhp_profile", "qhp_profile_read", "qhp_check", "qhp_last_error", "qhp_philox_normals",
-           "qhp_fft_c2c", "qhp_dfma_probe"]
+           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar"]
 
 
 class QhpError(RuntimeError):
@@ -84,6 +84,7 @@ def lib():
         L.qhp_philox_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, i64, vp, vp, vp]
         L.qhp_fft_c2c.argtypes = [vp, i32, i64, i32, vp]
         L.qhp_dfma_probe.argtypes = [vp, i32, i32, i64, vp]
+        L.qhp_pibar.argtypes = [vp, i64, vp, i64, C.c_double, i32, C.c_double, vp, C.POINTER(C.c_double), C.POINTER(i32)]
         for name in SYMBOLS:
             if name != "qhp_last_error":
                 getattr(L, name).restype = C.c_int
@@ -332,3 +333,17 @@ def qhp_dfma_probe(grid: int, block: int, iters: int, stream=None):
     if rc:
         raise QhpError(rc, "qhp_dfma_probe")
     return sink
+
+
+def qhp_pibar(wA, wB, beta: float, max_iter: int = 1000, tol: float = 1e-13, stream=None):
+    """PI-BAR (Eq. 27-28) on device series wA = U_B - U_A (samples of A), wB = U_A - U_B (samples
+    of B); returns (dF, iterations)."""
+    torch = _torch()
+    _chk_dev(wA, torch.float64, None, "wA")
+    _chk_dev(wB, torch.float64, None, "wB")
+    dF, it = C.c_double(0.0), C.c_int32(0)
+    rc = lib().qhp_pibar(_ptr(wA), int(wA.numel()), _ptr(wB), int(wB.numel()), float(beta), int(max_iter), float(tol),
+                         _stream_ptr(stream), C.byref(dF), C.byref(it))
+    if rc != 0:
+        raise QhpError(rc, "qhp_pibar")
+    return dF.value, it.value
