@@ -301,6 +301,12 @@ class Rpmd:
         return observables(self.top, self.P, self.Pc, self.T, self.Q, self.Pm, self.uc)
 
 
+def set_contraction_variant(v: int):
+    """0 = literal Eq. 20 (default); 1 = trigonometric interpolation (sqrt 2 on the Nyquist mode of an even P').
+    Process-wide switch of the oracle: reset it to 0 after use."""
+    lib().qo_set_contraction_variant(C.c_int(int(v)))
+
+
 def nm_forces_split(top: Topology, P: int, Pc: int, Q: np.ndarray, cells: bool | None = None):
     """Normal-mode forces of V_f and V_s separately (Eq. 18; used by the RESPA stepper)."""
     Q = _f64(Q)

@@ -148,14 +148,32 @@ void qo_nm_to_beads(int P, int64_t ndof, const double *Q, double *x) {
  * Q_n of the full polymer fed unchanged into the Pc-bead transform (literal reading G3).
  * Pins: C(P,P) = I; C(P,1) = 1/P; rows sum to 1.
  * ------------------------------------------------------------------------------------------ */
+/* Variant of reading G3 (default 0 = literal Eq. 20).  1 = trigonometric interpolation: for even Pc < P the
+ * highest contracted mode is the Nyquist mode of the Pc-bead polymer but the cos member of a degenerate pair
+ * of the full one; evaluating the band-limited interpolant of the P beads at the Pc points gives that mode
+ * the amplitude sqrt(2) Q_{Pc-1} (the sin partner vanishes there).  Pins (tests/test_oracle_nm.py): equals
+ * scipy.signal.resample of the bead positions; C(P,P) = I; odd Pc unchanged; forces = -gradient. */
+static int qo_contraction_variant = 0;
+void qo_set_contraction_variant(int v) { qo_contraction_variant = v; }
+static double qo_top_mode_scale(int P, int Pc) {
+  return (qo_contraction_variant == 1 && Pc % 2 == 0 && Pc < P) ? sqrt(2.0) : 1.0;
+}
+
 void qo_contract(int P, int Pc, int64_t ndof, const double *Q, double *xc) {
-  (void)P;
-  qo_nm_to_beads(Pc, ndof, Q, xc);   /* uses rows n < Pc of Q only ([P][ndof] layout) */
+  double sc = qo_top_mode_scale(P, Pc);
+  if (sc == 1.0) { qo_nm_to_beads(Pc, ndof, Q, xc); return; }   /* uses rows n < Pc of Q only ([P][ndof] layout) */
+  double *Qs = (double *)malloc(sizeof(double) * (size_t)Pc * ndof);
+  memcpy(Qs, Q, sizeof(double) * (size_t)Pc * ndof);
+  for (int64_t d = 0; d < ndof; ++d) Qs[(int64_t)(Pc - 1) * ndof + d] *= sc;
+  qo_nm_to_beads(Pc, ndof, Qs, xc);
+  free(Qs);
 }
 
 /* f^s_n = (1/sqrt Pc) sum_j T^(Pc)[j][n] Fc_j for n < Pc, 0 otherwise (chain rule on Eq. 20). */
 void qo_expand_force(int P, int Pc, int64_t ndof, const double *Fc, double *fs) {
   qo_beads_to_nm(Pc, ndof, Fc, fs);
+  double sc = qo_top_mode_scale(P, Pc);
+  if (sc != 1.0) for (int64_t d = 0; d < ndof; ++d) fs[(int64_t)(Pc - 1) * ndof + d] *= sc;
   for (int64_t e = (int64_t)Pc * ndof; e < (int64_t)P * ndof; ++e) fs[e] = 0.0;
 }
 

@@ -112,3 +112,38 @@ def test_harmonic_closed_form_values():
             wk = O.nm_freq(P, T_K)
             val = KB * T_K * ACC / m * np.sum(1.0 / (w ** 2 + wk ** 2))
         assert abs(val - q2) < 2e-5 * q2, (P, val, q2)
+
+
+def test_trigonometric_contraction_variant_equals_fourier_resampling():
+    """Variant 1 of reading G3: the contracted beads are the band-limited (Fourier) interpolant of the P
+    bead positions evaluated at P' equidistant points -- scipy.signal.resample computes exactly that,
+    independently; the literal Eq. 20 differs from it on the Nyquist mode of an even P' only."""
+    import scipy.signal as ss
+    rng = np.random.default_rng(11)
+    try:
+        for P, Pc in [(32, 4), (8, 4), (16, 2), (12, 6), (32, 5), (8, 3), (8, 8), (6, 1)]:
+            x = rng.standard_normal((P, 7))
+            Q = O.beads_to_nm(x)
+            ref = ss.resample(x, Pc, axis=0)
+            O.set_contraction_variant(1)
+            xv = O.contract(Q, Pc)
+            Cv = O.contraction_matrix(P, Pc)
+            O.set_contraction_variant(0)
+            xl = O.contract(Q, Pc)
+            assert np.abs(xv - ref).max() < 1e-13, (P, Pc)
+            if Pc % 2 == 0 and Pc < P:
+                assert np.abs(xl - ref).max() > 1e-3                  # the literal reading is something else ...
+                d = xl - xv                                           # ... by a pure (-1)^j pattern
+                assert np.abs(d + np.roll(d, 1, axis=0)).max() < 1e-13
+            else:
+                assert np.array_equal(xl, xv)
+            assert np.abs(Cv.sum(axis=1) - 1).max() < 1e-14           # rows still sum to one (centroid preserved)
+            # chain rule: expand_force is the transpose of the contraction
+            Fc = rng.standard_normal((Pc, 7))
+            O.set_contraction_variant(1)
+            fs = O.expand_force(Fc, P)
+            O.set_contraction_variant(0)
+            G = O.nm_to_beads(fs)
+            assert np.abs(G - (P / Pc) * np.einsum("ji,jd->id", Cv, Fc)).max() < 1e-12
+    finally:
+        O.set_contraction_variant(0)
