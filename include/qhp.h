@@ -117,6 +117,17 @@ int qhp_set_respa(qhp_system *sys, int n_alt);
  * square root of the Cayley transform of the free ring-polymer generator,
  *   (q, p) -> (1 + (w dt/2)^2)^(-1/2) (q + dt/(2m) p, p - m w^2 dt/2 q)      (reading G25),
  * stable for any w dt.  The centroid and P = 1 are unchanged.  May be called at any step. */
+/* Contraction variant (reading G3; Eq. 20).  QHP_CONTRACT_LITERAL (default): the
+ * P' lowest normal-mode amplitudes of the full polymer are fed unchanged into the P'-bead transform.
+ * QHP_CONTRACT_TRIG: the contracted beads are the band-limited (Fourier) interpolant of the P beads at P'
+ * points, which differs for even P' < P only: the Nyquist mode of the contracted polymer gets sqrt(2) times
+ * the amplitude of the cos member of the degenerate pair it is fed from (the sin partner vanishes at the
+ * contracted points); positions and the chain-rule force projection change together.  Call before
+ * qhp_set_state (QHP_ESTATE afterwards). */
+#define QHP_CONTRACT_LITERAL 0
+#define QHP_CONTRACT_TRIG 1
+int qhp_set_contraction(qhp_system *sys, int variant);
+
 #define QHP_ABLOCK_EXACT 0
 #define QHP_ABLOCK_CAYLEY 1
 int qhp_set_a_block(qhp_system *sys, int kind);

@@ -409,7 +409,7 @@ void qo_bead_forces(const qo_topology *t, int P, int Pc, const double *xb, doubl
   qo_nm_matrix(P, T); qo_nm_matrix(Pc, Tc);
   for (int j = 0; j < Pc; ++j) for (int i = 0; i < P; ++i) {
     double s = 0.0;
-    for (int n = 0; n < Pc; ++n) s += Tc[j * Pc + n] * T[i * P + n];
+    for (int n = 0; n < Pc; ++n) s += (n == Pc - 1 ? qo_top_mode_scale(P, Pc) : 1.0) * Tc[j * Pc + n] * T[i * P + n];
     C[j * P + i] = sqrt((double)Pc) / sqrt((double)P) * s;
   }
   double *xc = (double *)calloc((size_t)(Pc * nd), sizeof(double));

@@ -14,7 +14,7 @@ QHP_THERMO_NONE, QHP_THERMO_PILE, QHP_THERMO_ADQTB = 0, 1, 2
 _STATUS = {0: "QHP_OK", -1: "QHP_EINVAL", -2: "QHP_ENOMEM", -3: "QHP_ECUDA", -4: "QHP_ESTATE"}
 
 # every symbol include/qhp.h declares (tests check that the library exports them all)
-SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_respa", "qhp_set_a_block", "qhp_set_state", "qhp_get_state", "qhp_set_state_host",
+SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_respa", "qhp_set_a_block", "qhp_set_contraction", "qhp_set_state", "qhp_get_state", "qhp_set_state_host",
            "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
            "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma", "qhp_adqtb_ratio",
            "qhp_adqtb_segment", "qhp_counters", "qhp_profile", "qhp_profile_read", "qhp_check", "qhp_last_error", "qhp_philox_normals",
@@ -66,6 +66,7 @@ def lib():
         L.qhp_step.argtypes = [vp, i64]
         L.qhp_set_respa.argtypes = [vp, i32]
         L.qhp_set_a_block.argtypes = [vp, i32]
+        L.qhp_set_contraction.argtypes = [vp, i32]
         L.qhp_forces.argtypes = [vp, vp]
         L.qhp_observables.argtypes = [vp, vp, i32]
         L.qhp_observables_host.argtypes = [vp, vp, i32]
@@ -211,6 +212,10 @@ class System:
 
     def set_respa(self, n_alt: int):
         self._ok(self._L.qhp_set_respa(self._h, int(n_alt)))
+
+    def set_contraction(self, variant: str):
+        """"literal" (default, Eq. 20 as printed) or "trig" (Fourier interpolation; reading G3); before set_state."""
+        self._ok(self._L.qhp_set_contraction(self._h, {"literal": 0, "trig": 1}[variant]))
 
     def set_a_block(self, kind: str):
         """"exact" (default) or "cayley" = BCOCB (PAPER.md:151)."""

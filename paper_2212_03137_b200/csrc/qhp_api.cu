@@ -459,6 +459,18 @@ extern "C" int qhp_set_respa(qhp_system *s, int n_alt) {
   return QHP_OK;
 }
 
+extern "C" int qhp_set_contraction(qhp_system *s, int variant) {
+  if (!s) return QHP_EINVAL;
+  if (variant != QHP_CONTRACT_LITERAL && variant != QHP_CONTRACT_TRIG) { s->err = "unknown contraction variant"; return QHP_EINVAL; }
+  if (s->have_state) { s->err = "set the contraction variant before qhp_set_state"; return QHP_ESTATE; }
+  nm_matrix(s->Pc, s->T_Pc);
+  if (variant == QHP_CONTRACT_TRIG && s->Pc % 2 == 0 && s->Pc < s->P)
+    for (int j = 0; j < s->Pc; ++j) s->T_Pc[(size_t)j * s->Pc + s->Pc - 1] *= std::sqrt(2.0);   // column of the Nyquist mode
+  QHP_CUDA_OK(s, cudaMemcpyAsync(s->d_Tc, s->T_Pc.data(), sizeof(double) * s->T_Pc.size(), cudaMemcpyHostToDevice, s->stream));
+  QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
+  return QHP_OK;
+}
+
 extern "C" int qhp_set_a_block(qhp_system *s, int kind) {
   if (!s) return QHP_EINVAL;
   if (kind != QHP_ABLOCK_EXACT && kind != QHP_ABLOCK_CAYLEY) { s->err = "unknown A block"; return QHP_EINVAL; }

@@ -3,6 +3,7 @@ import numpy as np
 import pytest
 
 import oracle as O
+from workloads import water as W
 from helpers import read_golden
 
 KB, HBAR, ACC = 1.987204258640832e-3, 1.5178728306651436e-2, 418.4
@@ -145,5 +146,17 @@ def test_trigonometric_contraction_variant_equals_fourier_resampling():
             O.set_contraction_variant(0)
             G = O.nm_to_beads(fs)
             assert np.abs(G - (P / Pc) * np.einsum("ji,jd->id", Cv, Fc)).max() < 1e-12
+        # both force routes of the oracle (normal modes / explicit contraction matrix) follow the switch
+        top = W.water_box(27)
+        top["box"] = np.array([20.0] * 3)
+        t = O.Topology(top)
+        x, _ = W.initial_state(top, 8, 300.0, sigma_bead=0.05)
+        O.set_contraction_variant(1)
+        f, _ = O.nm_forces(t, 8, 4, O.beads_to_nm(x), cells=False)
+        Gm = O.bead_forces(t, 8, 4, x, cells=False)
+        O.set_contraction_variant(0)
+        Gl = O.bead_forces(t, 8, 4, x, cells=False)
+        assert np.abs(O.nm_to_beads(f) - Gm).max() < 1e-11 * np.abs(Gm).max()
+        assert np.abs(Gl - Gm).max() > 1e-6 * np.abs(Gm).max()
     finally:
         O.set_contraction_variant(0)
