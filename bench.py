@@ -48,7 +48,8 @@ FLOP_PER_PAIR_BEAD = 110.0
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_staged<false> launch at C4, from the
 # `ncu --set full` capture summarised in profiles/r1c_summary.md (per launch, like `achieved`)
-NCU_TRAFFIC_BYTES = {("C4", "k_pair_staged"): 1.3636e9 + 2.36e7}
+NCU_TRAFFIC_BYTES = {("C4", "k_pair_staged"): 1.3637e9 + 2.39e7,      # profiles/r1d_summary.md (dram read + write per launch)
+                     ("C3", "k_pair_staged"): 3.409e8 + 9.5e6}
 
 
 def measure_dfma_peak() -> float:
