@@ -351,11 +351,18 @@ def theta(omega, T_K: float):
 
 
 def qtb_filter(n_seg: int, dt: float, T_K: float, mass_amu: float, gamma_z: np.ndarray,
-               classical: bool = False) -> np.ndarray:
+               classical: bool = False, kappa=None) -> np.ndarray:
+    """kappa: optional amplitude factor kappa(omega_j), j = 0..n_seg, on H (reading G11)."""
     g = _f64(gamma_z)
     H = np.empty(n_seg + 1)
-    lib().qo_qtb_filter(C.c_int(n_seg), C.c_double(dt), C.c_double(T_K), C.c_double(mass_amu),
-                        _p(g), C.c_int(int(classical)), _p(H))
+    if kappa is None:
+        lib().qo_qtb_filter(C.c_int(n_seg), C.c_double(dt), C.c_double(T_K), C.c_double(mass_amu),
+                            _p(g), C.c_int(int(classical)), _p(H))
+    else:
+        k = _f64(kappa)
+        assert k.shape == (n_seg + 1,)
+        lib().qo_qtb_filter_kappa(C.c_int(n_seg), C.c_double(dt), C.c_double(T_K), C.c_double(mass_amu),
+                                  _p(g), C.c_int(int(classical)), _p(k), _p(H))
     return H
 
 
@@ -463,6 +470,7 @@ class Adqtb:
         self.avv = np.zeros((top.n_types, n_seg + 1))
         self.avf = np.zeros((top.n_types, n_seg + 1))
         self.ratio_started = False
+        self.kappa = None           # kernel-correction factor kappa(omega_j) [n_seg + 1] (reading G11), None = 1
 
     def set_state(self, x, p, step0: int = 0):
         assert step0 % self.n_seg == 0
@@ -475,7 +483,7 @@ class Adqtb:
 
     def kernels(self):
         return np.stack([qtb_kernel(qtb_filter(self.n_seg, self.dt, self.T, self.top.mass[z],
-                                               self.gamma[z], self.classical))
+                                               self.gamma[z], self.classical, self.kappa))
                          for z in range(self.top.n_types)])
 
     def _new_segment(self):

@@ -636,6 +636,19 @@ void qo_qtb_filter(int n_seg, double dt, double T_K, double mass_amu, const doub
   }
 }
 
+/* Kernel-correction hook (reading G11; PAPER.md:203 cites corrections "for finite timestep [33] and
+ * non-zero friction [35]" without defining them): H_z(omega_j) <- kappa(omega_j) H_z(omega_j) with a
+ * caller-supplied real factor kappa[j], j = 0..n_seg (amplitude factor: the noise PSD of Eq. 13 gets
+ * kappa^2).  kappa == NULL is the identity.
+ * Pins (tests/test_oracle_adqtb.py): kappa == 1 bit-identical; kappa = sqrt(kB T / Theta) gives the
+ * classical kernel h[k != 0] = 0 and the white-noise BAOAB trajectory; F_c linear in a constant kappa. */
+void qo_qtb_filter_kappa(int n_seg, double dt, double T_K, double mass_amu, const double *gamma_z,
+                         int classical, const double *kappa, double *H) {
+  qo_qtb_filter(n_seg, dt, T_K, mass_amu, gamma_z, classical, H);
+  if (kappa)
+    for (int j = 0; j <= n_seg; ++j) H[j] = kappa[j] * H[j];
+}
+
 /* h[k] = (1/N_k) sum_{j=0}^{N_k-1} H(omega_j) exp(+2 pi i j k / N_k), k = -n_seg..n_seg-1,
  * with H extended evenly (H_{N_k - j} = H_j): real and even.  Stored at h[k + n_seg].
  * Pins: DFT_{N_k}(h) = H; h even; Theta == kB T, gamma const  =>  h[k != 0] = 0. */

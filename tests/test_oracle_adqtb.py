@@ -218,3 +218,64 @@ def test_harmonic_kinetic_energy_is_quantum():
     assert abs(K_ref / K_q - 1.0424) < 0.01            # value quoted in SURVEY.md §8(c)
     assert abs(K / K_ref - 1) < 0.05, (K, K_ref, K_q)
     assert K > 5 * 0.5 * KB * T_K                       # nowhere near classical equipartition
+
+
+# ---------------------------------------------------------------- kernel-correction hook (reading G11)
+def test_kappa_identity_and_amplitude_convention():
+    """kappa(omega_j) multiplies the AMPLITUDE filter H (PSD gets kappa^2): kappa = 1 is bit-identical,
+    and kappa = sqrt(kB T / Theta) turns the quantum kernel of a flat gamma into the classical delta."""
+    n_seg, dt, T_K, m = 64, 0.0005, 300.0, 15.999
+    g = np.full(n_seg + 1, 20.0)
+    H0 = O.qtb_filter(n_seg, dt, T_K, m, g)
+    assert np.array_equal(O.qtb_filter(n_seg, dt, T_K, m, g, kappa=np.ones(n_seg + 1)), H0)
+    w = 2 * np.pi * np.arange(n_seg + 1) / (2 * n_seg * dt)
+    kap = np.sqrt(KB * T_K / O.theta(w, T_K))
+    assert kap[0] == 1.0 and kap[-1] < 0.3                                    # a real, non-trivial factor
+    h = O.qtb_kernel(O.qtb_filter(n_seg, dt, T_K, m, g, kappa=kap))
+    Hc = np.sqrt(2 * (m / ACC) * 20.0 * KB * T_K / dt)
+    assert abs(h[n_seg] - Hc) < 1e-12 * Hc
+    assert np.abs(np.delete(h, n_seg)).max() < 1e-12 * Hc
+    # DFT of the corrected kernel = kappa x DFT of the uncorrected one (G10 check carried over)
+    kap2 = 1.0 + 0.4 * np.sin(np.arange(n_seg + 1) * 0.3)
+    h2 = O.qtb_kernel(O.qtb_filter(n_seg, dt, T_K, m, g, kappa=kap2))
+    h0 = O.qtb_kernel(H0)
+    ext = lambda a: np.concatenate([a, a[-2:0:-1]])                          # even extension to N_k
+    D = lambda h: np.fft.fft(np.roll(h, -n_seg)).real                        # h[k], k = 0..N_k-1 ordering
+    assert np.abs(D(h2) - ext(kap2) * D(h0)).max() < 1e-12 * np.abs(D(h0)).max()
+
+
+def test_kappa_classicalising_factor_gives_white_noise_baoab():
+    """With kappa = sqrt(kB T / Theta) and adaptation off, the adQTB trajectory is the white-noise BAOAB
+    one (the pin of test_classical_limit_is_white_noise_baoab reached through the hook, Theta kept)."""
+    top = W.oscillator_box(4, 1.008, 769.3)
+    t = O.Topology(top)
+    dt, T_K, g0, seed, n_seg = 0.0005, 300.0, 20.0, 31, 16
+    rng = np.random.default_rng(10)
+    x = rng.standard_normal((1, 4, 3)) * 0.05
+    p = rng.standard_normal((1, 4, 3)) * 2.0
+    ref = O.Adqtb(t, dt, T_K, g0, seed, n_seg, a_gamma=0.0, classical=True, direct=True, cells=False)
+    sim = O.Adqtb(t, dt, T_K, g0, seed, n_seg, a_gamma=0.0, classical=False, direct=True, cells=False)
+    w = 2 * np.pi * np.arange(n_seg + 1) / (2 * n_seg * dt)
+    sim.kappa = np.sqrt(KB * T_K / O.theta(w, T_K))
+    for s in (ref, sim):
+        s.set_state(x, p)
+        s.step(40)
+    assert np.abs(sim.get_state()[0] - ref.get_state()[0]).max() < 1e-12
+    assert np.abs(sim.get_state()[1] - ref.get_state()[1]).max() < 1e-10
+    # and without the factor the quantum trajectory differs (the hook is not a no-op)
+    q = O.Adqtb(t, dt, T_K, g0, seed, n_seg, a_gamma=0.0, classical=False, direct=True, cells=False)
+    q.set_state(x, p)
+    q.step(40)
+    assert np.abs(q.get_state()[0] - ref.get_state()[0]).max() > 1e-6
+
+
+def test_kappa_constant_scales_the_coloured_force():
+    top = W.oscillator_box(3, 1.008, 769.3)
+    t = O.Topology(top)
+    n_seg, dt, T_K = 32, 0.0005, 300.0
+    g = 20.0 * (1 + 0.5 * np.sin(np.arange(n_seg + 1) * 0.2) ** 2)
+    h1 = O.qtb_kernel(O.qtb_filter(n_seg, dt, T_K, 1.008, g))[None]
+    h3 = O.qtb_kernel(O.qtb_filter(n_seg, dt, T_K, 1.008, g, kappa=np.full(n_seg + 1, 3.0)))[None]
+    F1 = O.qtb_colored_direct(t, n_seg, 5, 2, h1)
+    F3 = O.qtb_colored_direct(t, n_seg, 5, 2, h3)
+    assert np.abs(F3 - 3.0 * F1).max() < 1e-13 * np.abs(F1).max()
