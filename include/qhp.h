@@ -164,6 +164,14 @@ int qhp_adqtb_gamma(qhp_system *sys, double *gamma);
  * the SIMPLE rule (Eq. 23, thermostat a_gamma).  tau_ps: HOST pointer [n_types], or NULL for SIMPLE on
  * every type.  Synchronises. */
 int qhp_adqtb_ratio(qhp_system *sys, const double *tau_ps);
+/* adQTB: kernel-correction hook (PAPER.md:203 cites corrections of the QTB kernel "for finite timestep"
+ * and "non-zero friction" without defining them; SURVEY reading G11): the filter of Eq. 13-14 becomes
+ * H_z(omega_j) = kappa[j] sqrt(2 m_z gamma_z(omega_j) Theta(omega_j) / dt), omega_j = pi j / (n_seg dt),
+ * j = 0..n_seg, the same factor for every type (an AMPLITUDE factor: the noise PSD gets kappa^2).  It
+ * takes effect from the next noise generation (the next segment boundary, or the first step after
+ * qhp_set_state).  kappa: HOST pointer [n_seg+1], finite and >= 0 (else QHP_EINVAL); NULL restores the
+ * identity.  The caller keeps the buffer; the values are copied.  Synchronises. */
+int qhp_adqtb_kappa(qhp_system *sys, const double *kappa);
 int qhp_adqtb_segment(qhp_system *sys, double *Fc, double *vseg);
 /* Counters for measurement: out_host[0] = neighbour-list rebuilds so far, [1] = list entries,
  * [2] = pair-bead interactions inside r_cut at the current positions (full list, both

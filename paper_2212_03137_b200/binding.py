@@ -16,7 +16,7 @@ _STATUS = {0: "QHP_OK", -1: "QHP_EINVAL", -2: "QHP_ENOMEM", -3: "QHP_ECUDA", -4:
 # every symbol include/qhp.h declares (tests check that the library exports them all)
 SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_respa", "qhp_set_a_block", "qhp_set_contraction", "qhp_set_state", "qhp_get_state", "qhp_set_state_host",
            "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
-           "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma", "qhp_adqtb_ratio",
+           "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma", "qhp_adqtb_ratio", "qhp_adqtb_kappa",
            "qhp_adqtb_segment", "qhp_counters", "qhp_profile", "qhp_profile_read", "qhp_check", "qhp_last_error", "qhp_philox_normals",
            "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar"]
 
@@ -75,6 +75,7 @@ def lib():
         L.qhp_contracted.argtypes = [vp, vp]
         L.qhp_adqtb_gamma.argtypes = [vp, vp]
         L.qhp_adqtb_ratio.argtypes = [vp, vp]
+        L.qhp_adqtb_kappa.argtypes = [vp, vp]
         L.qhp_adqtb_segment.argtypes = [vp, vp, vp]
         L.qhp_counters.argtypes = [vp, C.POINTER(i64), i32]
         L.qhp_check.argtypes = [vp]
@@ -209,6 +210,16 @@ class System:
         if tau.size != self.n_types:
             raise ValueError("tau_ps: one value per atom type")
         self._ok(self._L.qhp_adqtb_ratio(self._h, tau.ctypes.data_as(C.c_void_p)))
+
+    def adqtb_kappa(self, kappa):
+        """kappa: kernel-correction factor kappa(omega_j), j = 0..n_seg, on the noise filter H (reading G11), or None."""
+        if kappa is None:
+            self._ok(self._L.qhp_adqtb_kappa(self._h, None))
+            return
+        k = np.ascontiguousarray(kappa, dtype=np.float64)
+        if k.shape != (self.n_seg + 1,):
+            raise ValueError("kappa: one value per frequency omega_j, j = 0..n_seg")
+        self._ok(self._L.qhp_adqtb_kappa(self._h, k.ctypes.data_as(C.c_void_p)))
 
     def set_respa(self, n_alt: int):
         self._ok(self._L.qhp_set_respa(self._h, int(n_alt)))

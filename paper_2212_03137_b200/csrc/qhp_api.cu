@@ -285,7 +285,7 @@ extern "C" int qhp_destroy(qhp_system *s) {
                   s->d_Tc, s->pos4, s->Fs, s->cent4, s->cref, s->pair_tab, s->cell_of, s->cell_count, s->cell_start,
                   s->cell_cursor, s->cell_tmp, s->order, s->rank, s->nbr, s->nbr16, s->nbr_count, s->d2max, s->counters,
                   s->red, s->obs, s->gamma, s->Hf, s->hk, s->H4, s->Fc, s->vseg, s->tw, s->atoms_by_type,
-                  s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p, s->ratio_tau, s->ratio_avv, s->ratio_avf};
+                  s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p, s->ratio_tau, s->ratio_avv, s->ratio_avf, s->kappa};
   for (void *p : ptrs) if (p) cudaFree(p);
   delete s;
   return QHP_OK;
@@ -564,6 +564,22 @@ extern "C" int qhp_adqtb_ratio(qhp_system *s, const double *tau_ps) {
   QHP_CUDA_OK(s, cudaMemsetAsync(s->ratio_avf, 0, sizeof(double) * s->nt * nf, s->stream));
   QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));     // tau_ps is the caller's host buffer
   s->ratio_started = false;
+  return QHP_OK;
+}
+
+extern "C" int qhp_adqtb_kappa(qhp_system *s, const double *kappa) {
+  if (!s) return QHP_EINVAL;
+  if (s->th.kind != QHP_THERMO_ADQTB) { s->err = "not an adQTB system"; return QHP_ESTATE; }
+  const size_t nf = (size_t)s->n_seg + 1;
+  if (!kappa) {                                         // back to the identity
+    if (s->kappa) { cudaStreamSynchronize(s->stream); cudaFree(s->kappa); s->kappa = nullptr; }
+    return QHP_OK;
+  }
+  for (size_t j = 0; j < nf; ++j)
+    if (!(kappa[j] >= 0.0) || !(kappa[j] < 1e300)) { s->err = "kappa must be finite and non-negative"; return QHP_EINVAL; }
+  if (!s->kappa) QHP_CUDA_OK(s, cudaMalloc(&s->kappa, sizeof(double) * nf));
+  QHP_CUDA_OK(s, cudaMemcpyAsync(s->kappa, kappa, sizeof(double) * nf, cudaMemcpyHostToDevice, s->stream));
+  QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));     // kappa is the caller's host buffer
   return QHP_OK;
 }
 

@@ -121,6 +121,7 @@ struct qhp_system {
   int64_t fc_segment = -1;
   double *ratio_tau = nullptr;             // [nt] ps, > 0: RATIO adaptation of that type (Eq. 24-26); NULL: SIMPLE for all
   double *ratio_avv = nullptr, *ratio_avf = nullptr;   // [nt][n_seg+1] exponential-window averages (Eq. 26)
+  double *kappa = nullptr;                 // [n_seg+1] kernel-correction factor on H (reading G11); NULL: 1
   bool ratio_started = false;
 
   // ---- per-phase profiling (qhp_profile) ----

@@ -168,16 +168,18 @@ __device__ __forceinline__ double qtb_theta(double w, double kT) {   // Eq. 14
   return 0.5 * hw / tanh(0.5 * hw / kT);
 }
 
-// Hf[z][j] = sqrt(2 (m_z/ACC) gamma_z[j] Theta(omega_j) / dt), omega_j = 2 pi j / (2 n_seg dt)
+// Hf[z][j] = kappa[j] sqrt(2 (m_z/ACC) gamma_z[j] Theta(omega_j) / dt), omega_j = 2 pi j / (2 n_seg dt);
+// kappa = kernel-correction factor of reading G11, NULL = 1
 __global__ void k_qtb_filter(int nt, int n_seg, double dt, double kT, int classical, const double *__restrict__ mass,
-                             const double *__restrict__ gamma, double *Hf) {
+                             const double *__restrict__ gamma, const double *__restrict__ kappa, double *Hf) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int nf = n_seg + 1;
   if (idx >= nt * nf) return;
   const int z = idx / nf, j = idx % nf;
   const double w = 2.0 * QHP_PI * j / (2.0 * n_seg * dt);
   const double th = classical ? kT : qtb_theta(w, kT);
-  Hf[idx] = sqrt(2.0 * (mass[z] / QHP_ACC) * gamma[idx] * th / dt);
+  const double H = sqrt(2.0 * (mass[z] / QHP_ACC) * gamma[idx] * th / dt);
+  Hf[idx] = kappa ? kappa[j] * H : H;
 }
 
 // hk[z][k + n_seg] = (1/N_k) sum_j H_ext[j] cos(2 pi j k / N_k), k = -n_seg..n_seg-1 (real, even)
@@ -479,7 +481,7 @@ int qhp_qtb_init(qhp_system *s) {
 // Q3 + Q2 + Q4 for segment `seg` with the current gamma_z
 int qhp_qtb_generate(qhp_system *s, int64_t seg) {
   const int ns = s->n_seg, nf = ns + 1, nt = s->nt;
-  k_qtb_filter<<<(nt * nf + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->dt, QHP_KB * s->T, s->th.classical, s->dt_.mass, s->gamma, s->Hf);
+  k_qtb_filter<<<(nt * nf + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->dt, QHP_KB * s->T, s->th.classical, s->dt_.mass, s->gamma, s->kappa, s->Hf);
   QHP_LAUNCH_OK(s);
   k_qtb_kernel<<<(nt * 2 * ns + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->Hf, s->hk);
   QHP_LAUNCH_OK(s);

@@ -111,3 +111,53 @@ def test_ratio_adaptation_matches_oracle(tau):
     ref.step(n_seg)
     assert np.abs(sysg.adqtb_gamma().cpu().numpy() - ref.gamma).max() < 1e-7 * np.abs(ref.gamma).max()
     sysg.check()
+
+
+def test_kappa_hook_matches_oracle():
+    """Kernel-correction factor kappa(omega_j) on the noise filter (reading G11): F_c, gamma and
+    positions over three adapting segments with a non-trivial kappa; NULL restores the identity; bad input."""
+    import paper_2212_03137_b200 as qhp
+    top = W.water_box(216)
+    n_seg = 64
+    kap = 1.0 + 0.4 * np.sin(np.arange(n_seg + 1) * 0.3) - 0.3 * np.arange(n_seg + 1) / n_seg
+    sysg, ref, x0, p0 = make_pair(top, 1, 1, 0.5, "adqtb", gamma0=20.0, n_seg=n_seg, a_gamma=0.5)
+    sysg.adqtb_kappa(kap)
+    ref.kappa = kap
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    for seg in range(3):
+        sysg.step(n_seg)
+        ref.step(n_seg)
+        Fc, _ = sysg.adqtb_segment(want_v=False)
+        assert np.abs(Fc.cpu().numpy() - ref.Fc).max() < 1e-11 * np.sqrt((ref.Fc ** 2).mean()), seg
+        g = sysg.adqtb_gamma().cpu().numpy()
+        assert np.abs(g - ref.gamma).max() < 1e-9 * ref.gamma.max(), seg
+    assert np.abs(sysg.get_state()[0].cpu().numpy() - ref.get_state()[0]).max() < 1e-8
+    sysg.adqtb_kappa(None)                       # identity again from the next segment on
+    ref.kappa = None
+    sysg.step(n_seg)
+    ref.step(n_seg)
+    Fc, _ = sysg.adqtb_segment(want_v=False)
+    assert np.abs(Fc.cpu().numpy() - ref.Fc).max() < 1e-11 * np.sqrt((ref.Fc ** 2).mean())
+    bad = kap.copy()
+    bad[3] = np.nan
+    with pytest.raises(qhp.QhpError):
+        sysg.adqtb_kappa(bad)
+    sysg.check()
+
+
+def test_kappa_classicalising_factor_is_white_noise_baoab():
+    """kappa = sqrt(kB T / Theta(omega)) with Theta kept quantum: the GPU trajectory equals the oracle's CLASSICAL
+    (Theta == kB T) one — the factor enters as an amplitude on H, at the right frequencies."""
+    import oracle as O
+    top = W.water_box(216)
+    n_seg = 16
+    sysg, ref, x0, p0 = make_pair(top, 1, 1, 0.5, "adqtb", gamma0=20.0, n_seg=n_seg, a_gamma=0.0)
+    ref.classical = True
+    w = 2 * np.pi * np.arange(n_seg + 1) / (2 * n_seg * 0.5e-3)
+    sysg.adqtb_kappa(np.sqrt(1.987204258640832e-3 * 300.0 / O.theta(w, 300.0)))
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    sysg.step(20)
+    ref.step(20)
+    assert np.abs(sysg.get_state()[0].cpu().numpy() - ref.get_state()[0]).max() < 1e-8
