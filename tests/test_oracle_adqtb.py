@@ -210,7 +210,6 @@ def test_harmonic_kinetic_energy_is_quantum():
         ks.append((sim.p ** 2).mean() / (2 * m) / ACC)
     K = np.mean(ks)
     w = np.linspace(1e-6, np.pi / dt, 400001)
-    integrand = 2 * g0 * w ** 2 * O.theta(w[::100], T_K).repeat(100)[:w.size] if False else None
     th = 0.5 * HBAR * w / np.tanh(0.5 * HBAR * w / (KB * T_K))
     f = 2 * g0 * w ** 2 * th / ((w0 ** 2 - w ** 2) ** 2 + g0 ** 2 * w ** 2)
     K_ref = 0.5 * 2 * np.trapezoid(f, w) / (2 * np.pi)
