@@ -645,10 +645,11 @@ __global__ void k_contract(const BoxArg bx, const double *__restrict__ Q, int N,
     const double q0 = Q[d];
     cent4[slot * 4 + c] = q0;
     if (c == 0) reinterpret_cast<long long *>(cent4)[slot * 4 + 3] = molid[atom];
+    // fp32 copy: w = molecule id | atom type << 28 (the list entries of the staged pair kernel carry the type)
     // single-precision copy, wrapped into [0, L), for the pre-test of the list build (cells.cu)
     float *centf = reinterpret_cast<float *>(cent4 + 4LL * N);
     centf[slot * 4 + c] = (float)(q0 - bx.box[c] * floor(q0 * bx.inv_box[c]));
-    if (c == 0) reinterpret_cast<int *>(centf)[slot * 4 + 3] = molid[atom];
+    if (c == 0) reinterpret_cast<int *>(centf)[slot * 4 + 3] = molid[atom] | (type[atom] << 28);
     cref[d] = q0;
   }
 }

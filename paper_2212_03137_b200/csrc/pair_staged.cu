@@ -9,13 +9,18 @@
 // shared memory, in coordinates relative to the cell centre (so the minimum image is applied per
 // staged atom, not per pair), and the neighbour table holds 16-bit indices into that staged array.
 //
-// Per atom i (one warp):
-//   check   32 list entries at a time: fp32 distance test on a float4 copy (conservative margin,
+// Per atom i (one warp); a list row = [near entries | far entries], each entry = staged index | type << 13:
+//   near    centroid distance at the list build < r_cut - skin: inside the cutoff for every bead as
+//           long as the list is valid (no bead is farther than skin/2 from that centroid), so the
+//           entry is evaluated straight from the row: no pre-test, no queue (47 % of the pairs);
+//   check   far entries, 32 at a time: fp32 distance test on a float4 copy (conservative margin,
 //           it only rejects pairs that are certainly outside r_c), ballot compaction of the
-//           survivors into a per-warp queue;
+//           survivors into a per-warp queue; the record of the next step is requested one step ahead;
 //   eval    whenever the queue holds >= 32 survivors: all 32 lanes evaluate one pair each in fp64
 //           (exact r^2 < r_c^2 test, LJ + damped-shifted-force Coulomb); no lane idles on the
 //           cutoff, which cost 41 % of the lanes before.
+// Shared memory is addressed through 32-bit shared addresses (inline PTX ld/st.shared): no generic
+// pointers, no 64-bit address arithmetic in the inner loops.
 // The DSF radial function needs no erfc/exp: with w = (alpha r)^2,
 //   erfc(x) + (2x/sqrt(pi)) e^{-x^2} = 1 - x^3 S(w),   erfc(x)/x = 1/x - E(w),
 // S and E entire in w, so F/r = qq (1/r^3 - alpha^3 S(w) - fshift/r) with 1/r from one rsqrt and
@@ -27,22 +32,26 @@
 #include "qhp_internal.cuh"
 
 #ifndef STG_THREADS
-#define STG_THREADS 896           // largest CTA (28 warps, 68 registers); the host launches fewer warps when shared memory is short
+#define STG_THREADS 768           // largest CTA (24 warps, <= 85 registers); the host launches fewer warps when shared memory is short
 #endif
 #define STG_MAX_WARPS (STG_THREADS / 32)
 #define STG_BLOCK 256             // list entries per row block (8 per lane)
-#define STG_QUEUE (STG_BLOCK + 32)
+#define STG_QUEUE (STG_BLOCK + 64)   // <= 31 left over + 31 from the near block + 256
+#define STG_IDX_BITS 13           // list entry = staged index | atom type << 13 (QHP_MAX_TYPES = 8)
+#define STG_IDX_MASK 0x1fffu
 
 struct StagedArgs {
-  int N, Pc, nt, split, cap;
+  int N, Pc, nt, split, cap;     // cap - 1 = dummy staged atom (infinitely far): target of the row padding
   int nc[3];
   double box[3], inv_box[3], cell_edge[3];
   const double *pos4;            // [Pc][N] (x, y, z, type bits), slot order
   double *Fs;                    // [Pc][N][3]
-  const uint16_t *nbr16;         // [N][stride] indices into the staged array of the row's cell (blocked, see below)
+  const uint16_t *nbr16;         // [N][stride] entries (blocked, see below), rows padded to a multiple of 32 with the dummy
   const int32_t *nbr_count, *cell_start;
   long long stride;
   const double *pair_tab;        // [nt*nt][4] = qq, 4 eps, sigma^2, LJ shift
+  double qs[QHP_MAX_TYPES];      // sqrt(Coulomb constant) * charge per type: qq = qs_i * qs_j
+  unsigned lj_mask[QHP_MAX_TYPES]; // bit tj: types (ti, tj) have a Lennard-Jones term
   double rc, rc2, u_scale, fshift, erfc_rc;
   float rc2f;
   double cS[QHP_NPOLY], cE[QHP_NPOLY];
@@ -69,20 +78,28 @@ __device__ __forceinline__ double poly_eval(const double *c, double u) {
   return fma(b, u, a);
 }
 
+// shared-memory accesses through 32-bit shared addresses (no generic pointers, no 64-bit address arithmetic)
+__device__ __forceinline__ float4 lds_f4(uint32_t a) { float4 v; asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a)); return v; }
+__device__ __forceinline__ double2 lds_d2(uint32_t a) { double2 v; asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a)); return v; }
+__device__ __forceinline__ double lds_d(uint32_t a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
+__device__ __forceinline__ uint32_t lds_u(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void sts_u(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
+
 // Row layout of the 16-bit table (written by k_list_build16, cells.cu): the entry of rank `pos` in a
 // row sits at (pos / 256) * 256 + (pos % 32) * 8 + (pos % 256) / 32, i.e. one 16-byte load per lane
-// brings entries pos = 256 m + 32 j + lane, j = 0..7; rows are padded with index 0 up to a multiple
-// of 256 entries.
-// F32: with the float4 copy for the fp32 pre-test (40 B per staged atom).  !F32: neighbourhoods too
-// large for that stage fp64 positions + an int type only (28 B per atom) and pre-test in fp64.
+// brings entries pos = 256 m + 32 j + lane, j = 0..7; a row is padded with the dummy index up to a
+// multiple of 32 entries, so a check step never needs a per-lane tail predicate.
+// Shared memory: XY[cap] (x, y) and Z[cap] fp64, cell-centred; F32: C[cap] float4 copy (x, y, z, type bits)
+// for the fp32 pre-test.  !F32 (neighbourhoods too large for 40 B per atom): 24 B per atom, fp64 pre-test.
 template <bool ENERGY, bool F32>
 __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double *sp = reinterpret_cast<double *>(smem_raw);                  // [cap][3] fp64, cell-centred
-  float4 *sf = reinterpret_cast<float4 *>(sp + 3 * (size_t)a.cap);    // F32: [cap] fp32 copy + type bits
-  int *st = reinterpret_cast<int *>(sp + 3 * (size_t)a.cap);          // !F32: [cap] types
-  double *tab = F32 ? reinterpret_cast<double *>(sf + a.cap) : reinterpret_cast<double *>(st + a.cap);
-  uint32_t *queue = reinterpret_cast<uint32_t *>(tab + QHP_MAX_TYPES * QHP_MAX_TYPES * 4);
+  double2 *XY = reinterpret_cast<double2 *>(smem_raw);
+  double *Z = reinterpret_cast<double *>(XY + a.cap);
+  float4 *C = reinterpret_cast<float4 *>(Z + a.cap);
+  double *tab = F32 ? reinterpret_cast<double *>(C + a.cap) : reinterpret_cast<double *>(Z + a.cap);
+  double *qtab = tab + QHP_MAX_TYPES * QHP_MAX_TYPES * 4;             // sqrt(Coulomb constant) * charge per type
+  uint32_t *queue = reinterpret_cast<uint32_t *>(qtab + QHP_MAX_TYPES);
   __shared__ int off[28], cbeg[27], next_atom;
   __shared__ double su[STG_MAX_WARPS];
 
@@ -90,7 +107,11 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   const int cell = blockIdx.x / a.split, part = blockIdx.x % a.split, bead = blockIdx.y;
   const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
 
-  for (int k = tid; k < a.nt * a.nt * 4; k += nthr) tab[k] = a.pair_tab[k];
+  for (int k = tid; k < a.nt * a.nt * 4; k += nthr) {      // (qq, 4 eps, sigma^2, shift) -> (24 eps, sigma^2, qq, shift)
+    const int f = k & 3;
+    tab[(k & ~3) + (f == 0 ? 2 : (f == 1 ? 0 : (f == 2 ? 1 : 3)))] = (f == 1 ? 6.0 : 1.0) * a.pair_tab[k];
+  }
+  if (tid < a.nt) qtab[tid] = a.qs[tid];
   if (tid < 27) {
     // same stencil order as the list build (cells.cu k_list_build16)
     const int ox = tid / 9, oy = (tid / 3) % 3, oz = tid % 3;
@@ -109,130 +130,173 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   __syncthreads();
   const int total = off[27];
   if (off[14] == off[13]) return;            // empty home cell
-  if (total > a.cap) {                       // cannot happen after the host-side capacity check
+  if (total > a.cap - 1) {                   // cannot happen after the host-side capacity check
     if (tid == 0) a.counters[7] = 1;
     return;
   }
   // ---- stage the neighbourhood in coordinates relative to the cell centre ------------------------
-  const double ctr[3] = {(cx + 0.5) * a.cell_edge[0], (cy + 0.5) * a.cell_edge[1], (cz + 0.5) * a.cell_edge[2]};
   const double4 *pos = reinterpret_cast<const double4 *>(a.pos4) + (long long)bead * a.N;
-  for (int g = tid, s = 0; g < total; g += nthr) {
-    while (g >= off[s + 1]) ++s;
-    const double4 p = pos[cbeg[s] + g - off[s]];
-    double lx = p.x - ctr[0], ly = p.y - ctr[1], lz = p.z - ctr[2];
-    lx = fma(-a.box[0], rint(lx * a.inv_box[0]), lx);
-    ly = fma(-a.box[1], rint(ly * a.inv_box[1]), ly);
-    lz = fma(-a.box[2], rint(lz * a.inv_box[2]), lz);
-    sp[3 * g] = lx; sp[3 * g + 1] = ly; sp[3 * g + 2] = lz;
-    if (F32) sf[g] = make_float4((float)lx, (float)ly, (float)lz, __int_as_float((int)__double_as_longlong(p.w)));
-    else st[g] = (int)__double_as_longlong(p.w);
+  {
+    const double ctr[3] = {(cx + 0.5) * a.cell_edge[0], (cy + 0.5) * a.cell_edge[1], (cz + 0.5) * a.cell_edge[2]};
+    const double MAGIC = 6755399441055744.0;             // 1.5 * 2^52: (t + MAGIC) - MAGIC = rint(t) for |t| < 2^51
+    constexpr int UN = 4;                                // independent loads in flight per thread
+    for (int g0 = tid; g0 < total; g0 += UN * nthr) {
+      double4 p[UN];
+      int s = 0;
+#pragma unroll
+      for (int u = 0; u < UN; ++u) {
+        const int g = g0 + u * nthr;
+        if (g < total) {
+          while (g >= off[s + 1]) ++s;
+          p[u] = pos[cbeg[s] + g - off[s]];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < UN; ++u) {
+        const int g = g0 + u * nthr;
+        if (g < total) {
+          double lx = p[u].x - ctr[0], ly = p[u].y - ctr[1], lz = p[u].z - ctr[2];
+          lx = fma(-a.box[0], (lx * a.inv_box[0] + MAGIC) - MAGIC, lx);
+          ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
+          lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
+          XY[g] = make_double2(lx, ly); Z[g] = lz;
+          if (F32) C[g] = make_float4((float)lx, (float)ly, (float)lz, __int_as_float((int)__double_as_longlong(p[u].w)));
+        }
+      }
+    }
+    if (tid == 0) {                                      // the dummy: every pre-test against it fails
+      XY[a.cap - 1] = make_double2(1e9, 1e9); Z[a.cap - 1] = 1e9;
+      if (F32) C[a.cap - 1] = make_float4(1e9f, 1e9f, 1e9f, 0.f);
+    }
   }
   __syncthreads();
 
   const int h0 = off[13], nh = off[14] - off[13], slot0 = cbeg[13];
-  uint32_t *ql = queue + warp * STG_QUEUE + lane;          // this lane's view of the warp's queue
-  unsigned lt = (1u << lane) - 1u;
-  asm volatile("" : "+l"(ql), "+r"(lt));                   // keep both in registers (ptxas would recompute them per use)
+  const uint32_t sXY = (uint32_t)__cvta_generic_to_shared(XY), sZ = (uint32_t)__cvta_generic_to_shared(Z),
+                 sC = (uint32_t)__cvta_generic_to_shared(C), sTab = (uint32_t)__cvta_generic_to_shared(tab), sQt = (uint32_t)__cvta_generic_to_shared(qtab),
+                 sQ = (uint32_t)__cvta_generic_to_shared(queue) + warp * (STG_QUEUE * 4);
+  const unsigned lt = (1u << lane) - 1u;
   double U = 0.0;
   unsigned long long hits = 0;
 
   // Atoms of the home cell are handed to the warps dynamically (the CTAs of one cell take the atoms
   // ii = part, part + split, ...); each atom is summed by one warp in a fixed order, so the result
-  // does not depend on which warp took it.  The next row block -- of this row or of the next atom's
-  // row -- is in flight while the current one is processed.
-  auto grab = [&]() {
+  // does not depend on which warp took it.
+  for (;;) {
     int t = 0;
     if (lane == 0) t = atomicAdd(&next_atom, 1);
-    return part + a.split * __shfl_sync(0xffffffffu, t, 0);
-  };
-  auto load_block = [&](int ii, int m) {
-    return *reinterpret_cast<const uint4 *>(a.nbr16 + (slot0 + ii) * a.stride + STG_BLOCK * m + 8 * lane);
-  };
-
-  int ii = grab();
-  int n = (ii < nh) ? a.nbr_count[slot0 + ii] : 0;
-  uint4 cur = make_uint4(0u, 0u, 0u, 0u), nxt = cur;
-  if (ii < nh && n > 0) cur = load_block(ii, 0);
-  int ii_n = grab();
-  int n_n = (ii_n < nh) ? a.nbr_count[slot0 + ii_n] : 0;
-
-  while (ii < nh) {
-    const int ei = h0 + ii;
+    const int ii = part + a.split * __shfl_sync(0xffffffffu, t, 0);
+    if (ii >= nh) break;
+    const uint32_t ei = (uint32_t)(h0 + ii);
     const long long slot = slot0 + ii;
-    const float4 fi = F32 ? sf[ei] : make_float4(0.f, 0.f, 0.f, 0.f);
-    const double xi = sp[3 * ei], yi = sp[3 * ei + 1], zi = sp[3 * ei + 2];
-    const double *tab_i = tab + (F32 ? __float_as_int(fi.w) : st[ei]) * a.nt * 4;
+    const int nc2 = a.nbr_count[slot];                   // far | near << 16 (cells.cu k_list_build16)
+    const int n = nc2 & 0xffff, nnear = nc2 >> 16;
+    const uint16_t *rowp = a.nbr16 + slot * a.stride;
+    const int nblk = 1 + (n + STG_BLOCK - 1) / STG_BLOCK;  // block 0: near entries, blocks 1..: far entries
+    uint4 cur = *reinterpret_cast<const uint4 *>(rowp + 8 * lane);
+    const double2 xyi = lds_d2(sXY + ei * 16);
+    const double zi = lds_d(sZ + ei * 8);
+    float4 ci = make_float4(0.f, 0.f, 0.f, 0.f);
+    int ti;
+    if (F32) { ci = lds_f4(sC + ei * 16); ti = __float_as_int(ci.w); }
+    else ti = (int)__double_as_longlong(pos[slot].w);
+    const uint32_t sTi = sTab + (uint32_t)(ti * a.nt) * 32u;
+    const double qi = lds_d(sQt + ti * 8);
+    const unsigned lj_mask = a.lj_mask[ti];
+    const bool lj_row = lj_mask != 0u;
     double Fx = 0.0, Fy = 0.0, Fz = 0.0;
-    int qn = 0;
+    uint32_t qa = sQ;                                    // byte address of the queue end
 
-    // one pair per lane, fp64: LJ + damped-shifted-force Coulomb (oracle O3)
+    // one pair per lane, fp64: LJ + damped-shifted-force Coulomb (oracle O3); the fp64 test decides
     auto eval = [&](uint32_t entry, bool active) {
-      const double *pj = sp + 3 * (entry & 0xffffu);
-      const double *pt = tab_i + 4 * (entry >> 16);
-      const double dx = xi - pj[0], dy = yi - pj[1], dz = zi - pj[2];
+      const uint32_t sj = entry & STG_IDX_MASK, tj = entry >> STG_IDX_BITS;
+      const double2 xyj = lds_d2(sXY + sj * 16);
+      const double zj = lds_d(sZ + sj * 8);
+      const double qq = qi * lds_d(sQt + tj * 8);
+      const double dx = xyi.x - xyj.x, dy = xyi.y - xyj.y, dz = zi - zj;
       const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-      const bool in = active && r2 < a.rc2;          // the fp64 test decides
-      const double r2s = in ? r2 : a.rc2;
-      const double qq = pt[0], eps4 = pt[1];
-      const double y = rsqrt_seeded(r2s), y2 = y * y, y3 = y2 * y;
-      const double u = fma(r2s, a.u_scale, -1.0);
-      double fr = qq * fma(-a.fshift, y, y3 - poly_eval(a.cS, u));
-      double s6 = 0.0;
-      if (__any_sync(0xffffffffu, eps4 != 0.0)) {
-        const double s2 = pt[2] * y2;
+      const bool in = active && r2 < a.rc2;
+      const double y = rsqrt_seeded(r2), y2 = y * y;
+      const double u = fma(r2, a.u_scale, -1.0);
+      double fr = qq * fma(y, y2 - a.fshift, -poly_eval(a.cS, u));
+      double s6 = 0.0, eps24 = 0.0;
+      if (lj_row && __any_sync(0xffffffffu, (lj_mask >> tj) & 1u)) {   // LJ partners are rare (O-O only in water)
+        const double2 lj = lds_d2(sTi + tj * 32);        // 24 eps, sigma^2
+        eps24 = lj.x;
+        const double s2 = lj.y * y2;
         s6 = s2 * s2 * s2;
-        fr = fma(6.0 * eps4 * y2, fma(2.0 * s6, s6, -s6), fr);
+        fr = fma(eps24 * y2, fma(s6 + s6, s6, -s6), fr);
       }
       fr = in ? fr : 0.0;
       Fx = fma(fr, dx, Fx); Fy = fma(fr, dy, Fy); Fz = fma(fr, dz, Fz);
       if (ENERGY) {
-        const double r = r2s * y;
-        const double up = qq * (y - poly_eval(a.cE, u) - a.erfc_rc + a.fshift * (r - a.rc)) + eps4 * (s6 * s6 - s6) - pt[3];
+        const double r = r2 * y;
+        const double up = qq * (y - poly_eval(a.cE, u) - a.erfc_rc + a.fshift * (r - a.rc)) +
+                          (1.0 / 6.0) * eps24 * (s6 * s6 - s6) - lds_d(sTi + tj * 32 + 24);
         U += in ? up : 0.0;
         hits += in ? 1ull : 0ull;
       }
     };
 
-    for (int m = 0; STG_BLOCK * m < n; ++m) {
-      if (STG_BLOCK * (m + 1) < n) nxt = load_block(ii, m + 1);
-      else if (ii_n < nh && n_n > 0) nxt = load_block(ii_n, 0);
-      // ---- check: fp32 pre-test of 8 x 32 entries, survivors compacted into the queue ----------------
-      const int left = n - STG_BLOCK * m - lane;           // entry j of this lane is real iff 32 j < left
+    for (int m = 0; m < nblk; ++m) {
+      uint4 nxt = cur;
+      if (m + 1 < nblk) nxt = *reinterpret_cast<const uint4 *>(rowp + STG_BLOCK * (m + 1) + 8 * lane);
       const uint32_t w[4] = {cur.x, cur.y, cur.z, cur.w};
+      auto entry = [&](int j) { return (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu); };
+      if (m == 0) {
+        // ---- near entries: inside the cutoff for every bead while the list is valid -> no pre-test, no queue ----
+        const int nfull = nnear >> 5, rem = nnear & 31;
+        // rolled loop (one copy of the evaluation code): entry j of this lane selected from the four words
+#pragma unroll 1
+        for (int j = 0; j <= nfull; ++j) {
+          const uint32_t ww = (j & 4) ? ((j & 2) ? cur.w : cur.z) : ((j & 2) ? cur.y : cur.x);
+          const uint32_t e = (j & 1) ? (ww >> 16) : (ww & 0xffffu);
+          if (j < nfull) eval(e, true);
+          else if (rem) {                                // the partial last step joins the queue of the far survivors
+            if (lane < rem) sts_u(qa + lane * 4, e);
+            qa += rem * 4;
+          }
+        }
+      } else {
+      const int nst = min(8, (n - STG_BLOCK * (m - 1) + 31) >> 5);
+      // ---- check: pre-test of 32 entries per step, survivors compacted into the queue; the staged record
+      //      of the next step is requested before this step's compaction store ------------------------------
+      float4 cj = make_float4(0.f, 0.f, 0.f, 0.f);
+      double2 xyj = make_double2(0.0, 0.0);
+      double zj = 0.0;
+      if (F32) cj = lds_f4(sC + (entry(0) & STG_IDX_MASK) * 16);
+      else { xyj = lds_d2(sXY + (entry(0) & STG_IDX_MASK) * 16); zj = lds_d(sZ + (entry(0) & STG_IDX_MASK) * 8); }
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
-        if (32 * j >= n - STG_BLOCK * m) break;            // warp-uniform: the row ends before this step
-        const uint32_t e = (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
+        if (j >= nst) break;
+        const uint32_t e = entry(j);
         bool hit;
-        uint32_t tj;
         if (F32) {
-          const float4 pj = sf[e];
-          const float dxf = fi.x - pj.x, dyf = fi.y - pj.y, dzf = fi.z - pj.z;
-          const float r2f = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf));
-          hit = (32 * j < left) && r2f < a.rc2f;
-          tj = (uint32_t)__float_as_int(pj.w);
+          const float dxf = ci.x - cj.x, dyf = ci.y - cj.y, dzf = ci.z - cj.z;
+          hit = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf)) < a.rc2f;
+          if (j < 7) cj = lds_f4(sC + (entry(j + 1) & STG_IDX_MASK) * 16);
         } else {
-          const double *pj = sp + 3 * e;
-          const double dx = xi - pj[0], dy = yi - pj[1], dz = zi - pj[2];
-          hit = (32 * j < left) && fma(dz, dz, fma(dy, dy, dx * dx)) < a.rc2;
-          tj = (uint32_t)st[e];
+          const double dx = xyi.x - xyj.x, dy = xyi.y - xyj.y, dz = zi - zj;
+          hit = fma(dz, dz, fma(dy, dy, dx * dx)) < a.rc2;
+          if (j < 7) { xyj = lds_d2(sXY + (entry(j + 1) & STG_IDX_MASK) * 16); zj = lds_d(sZ + (entry(j + 1) & STG_IDX_MASK) * 8); }
         }
         const unsigned mask = __ballot_sync(0xffffffffu, hit);
-        if (hit) ql[qn + __popc(mask & lt) - lane] = e | (tj << 16);
-        qn += __popc(mask);
+        if (hit) sts_u(qa + __popc(mask & lt) * 4, e);
+        qa += __popc(mask) * 4;
+      }
       }
       __syncwarp();
       // ---- eval: full warps of survivors ---------------------------------------------------------------
-      while (qn >= 32) {
-        qn -= 32;
-        eval(ql[qn], true);
+      while (qa >= sQ + 128) {
+        qa -= 128;
+        eval(lds_u(qa + lane * 4), true);
       }
       __syncwarp();
       cur = nxt;
     }
-    if (qn > 0) {
-      const bool act = lane < qn;
-      eval(act ? ql[0] : (uint32_t)ei, act);
+    if (qa > sQ) {
+      const bool act = sQ + lane * 4 < qa;
+      eval(act ? lds_u(sQ + lane * 4) : ei, act);
       __syncwarp();
     }
 #pragma unroll
@@ -245,10 +309,6 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       double *o = a.Fs + ((long long)bead * a.N + slot) * 3;
       o[0] = Fx; o[1] = Fy; o[2] = Fz;
     }
-    if (n == 0 && ii_n < nh && n_n > 0) cur = load_block(ii_n, 0);   // nothing was prefetched for an empty row
-    ii = ii_n; n = n_n;
-    ii_n = grab();
-    n_n = (ii_n < nh) ? a.nbr_count[slot0 + ii_n] : 0;
   }
   if (ENERGY) {
 #pragma unroll
@@ -321,9 +381,9 @@ static long double fit_poly(int which, long double wmax, long double scale, doub
   return worst;
 }
 
-static size_t staged_atom_bytes(bool f32) { return 3 * sizeof(double) + (f32 ? sizeof(float4) : sizeof(int)); }
+static size_t staged_atom_bytes(bool f32) { return 3 * sizeof(double) + (f32 ? sizeof(float4) : 0); }
 static size_t staged_smem_bytes(int cap, int warps, bool f32) {
-  return (size_t)cap * staged_atom_bytes(f32) + 16 + sizeof(double) * QHP_MAX_TYPES * QHP_MAX_TYPES * 4 +
+  return (size_t)cap * staged_atom_bytes(f32) + 16 + sizeof(double) * (QHP_MAX_TYPES * QHP_MAX_TYPES * 4 + QHP_MAX_TYPES) +
          sizeof(uint32_t) * (size_t)warps * STG_QUEUE;
 }
 
@@ -365,14 +425,14 @@ int qhp_pair_staged_partials(const qhp_system *s) { return s->ncell * 8 * s->Pc;
 // list builds); sets staged_warps / staged_cap.  False: the neighbourhood does not fit at all.
 bool qhp_pair_staged_fit(qhp_system *s, long long region) {
   static const int tries[] = {STG_MAX_WARPS, 24, 16};
-  const long long need = region + region / 16 + 32;
+  const long long need = region + region / 16 + 32 + 1;               // + the dummy at cap - 1
   // first choice: the fp32 pre-test copy with the largest CTA; then the same CTA sizes without the copy
   for (int f32 = 1; f32 >= 0; --f32)
     for (int w : tries) {
       if (w > STG_MAX_WARPS) continue;
       const long long room = (long long)s->staged_smem_max - (long long)staged_smem_bytes(0, w, f32 != 0);
       long long cap = room / (long long)staged_atom_bytes(f32 != 0);
-      if (cap > 65534) cap = 65534;                                    // 16-bit list entries
+      if (cap > (1 << STG_IDX_BITS)) cap = 1 << STG_IDX_BITS;           // 13-bit staged indices in the list entries
       cap &= ~3LL;                                                     // keeps the arrays behind the positions aligned
       if (cap >= need) { s->staged_warps = w; s->staged_cap = (int)cap; s->staged_f32 = f32 != 0; return true; }
       if (f32 && w == STG_MAX_WARPS) break;                            // a smaller CTA is worse than dropping the copy
@@ -402,6 +462,12 @@ int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned lo
     a.rc2f = (float)(rc * rc + 4.0 * err) * (1.0f + 1.2e-7f);
   }
   for (int k = 0; k < QHP_NPOLY; ++k) { a.cS[k] = s->polyS[k]; a.cE[k] = s->polyE[k]; }
+  for (int t = 0; t < s->nt; ++t) {
+    a.qs[t] = sqrt(QHP_COUL) * s->charge[t];
+    a.lj_mask[t] = 0u;
+    for (int u = 0; u < s->nt; ++u)
+      if (s->lj_eps[t] > 0 && s->lj_eps[u] > 0) a.lj_mask[t] |= 1u << u;
+  }
   a.part = part; a.count = count; a.counters = (long long *)s->counters;
   const dim3 grid((unsigned)(s->ncell * s->staged_split), (unsigned)s->Pc);
   const size_t smem = staged_smem_bytes(s->staged_cap, s->staged_warps, s->staged_f32);
