@@ -109,14 +109,10 @@ int qhp_step(qhp_system *sys, int64_t nsteps);
  * with V_f (bonds, angles, tethers; all P beads) in Bf and V_s (LJ + DSF Coulomb; P_contract beads) in
  * Bs.  qhp_step keeps counting INNER steps of dt (one Philox index per O block) and then accepts
  * multiples of n_alt only; V_s and the neighbour objects are evaluated once per n_alt inner steps.
- * n_alt = 1 (default) is plain B A O A B.  Call it at a multiple of n_alt steps; not with adQTB. */
+ * n_alt = 1 (default) is plain B A O A B.  Call it at a multiple of n_alt steps (the closing kicks of the
+ * last step are applied first, with the n_alt they were taken under); not with adQTB. */
 int qhp_set_respa(qhp_system *sys, int n_alt);
 
-/* A block of the splitting (PAPER.md:151): QHP_ABLOCK_EXACT (default) = exact harmonic evolution of the
- * fluctuation modes over dt/2 (Eq. 17); QHP_ABLOCK_CAYLEY = the BCOCB variant, whose half-step is the
- * square root of the Cayley transform of the free ring-polymer generator,
- *   (q, p) -> (1 + (w dt/2)^2)^(-1/2) (q + dt/(2m) p, p - m w^2 dt/2 q)      (DESIGN.md reading G25),
- * stable for any w dt.  The centroid and P = 1 are unchanged.  May be called at any step. */
 /* Contraction variant (reading G3; Eq. 20).  QHP_CONTRACT_LITERAL (default): the
  * P' lowest normal-mode amplitudes of the full polymer are fed unchanged into the P'-bead transform.
  * QHP_CONTRACT_TRIG: the contracted beads are the band-limited (Fourier) interpolant of the P beads at P'
@@ -128,6 +124,11 @@ int qhp_set_respa(qhp_system *sys, int n_alt);
 #define QHP_CONTRACT_TRIG 1
 int qhp_set_contraction(qhp_system *sys, int variant);
 
+/* A block of the splitting (PAPER.md:151): QHP_ABLOCK_EXACT (default) = exact harmonic evolution of the
+ * fluctuation modes over dt/2 (Eq. 17); QHP_ABLOCK_CAYLEY = the BCOCB variant, whose half-step is the
+ * square root of the Cayley transform of the free ring-polymer generator,
+ *   (q, p) -> (1 + (w dt/2)^2)^(-1/2) (q + dt/(2m) p, p - m w^2 dt/2 q)      (DESIGN.md reading G25),
+ * stable for any w dt.  The centroid and P = 1 are unchanged.  May be called at any step. */
 #define QHP_ABLOCK_EXACT 0
 #define QHP_ABLOCK_CAYLEY 1
 int qhp_set_a_block(qhp_system *sys, int kind);

@@ -633,8 +633,17 @@ __global__ void k_contract(const BoxArg bx, const double *__restrict__ Q, int N,
     for (int n = 0; n < Pc; ++n) s += Tc[j * Pc + n] * Q[n * ND + d];
     const double xc = spc * s;
     if (mode == 0) {
-      // a list built on the centroids can only cover beads closer than skin/2 to their centroid
-      if (cent4 && (xc - Q[d]) * (xc - Q[d]) > thresh2) counters[6] = 1;
+      // a list built on the centroids can only cover beads closer than skin/2 to their centroid: the
+      // thread of component 0 tests the NORM of the bead's offset (all three components)
+      if (cent4 && c == 0) {
+        double n2 = (xc - Q[d]) * (xc - Q[d]);
+        for (int cc = 1; cc < 3; ++cc) {
+          double sc = 0.0;
+          for (int n = 0; n < Pc; ++n) sc += Tc[j * Pc + n] * Q[n * ND + d + cc];
+          n2 += (spc * sc - Q[d + cc]) * (spc * sc - Q[d + cc]);
+        }
+        if (n2 > thresh2) counters[6] = 1;
+      }
       pos4[((long long)j * N + slot) * 4 + c] = xc;
       if (c == 0) reinterpret_cast<long long *>(pos4)[((long long)j * N + slot) * 4 + 3] = type[atom];
     } else {

@@ -455,6 +455,9 @@ extern "C" int qhp_set_respa(qhp_system *s, int n_alt) {
   if (n_alt < 1) { s->err = "n_alt must be >= 1"; return QHP_EINVAL; }
   if (s->th.kind == QHP_THERMO_ADQTB && n_alt != 1) { s->err = "RESPA is not available with adQTB"; return QHP_EINVAL; }
   if (s->have_state && s->step % n_alt != 0) { s->err = "n_alt must divide the current step index"; return QHP_ESTATE; }
+  // the closing half kicks of the last step are still pending and carry the weights of the OLD n_alt
+  // (w_slow = n_alt dt/2, qhp_nm_integrate): apply them before the weights change
+  if (s->have_state) { const int rc = flush_kick(s); if (rc) return rc; }
   s->n_alt = n_alt;
   return QHP_OK;
 }

@@ -3,7 +3,7 @@ segment spectra and the gamma_z(omega) adaptation (Eq. 12-14, 21-23; l.
 import numpy as np
 import pytest
 
-from gpu_common import make_pair, to_dev
+from gpu_common import make_pair, oracle_adapt_from_segment, to_dev
 from workloads import water as W
 
 pytestmark = pytest.mark.gpu
@@ -77,13 +77,47 @@ def test_c1_first_segment_and_boundary():
     assert np.abs(Fc.cpu().numpy() - ref.Fc).max() < 1e-11 * np.sqrt((ref.Fc ** 2).mean())
     sysg.step(n_seg - 20)
     ref.step(n_seg - 20)
+    # trajectories diverge chaotically over 1024 steps (Lyapunov growth of rounding differences): the
+    # velocities are compared with a tolerance that reflects it, and gamma_z is compared at 1e-9 against the
+    # oracle's spectra + adaptation applied to the product's OWN segment arrays
     g = sysg.adqtb_gamma().cpu().numpy()
-    # trajectories diverge chaotically over 1024 steps (Lyapunov growth of rounding differences), so
-    # gamma after the segment is compared with a tolerance that reflects the velocity differences
-    _, v = sysg.adqtb_segment(want_fc=False)
-    dv = np.abs(v.cpu().numpy() - ref.vseg).max() / np.sqrt((ref.vseg ** 2).mean())
+    Fc, v = sysg.adqtb_segment()
+    Fc, v = Fc.cpu().numpy(), v.cpu().numpy()
+    dv = np.abs(v - ref.vseg).max() / np.sqrt((ref.vseg ** 2).mean())
     assert dv < 1e-4
-    assert np.abs(g - ref.gamma).max() < max(1e-9, 100 * dv) * ref.gamma.max()
+    import oracle as O
+    g_ref, _ = oracle_adapt_from_segment(O.Topology(top), n_seg, 0.5e-3, 20.0, 0.5, 0.01, v, Fc,
+                                         np.full_like(g, 20.0))
+    assert np.abs(g - g_ref).max() < 1e-9 * g_ref.max()
+    assert np.abs(g - 20.0).max() > 0.1                     # the adaptation did move gamma
+    sysg.check()
+
+
+@pytest.mark.parametrize("tau", [None, [0.05, -1.0]])
+def test_c1_segment_size_gamma_at_1e9(tau):
+    """configs[1]'s n_seg = 1024 (128-thread spectra groups, 9 bins per thread, 2048-point in-kernel FFT): gamma_z
+    after each of two adapting segments to 1e-9 of the oracle's update of the product's own v_seg, F_c; SIMPLE
+    (Eq. 23) and, for the types with tau > 0, RATIO (Eq. 24-26)."""
+    import oracle as O
+    top = W.water_box(216)
+    n_seg, dt, g0 = 1024, 0.5e-3, 20.0
+    sysg, _, x0, p0 = make_pair(top, 1, 1, 0.5, "adqtb", gamma0=g0, n_seg=n_seg, a_gamma=0.5)
+    otop = O.Topology(top)
+    ratio = None
+    if tau is not None:
+        sysg.adqtb_ratio(tau)
+        z = np.zeros((otop.n_types, n_seg + 1))
+        ratio = dict(tau=tau, avv=z, avf=z.copy(), started=False)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    g_prev = np.full((otop.n_types, n_seg + 1), g0)
+    for seg in range(2):
+        sysg.step(n_seg)
+        Fc, v = sysg.adqtb_segment()
+        g = sysg.adqtb_gamma().cpu().numpy()
+        g_ref, ratio = oracle_adapt_from_segment(otop, n_seg, dt, g0, 0.5, 0.01, v.cpu().numpy(), Fc.cpu().numpy(),
+                                                 g_prev, ratio)
+        assert np.abs(g - g_ref).max() < 1e-9 * np.abs(g_ref).max(), seg
+        g_prev = g
     sysg.check()
 
 

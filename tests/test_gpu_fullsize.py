@@ -8,7 +8,7 @@ one, are compared on a seeded sample.  Tolerances are BASELINE.json north_star's
 import numpy as np
 import pytest
 
-from gpu_common import make_pair, to_dev
+from gpu_common import make_pair, oracle_adapt_from_segment, to_dev
 from workloads import water as W
 
 pytestmark = pytest.mark.gpu
@@ -65,11 +65,11 @@ def test_c4_full_size_lists_forces_steps():
     G = sysg.forces().cpu().numpy()
     Gref = ref.forces()
     assert np.abs(G - Gref).max() < FTOL * np.abs(Gref).max()
-    sysg.step(2)
-    ref.step(2)
+    sysg.step(10)                                               # half of north_star's 20 steps at full size
+    ref.step(10)                                                # (~25 s per oracle step); 20 steps: smaller boxes
     x1, p1, st = sysg.get_state()
     xr, pr = ref.get_state()
-    assert st == 2
+    assert st == 10
     assert np.abs(x1.cpu().numpy() - xr).max() < XTOL
     assert np.abs(p1.cpu().numpy() - pr).max() < 1e-9 * np.abs(pr).max()
     obs = sysg.observables().cpu().numpy()
@@ -119,4 +119,30 @@ def test_c3_full_size_lists_forces_noise_steps():
     assert st == 1
     assert np.abs(x1.cpu().numpy().reshape(-1)[rows] - ref.x[rows]).max() < XTOL
     sysg.step(3)
+    sysg.check()
+
+
+def test_c3_box_every_dof_segment_end_at_bench_size():
+    """216,000 atoms, adQTB with n_seg = 64 (segment arrays 332 MB instead of 5.3 GB): two whole segments, so
+    that the spectra launch over all 648,000 DOF, the fixed-order reduction of its per-CTA partials and the
+    adaptation run at the size bench.py times; gamma_z to 1e-9 of the oracle's update of the product's own
+    segment arrays (every DOF enters the per-type means)."""
+    import oracle as O
+    cfg = W.CONFIGS["C3"]
+    top = W.water_box(cfg["n_mol"])
+    n_seg, dt, g0 = 64, cfg["dt_fs"] * 1e-3, cfg["gamma0"]
+    sysg, _, x0, p0 = make_pair(top, 1, 1, cfg["dt_fs"], "adqtb", gamma0=g0, n_seg=n_seg, a_gamma=cfg["a_gamma"])
+    otop = O.Topology(top)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    g_prev = np.full((otop.n_types, n_seg + 1), g0)
+    for seg in range(2):
+        sysg.step(n_seg)
+        Fc, v = sysg.adqtb_segment()
+        g = sysg.adqtb_gamma().cpu().numpy()
+        g_ref, _ = oracle_adapt_from_segment(otop, n_seg, dt, g0, cfg["a_gamma"], 0.01, v.cpu().numpy(),
+                                             Fc.cpu().numpy(), g_prev)
+        del Fc, v
+        assert np.abs(g - g_ref).max() < 1e-9 * np.abs(g_ref).max(), seg
+        assert np.abs(g - g_prev).max() > 1e-3
+        g_prev = g
     sysg.check()

@@ -76,3 +76,34 @@ def test_step_count_must_be_a_multiple_of_n_alt():
     sysg.set_respa(1)
     sysg.step(1)
     sysg.check()
+
+
+def test_n_alt_switch_mid_run_matches_oracle():
+    """qhp_set_respa between steps: the pending closing kick of the last outer step must be applied with the
+    n_alt it was taken under (4 -> 1 and 1 -> 4).  The oracle side chains three drivers through their state."""
+    import oracle as O
+    import paper_2212_03137_b200 as qhp
+    top = W.water_box(216)
+    P, Pc, dt = 8, 4, 0.25e-3
+    x0, p0 = W.initial_state(top, P, T_K)
+    sysg = qhp.System(top, P, Pc, dt, T_K, "pile", gamma0=1.0, seed=W.MASTER_SEED)
+    sysg.set_respa(4)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    sysg.step(4)
+    sysg.set_respa(1)
+    sysg.step(4)
+    sysg.set_respa(4)
+    sysg.step(8)
+    x1, p1, st = sysg.get_state()
+    assert st == 16
+    otop = O.Topology(top)
+    x, p, step = x0, p0, 0
+    for n_alt, n in ((4, 4), (1, 4), (4, 8)):
+        ref = O.RpmdRespa(otop, P, Pc, dt, T_K, "pile", 1.0, W.MASTER_SEED, n_alt)
+        ref.set_state(x, p, step)
+        ref.step(n)
+        x, p = ref.get_state()
+        step += n
+    assert np.abs(x1.cpu().numpy() - x).max() < XTOL
+    assert np.abs(p1.cpu().numpy() - p).max() < 1e-6 * np.abs(p).max()
+    sysg.check()

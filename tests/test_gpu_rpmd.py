@@ -160,6 +160,28 @@ def test_skin_smaller_than_bead_spread_is_reported():
         sysg.check()
 
 
+def test_skin_guard_uses_the_norm_of_the_bead_offset():
+    """One bead pair displaced by (d, d, d) with d < skin/2 < sqrt(3) d: every component is inside the bound,
+    the distance is not -- the guard must fire (it compared components)."""
+    import paper_2212_03137_b200 as qhp
+    top = W.water_box(216)
+    top["skin"] = 1.0
+    sysg, _, x0, p0 = make_pair(top, 2, 2, 0.5, "pile", sigma_bead=0.0)
+    x0 = x0.copy()
+    x0[0, 0, :] += 0.4
+    x0[1, 0, :] -= 0.4
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    with pytest.raises(qhp.QhpError):
+        sysg.check()
+    # the same displacement along one axis only stays inside skin/2: accepted
+    sysg2, _, x0, p0 = make_pair(top, 2, 2, 0.5, "pile", sigma_bead=0.0)
+    x0 = x0.copy()
+    x0[0, 0, 0] += 0.4
+    x0[1, 0, 0] -= 0.4
+    sysg2.set_state(to_dev(x0), to_dev(p0), 0)
+    sysg2.check()
+
+
 def test_harmonic_oscillators_single_atom_molecules():
     """Tethered, non-interacting atoms (each its own molecule, no bonds): the harmonic system of the
     closed-form pins; exercises tether forces and ragged tiles."""
