@@ -224,6 +224,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--a-block", choices=["exact", "cayley"], default="exact", help="cayley = BCOCB (PAPER.md:151); exact = the BASELINE.json configs")
     ap.add_argument("--n-alt", type=int, default=1, help="BAOAB-RESPA inner steps per V_s evaluation (PAPER.md Eq. 19); 1 = the BASELINE.json configs")
+    ap.add_argument("--n-mol", type=int, default=0, help="profiling aid: the same workload on a box of this many waters (0 = the BASELINE.json size)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -247,6 +248,8 @@ def main():
         dist.barrier()
 
     cfg = workload(args.workload)
+    if args.n_mol > 0:
+        cfg["n_mol"] = args.n_mol
     top, sysg, x0, p0 = build_system(cfg)
     N, P, K = top["n_atoms"], cfg["P"], args.steps
     xd = torch.as_tensor(x0).cuda()

@@ -46,6 +46,7 @@ struct IntArgs {
   // adQTB (P = 1)
   const double *Fc;
   double *vseg;
+  const int32_t *seg_slot;   // atom -> segment slot (qhp_seg_addr)
   int n_seg, n_loc;
   double qa, qbA;
   // outputs of the auxiliary kernels
@@ -281,7 +282,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
 #pragma unroll
       for (int k = 0; k < PF; ++k) pl[k] = a.Pm[k * a.ND + dof];
     }
-    if (THERMO == 2 && a.do_step) fc_early = a.Fc[(long long)a.n_loc * a.ND + dof];
+    if (THERMO == 2 && a.do_step) fc_early = a.Fc[qhp_seg_addr(a.seg_slot[atom], a.n_seg, a.n_loc) + c];
   }
 
   // ---- phase 1: Q -> bead positions (shared tile), V_f per (molecule, bead) -------------------------
@@ -346,7 +347,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
           p = mc.c1[n] * p + (mc.c2k[n] * sqm) * ft[n * TD + t];
         } else if (THERMO == 2) {
           // classical BAOAB carrying the coloured force (Eq. 12, l.199; readings G14, G16)
-          const long long k = (long long)a.n_loc * a.ND + dof;   // [n_seg][3N]: step-contiguous
+          const long long k = qhp_seg_addr(a.seg_slot[atom], a.n_seg, a.n_loc) + c;
           const double pn = a.qa * p + a.qbA * fc_early;
           a.vseg[k] = (p + pn) / (2.0 * m);
           p = pn;
@@ -458,6 +459,7 @@ __global__ void __launch_bounds__(128) k_integrate_mol1(const IntArgs a, int n_m
       double z[3] = {0.0, 0.0, 0.0};
       if (THERMO == 1 && a.do_step) qhp_normals3(a.seed, (uint32_t)atom, 0u, QHP_TAG_PILE, (uint64_t)a.step, z);
       double dsum = 0.0;
+      const long long segb = THERMO == 2 ? qhp_seg_addr(a.seg_slot[atom], a.n_seg, a.n_loc) : 0;
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         const long long dof = 3LL * atom + c;
@@ -468,7 +470,7 @@ __global__ void __launch_bounds__(128) k_integrate_mol1(const IntArgs a, int n_m
           if (THERMO == 1) {
             p = __ldg(cf + 3) * p + __ldg(cf + 4) * z[c];
           } else if (THERMO == 2) {
-            const long long k = (long long)a.n_loc * a.ND + dof;   // [n_seg][3N]: step-contiguous
+            const long long k = segb + c;
             const double pn = a.qa * p + a.qbA * a.Fc[k];
             a.vseg[k] = (p + pn) / (2.0 * mass);
             p = pn;
@@ -706,7 +708,7 @@ static IntArgs make_args(qhp_system *s) {
   a.tether_k = s->has_tether ? s->dt_.tether_k : nullptr; a.mass = s->dt_.mass;
   a.rank = s->rank; a.pos4 = s->pos4; a.Fs = s->Fs; a.cref = s->cref; a.d2max = s->d2max;
   a.seed = s->th.seed; a.hdt = 0.5 * s->dt; a.w_fast = 1.0; a.w_slow = 1.0;
-  a.Fc = s->Fc; a.vseg = s->vseg; a.n_seg = s->n_seg;
+  a.Fc = s->Fc; a.vseg = s->vseg; a.seg_slot = s->seg_slot; a.n_seg = s->n_seg;
   a.kT = QHP_KB * s->T;
   return a;
 }

@@ -78,7 +78,7 @@ extern "C" int qhp_create(const qhp_topology *top, int P, int P_contract, double
   if (kind == QHP_THERMO_ADQTB) {
     if (P != 1) CREATE_FAIL(QHP_EINVAL, "adQTB requires P = 1");
     const int ns = thermo->n_seg;
-    if (ns < 8 || ns > 1024 || (ns & (ns - 1))) CREATE_FAIL(QHP_EINVAL, "n_seg must be a power of two in [8, 1024]");
+    if (ns < 8 || ns > 2048 || (ns & (ns - 1))) CREATE_FAIL(QHP_EINVAL, "n_seg must be a power of two in [8, 2048]");
   }
   const int N = top->n_atoms, nt = top->n_types;
   for (int i = 0; i < N; ++i) {
@@ -284,7 +284,7 @@ extern "C" int qhp_destroy(qhp_system *s) {
                   d.bond_r0, d.angle_idx, d.angle_k, d.angle_th0, d.mass, d.tether_k, d.tiles, s->Q, s->Pm, s->coef,
                   s->d_Tc, s->pos4, s->Fs, s->cent4, s->cref, s->pair_tab, s->cell_of, s->cell_count, s->cell_start,
                   s->cell_cursor, s->cell_tmp, s->order, s->rank, s->nbr, s->nbr16, s->nbr_count, s->d2max, s->counters,
-                  s->red, s->obs, s->gamma, s->Hf, s->hk, s->H4, s->Fc, s->vseg, s->tw, s->atoms_by_type,
+                  s->red, s->obs, s->gamma, s->Hf, s->hk, s->H4, s->Fc, s->vseg, s->tw, s->seg_slot, s->slot_atom,
                   s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p, s->ratio_tau, s->ratio_avv, s->ratio_avf, s->kappa};
   for (void *p : ptrs) if (p) cudaFree(p);
   delete s;
@@ -589,7 +589,7 @@ extern "C" int qhp_adqtb_kappa(qhp_system *s, const double *kappa) {
 extern "C" int qhp_adqtb_segment(qhp_system *s, double *Fc, double *vseg) {
   if (!s) return QHP_EINVAL;
   if (s->th.kind != QHP_THERMO_ADQTB) { s->err = "not an adQTB system"; return QHP_ESTATE; }
-  // internal layout is [n_seg][3N] (step-contiguous); the hook returns [3N][n_seg]
+  // internal layout: groups of 4 type-sorted atoms, one 96-byte row per step; the hook returns [3N][n_seg]
   int rc = QHP_OK;
   if (Fc) rc = qhp_qtb_export_segment(s, s->Fc, Fc);
   if (!rc && vseg) rc = qhp_qtb_export_segment(s, s->vseg, vseg);
@@ -671,7 +671,7 @@ __global__ void k_twiddle_hook(double2 *tw, int n) {
 }
 
 extern "C" int qhp_fft_c2c(double *data, int n, int64_t batch, int sign, void *cuda_stream) {
-  if (!data || n < 8 || n > 4096 || (n & (n - 1)) || batch < 0 || (sign != 1 && sign != -1)) return QHP_EINVAL;
+  if (!data || n < 8 || n > 8192 || (n & (n - 1)) || batch < 0 || (sign != 1 && sign != -1)) return QHP_EINVAL;
   if (batch == 0) return QHP_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   double2 *tw = nullptr;

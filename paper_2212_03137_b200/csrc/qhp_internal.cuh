@@ -109,11 +109,16 @@ struct qhp_system {
   double *Hf = nullptr;      // [nt][n_seg+1] filter H_z
   double *hk = nullptr;      // [nt][2 n_seg] kernel h_z
   double *H4 = nullptr;      // [nt][4 n_seg][2] spectrum of the zero-padded shifted kernel
-  double *Fc = nullptr, *vseg = nullptr;  // [n_seg][3N] (step-contiguous: the integrator reads/writes one row per step)
+  // segment arrays F_c, v_seg: [n_groups][n_seg][12]: groups of 4 "segment slots" (atoms sorted by type, every
+  // type padded to a multiple of 4), one 96-byte row (4 atoms x 3 components) per step: sector-exact per-step
+  // access for the integrator, one contiguous n_seg x 96 B region per group for the per-segment FFT kernels
+  double *Fc = nullptr, *vseg = nullptr;
+  int32_t *seg_slot = nullptr;    // [N] atom -> segment slot
+  int32_t *slot_atom = nullptr;   // [n_slots] segment slot -> atom (-1: padding)
+  int n_slots = 0;
   double *tw = nullptr;      // twiddles exp(-2 pi i k / NT) [NT][2], NT = 4 n_seg
-  int32_t *atoms_by_type = nullptr; // [N]
   std::vector<int> type_start;     // [nt+1] offsets into atoms_by_type
-  int32_t *spec_cta = nullptr;     // [n_spec_cta][3] (type, begin, end) into atoms_by_type
+  int32_t *spec_cta = nullptr;     // [n_spec_cta][3] (type, first group, end group)
   int n_spec_cta = 0;
   std::vector<int> spec_cta_host;
   double *spec_part = nullptr;     // [n_spec_cta][2][n_seg+1]
@@ -161,7 +166,7 @@ int qhp_pair_partials(const qhp_system *s);          // upper bound of per-CTA e
 int qhp_qtb_init(qhp_system *s);
 int qhp_qtb_generate(qhp_system *s, int64_t seg);
 int qhp_qtb_adapt(qhp_system *s);
-int qhp_qtb_export_segment(qhp_system *s, const double *in, double *out);   // [n_seg][3N] -> [3N][n_seg]
+int qhp_qtb_export_segment(qhp_system *s, const double *in, double *out);   // internal layout -> [3N][n_seg]
 int qhp_fft_launch(double *data, int n, int64_t batch, int sign, const double *tw, int tw_n, cudaStream_t st);
 
 #define QHP_CUDA_OK(s, call)                                                          \
@@ -182,3 +187,8 @@ int qhp_fft_launch(double *data, int n, int64_t batch, int sign, const double *t
     }                                                                                 \
     (s)->n_launch++;                                                                  \
   } while (0)
+
+// address of (segment slot s, component c, step n) in the segment arrays F_c / v_seg
+__host__ __device__ __forceinline__ long long qhp_seg_addr(int slot, int n_seg, int n) {
+  return ((long long)(slot >> 2) * n_seg + n) * 12 + (slot & 3) * 3;
+}

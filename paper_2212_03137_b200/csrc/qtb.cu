@@ -16,6 +16,14 @@
 // ---------------------------------------------------------------------------------------------
 // FFT
 // ---------------------------------------------------------------------------------------------
+// Shared-memory FFT buffers are swizzled: element i lives at FPAD(i) = i ^ (((i >> 3) ^ (i >> 6)) & 7).  The first
+// pass of a transform stores R consecutive elements per thread, i.e. at a lane stride of 16 R bytes (256 B for
+// radix 16), which unswizzled is an 8-way bank conflict on every store (measured: half of all shared-memory
+// wavefronts of the segment kernels); the XOR of the 16-byte bank-group index with bits 3-5 and 6-8 of the
+// element index makes the stores of lane strides 2, 4, 8 and 16 elements conflict-free and leaves runs of 8
+// consecutive elements (all other accesses) inside one aligned 128-byte row.  No extra memory.
+#define FPAD(i) ((i) ^ ((((i) >> 3) ^ ((i) >> 6)) & 7))
+#define FPAD_LEN(n) (n)
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
   return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
@@ -43,7 +51,8 @@ __device__ __forceinline__ void dft4(double2 &a, double2 &b, double2 &c, double2
 // version of the noise kernel), or 4 radix-4 / 8 radix-2 butterflies.  Reads are contiguous in t.
 // Input twiddles w^(k u) are successive powers of one table entry w^k (<= 15 products, ~1e-14 relative).
 template <int R, int SG>
-__device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const double2 *__restrict__ tw, int tw_n, int t) {
+__device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const double2 *__restrict__ tw, int tw_n, int t,
+                                         const double2 wpre = make_double2(0.0, 0.0), bool have_w = false) {
   constexpr int G = 16 / R;                       // butterflies per thread
   const int nth = n >= 16 ? n >> 4 : 1, nb = n / R;
   const bool on = t < nth;
@@ -57,9 +66,9 @@ __device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const doub
       if (j < nb) {
         const int k = j & (Ns - 1);
 #pragma unroll
-        for (int u = 0; u < R; ++u) v[q * R + u] = buf[j + u * nb];
+        for (int u = 0; u < R; ++u) v[q * R + u] = buf[FPAD(j + u * nb)];
         if (k) {
-          const double2 w1 = twiddle(tw, tw_n, k, Ns * R, SG);
+          const double2 w1 = have_w ? wpre : twiddle(tw, tw_n, k, Ns * R, SG);
           double2 w = w1;
 #pragma unroll
           for (int u = 1; u < R; ++u) {
@@ -95,7 +104,7 @@ __device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const doub
 #pragma unroll
         for (int c = 0; c < 4; ++c)
 #pragma unroll
-          for (int d = 0; d < 4; ++d) buf[j0[0] + (c + 4 * d) * Ns] = v[4 * c + d];
+          for (int d = 0; d < 4; ++d) buf[FPAD(j0[0] + (c + 4 * d) * Ns)] = v[4 * c + d];
       }
     } else {
 #pragma unroll
@@ -104,11 +113,11 @@ __device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const doub
           if (R == 4) {
             dft4<SG>(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
 #pragma unroll
-            for (int u = 0; u < 4; ++u) buf[j0[q] + u * Ns] = v[4 * q + u];
+            for (int u = 0; u < 4; ++u) buf[FPAD(j0[q] + u * Ns)] = v[4 * q + u];
           } else {
             const double2 x0 = v[2 * q], x1 = v[2 * q + 1];
-            buf[j0[q]] = make_double2(x0.x + x1.x, x0.y + x1.y);
-            buf[j0[q] + Ns] = make_double2(x0.x - x1.x, x0.y - x1.y);
+            buf[FPAD(j0[q])] = make_double2(x0.x + x1.x, x0.y + x1.y);
+            buf[FPAD(j0[q] + Ns)] = make_double2(x0.x - x1.x, x0.y - x1.y);
           }
         }
     }
@@ -118,12 +127,31 @@ __device__ __forceinline__ void fft_pass(double2 *buf, int n, int Ns, const doub
 
 // In-place Stockham FFT of buf[0..n) by blockDim.x >= max(n/16, 1) threads (all threads of the CTA
 // must call).  sign = -1 forward, +1 inverse (unnormalised).  Result in natural order.
+// Radix schedule: the factor of n that is not a power of 16 goes FIRST (radix-2 / radix-4 passes at small Ns need
+// at most a handful of twiddles), then radix-16 passes; the one table entry w^k a thread needs in each radix-16
+// pass is requested before the first pass, so that no pass waits on a global load.
 template <int SG>
 __device__ __forceinline__ void fft_smem_sg(double2 *buf, int n, const double2 *__restrict__ tw, int tw_n, int t) {
+  int r0 = n, m16 = 0;
+  while (r0 >= 16 && (r0 & 15) == 0) { r0 >>= 4; ++m16; }            // n = r0 * 16^m16, r0 in {1, 2, 4, 8}
+  double2 w16[3] = {make_double2(1.0, 0.0), make_double2(1.0, 0.0), make_double2(1.0, 0.0)};
+  {
+    int Ns = r0;
+#pragma unroll
+    for (int p = 0; p < 3; ++p)
+      if (p < m16) {
+        const int k = t & (Ns - 1);
+        if (t < (n >> 4)) w16[p] = twiddle(tw, tw_n, k, Ns * 16, SG);
+        Ns <<= 4;
+      }
+  }
   int Ns = 1;
-  while (n / Ns >= 16 && ((n / Ns) & 15) == 0) { fft_pass<16, SG>(buf, n, Ns, tw, tw_n, t); Ns <<= 4; }
-  while (((n / Ns) & 3) == 0 && Ns < n) { fft_pass<4, SG>(buf, n, Ns, tw, tw_n, t); Ns <<= 2; }
-  while (Ns < n) { fft_pass<2, SG>(buf, n, Ns, tw, tw_n, t); Ns <<= 1; }
+  if (r0 == 2) { fft_pass<2, SG>(buf, n, 1, tw, tw_n, t); Ns = 2; }
+  else if (r0 == 4) { fft_pass<4, SG>(buf, n, 1, tw, tw_n, t); Ns = 4; }
+  else if (r0 == 8) { fft_pass<2, SG>(buf, n, 1, tw, tw_n, t); fft_pass<4, SG>(buf, n, 2, tw, tw_n, t); Ns = 8; }
+#pragma unroll
+  for (int p = 0; p < 3; ++p)
+    if (p < m16) { fft_pass<16, SG>(buf, n, Ns, tw, tw_n, t, w16[p], true); Ns <<= 4; }
 }
 // t: index of the calling thread inside its FFT (threads t >= max(n/16, 1) only take part in the barriers);
 // several FFTs of the same length can run side by side in one CTA on different buffers.
@@ -140,19 +168,19 @@ __global__ void k_twiddle(double2 *tw, int n) {
   tw[m] = make_double2(c, s);
 }
 
-__global__ void __launch_bounds__(512) k_fft_batch(double2 *data, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
+__global__ void __launch_bounds__(512, 1) k_fft_batch(double2 *data, int n, int sign, const double2 *__restrict__ tw, int tw_n) {
   extern __shared__ double2 fbuf[];
   double2 *d = data + (long long)blockIdx.x * n;
-  for (int k = threadIdx.x; k < n; k += blockDim.x) fbuf[k] = d[k];
+  for (int k = threadIdx.x; k < n; k += blockDim.x) fbuf[FPAD(k)] = d[k];
   __syncthreads();
   fft_smem(fbuf, n, sign, tw, tw_n, threadIdx.x);
-  for (int k = threadIdx.x; k < n; k += blockDim.x) d[k] = fbuf[k];
+  for (int k = threadIdx.x; k < n; k += blockDim.x) d[k] = fbuf[FPAD(k)];
 }
 
 static int fft_threads(int n) { return n / 16 < 32 ? 32 : n / 16; }
 
 int qhp_fft_launch(double *data, int n, int64_t batch, int sign, const double *tw, int tw_n, cudaStream_t st) {
-  const size_t smem = sizeof(double2) * (size_t)n;
+  const size_t smem = sizeof(double2) * (size_t)FPAD_LEN(n);
   cudaError_t e = cudaFuncSetAttribute(k_fft_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return QHP_ECUDA;
   k_fft_batch<<<(unsigned)batch, fft_threads(n), smem, st>>>((double2 *)data, n, sign, (const double2 *)tw, tw_n);
@@ -217,108 +245,126 @@ __global__ void k_qtb_spectrum4(int nt, int n_seg, const double *__restrict__ hk
   H4[idx] = make_double2(re, im);
 }
 
-// ---------------------------------------------------------------------------------------------
-// Q2 + Q4: one CTA per atom.  (x, y) white noise of the atom go through one complex FFT (the
-// kernel h is real, so real and imaginary parts are filtered independently), z through a second.
-//   F_c[dof][n] = sum_k h_z[k] r(dof, seg*n_seg + n - k + n_seg),  n = 0..n_seg-1
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256, 2) k_qtb_noise(int n_seg, long long ND, unsigned long long seed, long long seg, const int32_t *__restrict__ type,
-                            const double2 *__restrict__ H4, const double2 *__restrict__ tw, double *Fc) {
-  extern __shared__ double2 nbuf[];
-  const int nf = 4 * n_seg, nw = 3 * n_seg;
-  double *zb = reinterpret_cast<double *>(nbuf + nf);
-  const int atom = blockIdx.x, t = threadIdx.x;
-  const double2 *Hz = H4 + (long long)type[atom] * nf;
-  for (int m = t; m < nf; m += blockDim.x) {
+// white noise of one pass of k_qtb_noise into the transform buffer (own function: the constants of the
+// Box-Muller evaluation must not stay live across the transforms, which need every register)
+__device__ __noinline__ void qtb_fill_noise(double2 *nbuf, double *zb, int nf, int nw, int n_seg, int pass, int atom,
+                                            unsigned long long seed, long long seg, int t, int nthr) {
+  for (int m = t; m < nf; m += nthr) {
+    double2 v = make_double2(0.0, 0.0);
     if (m < nw) {
-      double z[3];
-      qhp_normals3(seed, (uint32_t)atom, 0u, QHP_TAG_QTB, (uint64_t)(seg * n_seg + m), z);
-      nbuf[m] = make_double2(z[0], z[1]);
-      zb[m] = z[2];
-    } else {
-      nbuf[m] = make_double2(0.0, 0.0);
-    }
-  }
-  const double inv = 1.0 / (double)nf;
-  double fx[4] = {0.0, 0.0, 0.0, 0.0}, fy[4] = {0.0, 0.0, 0.0, 0.0};   // 4 blockDim.x >= n_seg: samples n = t + u blockDim.x
-  for (int pass = 0; pass < 2; ++pass) {
-    __syncthreads();
-    fft_smem(nbuf, nf, -1, tw, nf, t);
-    for (int q = t; q < nf; q += blockDim.x) nbuf[q] = cmul(nbuf[q], Hz[q]);
-    __syncthreads();
-    fft_smem(nbuf, nf, +1, tw, nf, t);
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int n = t + u * blockDim.x;
-      if (n < n_seg) {
-        const double2 y = nbuf[n + 2 * n_seg];
-        if (pass == 0) { fx[u] = y.x * inv; fy[u] = y.y * inv; }
-        else {
-          // Fc[n][dof] (step-contiguous for the integrator): the three components of one sample together
-          double *out = Fc + (long long)n * ND + 3LL * atom;
-          out[0] = fx[u]; out[1] = fy[u]; out[2] = y.x * inv;
-        }
+      if (pass < 2) {
+        double z[3] = {0.0, 0.0, 0.0};
+        if (atom >= 0) qhp_normals3(seed, (uint32_t)atom, 0u, QHP_TAG_QTB, (uint64_t)(seg * n_seg + m), z);
+        v = make_double2(z[0], z[1]);
+        zb[pass * nw + m] = z[2];
+      } else {
+        v = make_double2(zb[m], zb[nw + m]);
       }
     }
-    if (pass == 0) {
-      __syncthreads();
-      for (int m = t; m < nf; m += blockDim.x) nbuf[m] = make_double2(m < nw ? zb[m] : 0.0, 0.0);
-    }
+    nbuf[FPAD(m)] = v;
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// Q5 + Q6: spectra.  One CTA walks a run of atoms of one type; v and F_c of a DOF are the real and
-// imaginary part of one zero-padded N_k-point transform.  Per-CTA sums -> fixed-order reduction.
+// Q2 + Q4: one CTA per PAIR of segment slots (two atoms of one type, qhp_internal.cuh).  The kernel h is
+// real, so real and imaginary part of a complex sequence are filtered independently: (x0, y0), (x1, y1)
+// and (z0, z1) are three complex transforms for six components (the z components of two atoms share one).
+//   F_c[dof][n] = sum_k h_z[k] r(dof, seg*n_seg + n - k + n_seg),  n = 0..n_seg-1
+// Output: the 48-byte half row of the pair in the segment layout [group][n_seg][12].
 // ---------------------------------------------------------------------------------------------
-// One CTA = 3 groups of max(n_k/16, 32) threads; group c transforms DOF c of the current atom (v and
-// F_c as real and imaginary part of one zero-padded n_k-point FFT).  Every thread accumulates its own
-// frequency bins in registers over all atoms of the CTA's run; the three groups are combined once at
-// the end in a fixed order.  SPEC_BINS bounds (n_seg + 1) / group size (n_seg <= 1024: 1025 / 128).
-#define SPEC_BINS 9
-__global__ void __launch_bounds__(384, 2) k_qtb_spectra(int n_seg, long long ND, const int32_t *__restrict__ cta_tab, const int32_t *__restrict__ atoms,
-                              const double *__restrict__ vseg, const double *__restrict__ Fc,
-                              const double2 *__restrict__ tw, int tw_n, double *part) {
-  extern __shared__ double2 sbuf_all[];
-  const int nk = 2 * n_seg, nf = n_seg + 1, gsz = blockDim.x / 3;
-  const int c = threadIdx.x / gsz, t = threadIdx.x - c * gsz;
-  double2 *sbuf = sbuf_all + (size_t)c * nk;
-  double avv[SPEC_BINS], avf[SPEC_BINS];
-#pragma unroll
-  for (int m = 0; m < SPEC_BINS; ++m) { avv[m] = 0.0; avf[m] = 0.0; }
-  const int b = cta_tab[3 * blockIdx.x + 1], e = cta_tab[3 * blockIdx.x + 2];
-  for (int ia = b; ia < e; ++ia) {
-    const long long d = 3LL * atoms[ia] + c;
-    for (int n = t; n < nk; n += gsz)
-      sbuf[n] = (n < n_seg) ? make_double2(vseg[(long long)n * ND + d], Fc[(long long)n * ND + d]) : make_double2(0.0, 0.0);
+__global__ void __launch_bounds__(512, 1) k_qtb_noise(int n_seg, unsigned long long seed, long long seg, const int32_t *__restrict__ slot_atom,
+                                                   const int32_t *__restrict__ type, const double2 *__restrict__ H4,
+                                                   const double2 *__restrict__ tw, double *Fc) {
+  extern __shared__ double2 nbuf[];
+  const int nf = 4 * n_seg, nw = 3 * n_seg;
+  double *zb = reinterpret_cast<double *>(nbuf + FPAD_LEN(nf)); // [2][nw] z noise of the two atoms
+  const int slot0 = 2 * blockIdx.x, t = threadIdx.x;
+  const int at[2] = {slot_atom[slot0], slot_atom[slot0 + 1]};
+  if (at[0] < 0 && at[1] < 0) return;                           // padding
+  const double2 *Hz = H4 + (long long)type[at[0] >= 0 ? at[0] : at[1]] * nf;
+  const double inv = 1.0 / (double)nf;
+  for (int pass = 0; pass < 3; ++pass) {
+    qtb_fill_noise(nbuf, zb, nf, nw, n_seg, pass, pass < 2 ? at[pass] : -1, seed, seg, t, blockDim.x);
     __syncthreads();
-    fft_smem(sbuf, nk, -1, tw, tw_n, t);
-#pragma unroll
-    for (int m = 0; m < SPEC_BINS; ++m) {
-      const int j = t + m * gsz;
-      if (j < nf) {
-        const double2 A = sbuf[j], Zm = sbuf[(nk - j) & (nk - 1)];
-        const double vx = 0.5 * (A.x + Zm.x), vy = 0.5 * (A.y - Zm.y);     // V_j
-        const double px = 0.5 * (A.y + Zm.y), py = -0.5 * (A.x - Zm.x);    // Phi_j
-        avv[m] += vx * vx + vy * vy;
-        avf[m] += vx * px + vy * py;
-      }
+    fft_smem(nbuf, nf, -1, tw, nf, t);
+    // inverse transform = conj(forward(conj(.))): one transform direction in this kernel
+#pragma unroll 8
+    for (int q = t; q < nf; q += blockDim.x) {
+      const double2 p = cmul(nbuf[FPAD(q)], Hz[q]);
+      nbuf[FPAD(q)] = make_double2(p.x, -p.y);
+    }
+    __syncthreads();
+    fft_smem(nbuf, nf, -1, tw, nf, t);
+    // every pass writes its own pieces of the pair's 48-byte half rows (x0 y0 z0 x1 y1 z1); L2 merges them
+    for (int n = t; n < n_seg; n += blockDim.x) {
+      double2 y = nbuf[FPAD(n + 2 * n_seg)];
+      y.y = -y.y;
+      double *out = Fc + qhp_seg_addr(slot0, n_seg, n);
+      if (pass == 0) *reinterpret_cast<double2 *>(out) = make_double2(y.x * inv, y.y * inv);
+      else if (pass == 1) { out[3] = y.x * inv; out[4] = y.y * inv; }
+      else { out[2] = y.x * inv; out[5] = y.y * inv; }
     }
     __syncthreads();
   }
-  // combine the three groups: (x + y) + z per bin
-  double *red = reinterpret_cast<double *>(sbuf_all);          // [3][2][nf]
-#pragma unroll
-  for (int m = 0; m < SPEC_BINS; ++m) {
-    const int j = t + m * gsz;
-    if (j < nf) { red[(c * 2) * nf + j] = avv[m]; red[(c * 2 + 1) * nf + j] = avf[m]; }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Q5 + Q6: spectra.  One CTA walks a run of slot groups (4 atoms, 12 DOF) of one type; v and F_c of a DOF
+// are the real and imaginary part of one zero-padded N_k-point transform.  A group is one contiguous
+// n_seg x 96 B region of each segment array, read with coalesced loads; DPR of its 12 DOFs are transformed
+// side by side per round (DPR thread groups of max(N_k/16, 32) threads).  The bins are accumulated in one
+// shared array per CTA, the thread groups adding in a fixed order; per-CTA sums -> fixed-order reduction.
+// ---------------------------------------------------------------------------------------------
+template <int DPR>
+__global__ void __launch_bounds__(512, 1) k_qtb_spectra(int n_seg, const int32_t *__restrict__ cta_tab,
+                                                        const double *__restrict__ vseg, const double *__restrict__ Fc,
+                                                        const double2 *__restrict__ tw, int tw_n, double *part) {
+  extern __shared__ double2 sbuf_all[];
+  const int nk = 2 * n_seg, nf = n_seg + 1, gsz = blockDim.x / DPR, bl = nk + 1;   // + 1: the DOF buffers start one bank group apart
+  const int c = threadIdx.x / gsz, t = threadIdx.x - c * gsz;
+  double *acc = reinterpret_cast<double *>(sbuf_all + (size_t)2 * DPR * bl);   // [2][nf]
+  for (int j = threadIdx.x; j < 2 * nf; j += blockDim.x) acc[j] = 0.0;
+  const int gb = cta_tab[3 * blockIdx.x + 1], ge = cta_tab[3 * blockIdx.x + 2];
+  constexpr int RPG = 12 / DPR;                          // rounds per group
+  const int rounds = (ge - gb) * RPG;
+  // round q of the CTA: DOFs [r DPR, (r + 1) DPR) of group g; its (v, F_c) samples go straight from global to
+  // shared memory (cp.async, 8 bytes each) while the previous round is being transformed (two buffers)
+  auto issue = [&](int q, double2 *buf) {
+    const int g = gb + q / RPG, r = q - (q / RPG) * RPG;
+    const double *vg = vseg + (long long)g * n_seg * 12 + r * DPR, *fg = Fc + (long long)g * n_seg * 12 + r * DPR;
+    for (int idx = threadIdx.x; idx < n_seg * DPR; idx += blockDim.x) {
+      const int n = idx / DPR, d = idx - n * DPR;
+      double2 *dst = buf + (size_t)d * bl + FPAD(n);
+      const uint32_t sa = (uint32_t)__cvta_generic_to_shared(dst);
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(vg + (long long)n * 12 + d) : "memory");
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa + 8), "l"(fg + (long long)n * 12 + d) : "memory");
+      buf[(size_t)d * bl + FPAD(n_seg + n)] = make_double2(0.0, 0.0);      // zero padding to N_k
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  if (rounds > 0) issue(0, sbuf_all);
+  for (int q = 0; q < rounds; ++q) {
+    double2 *cur = sbuf_all + (size_t)(q & 1) * DPR * bl, *nxt = sbuf_all + (size_t)((q + 1) & 1) * DPR * bl;
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+    if (q + 1 < rounds) issue(q + 1, nxt);
+    double2 *sbuf = cur + (size_t)c * bl;
+    fft_smem(sbuf, nk, -1, tw, tw_n, t);
+    for (int cc = 0; cc < DPR; ++cc) {                   // the thread groups add in a fixed order
+      if (c == cc)
+        for (int j = t; j < nf; j += gsz) {
+          const double2 A = sbuf[FPAD(j)], Zm = sbuf[FPAD((nk - j) & (nk - 1))];
+          const double vx = 0.5 * (A.x + Zm.x), vy = 0.5 * (A.y - Zm.y);     // V_j
+          const double px = 0.5 * (A.y + Zm.y), py = -0.5 * (A.x - Zm.x);    // Phi_j
+          acc[j] += vx * vx + vy * vy;
+          acc[nf + j] += vx * px + vy * py;
+        }
+      __syncthreads();
+    }
   }
   __syncthreads();
   double *o = part + (long long)blockIdx.x * 2 * nf;
-  for (int j = threadIdx.x; j < nf; j += blockDim.x) {
-    o[j] = (red[j] + red[2 * nf + j]) + red[4 * nf + j];
-    o[nf + j] = (red[nf + j] + red[3 * nf + j]) + red[5 * nf + j];
-  }
+  for (int j = threadIdx.x; j < 2 * nf; j += blockDim.x) o[j] = acc[j];
 }
 
 __global__ void k_qtb_reduce(int nt, int n_seg, int n_cta, const int32_t *__restrict__ cta_tab, const double *__restrict__ part,
@@ -394,28 +440,26 @@ __global__ void k_qtb_adapt_ratio(int nt, int n_seg, const double *__restrict__ 
   }
 }
 
-// parity hook: internal [n_seg][3N] -> documented [3N][n_seg]
-__global__ void k_seg_transpose(const double *__restrict__ in, double *__restrict__ out, long long ND, int n_seg) {
-  __shared__ double tile[32][33];
-  const long long d0 = (long long)blockIdx.x * 32;
-  const int n0 = blockIdx.y * 32;
-  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-    const long long d = d0 + threadIdx.x;
-    const int n = n0 + r;
-    tile[r][threadIdx.x] = (d < ND && n < n_seg) ? in[n * ND + d] : 0.0;
+// parity hook: internal [group][n_seg][12] -> documented [3N][n_seg] (atom order)
+__global__ void k_seg_export(const double *__restrict__ in, double *__restrict__ out, const int32_t *__restrict__ slot_atom,
+                             int n_seg) {
+  __shared__ double tile[12][65];
+  const int g = blockIdx.x, n0 = blockIdx.y * 64;
+  for (int idx = threadIdx.x; idx < 64 * 12; idx += blockDim.x) {
+    const int k = idx / 12, d = idx - k * 12;
+    if (n0 + k < n_seg) tile[d][k] = in[((long long)g * n_seg + n0 + k) * 12 + d];
   }
   __syncthreads();
-  for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-    const long long d = d0 + r;
-    const int n = n0 + threadIdx.x;
-    if (d < ND && n < n_seg) out[d * n_seg + n] = tile[threadIdx.x][r];
+  for (int idx = threadIdx.x; idx < 64 * 12; idx += blockDim.x) {
+    const int d = idx / 64, k = idx - d * 64;
+    const int at = slot_atom[4 * g + d / 3];
+    if (at >= 0 && n0 + k < n_seg) out[(3LL * at + d % 3) * n_seg + n0 + k] = tile[d][k];
   }
 }
 
 int qhp_qtb_export_segment(qhp_system *s, const double *in, double *out) {
-  const long long ND = 3LL * s->N;
-  const dim3 grid((unsigned)((ND + 31) / 32), (unsigned)((s->n_seg + 31) / 32)), block(32, 8);
-  k_seg_transpose<<<grid, block, 0, s->stream>>>(in, out, ND, s->n_seg);
+  const dim3 grid((unsigned)(s->n_slots / 4), (unsigned)((s->n_seg + 63) / 64));
+  k_seg_export<<<grid, 256, 0, s->stream>>>(in, out, s->slot_atom, s->n_seg);
   QHP_LAUNCH_OK(s);
   return QHP_OK;
 }
@@ -430,7 +474,6 @@ __global__ void k_fill(double *p, long long n, double v) {
 // ---------------------------------------------------------------------------------------------
 int qhp_qtb_init(qhp_system *s) {
   const int ns = s->n_seg, nf = ns + 1, nt = s->nt, N = s->N;
-  const size_t seg_bytes = sizeof(double) * 3 * (size_t)N * ns;
   QHP_CUDA_OK(s, cudaMalloc(&s->gamma, sizeof(double) * nt * nf));
   QHP_CUDA_OK(s, cudaMalloc(&s->Hf, sizeof(double) * nt * nf));
   QHP_CUDA_OK(s, cudaMalloc(&s->hk, sizeof(double) * nt * 2 * ns));
@@ -438,6 +481,26 @@ int qhp_qtb_init(qhp_system *s) {
   QHP_CUDA_OK(s, cudaMalloc(&s->Cvv, sizeof(double) * nt * nf));
   QHP_CUDA_OK(s, cudaMalloc(&s->CvF, sizeof(double) * nt * nf));
   QHP_CUDA_OK(s, cudaMalloc(&s->tw, sizeof(double) * 2 * 4 * ns));
+  // segment slots: atoms sorted by type, every type padded to whole groups of 4 slots
+  std::vector<int32_t> type_host(N), seg_slot(N), slot_atom;
+  QHP_CUDA_OK(s, cudaMemcpy(type_host.data(), s->dt_.type, sizeof(int32_t) * N, cudaMemcpyDeviceToHost));
+  s->type_start.assign(nt + 1, 0);
+  std::vector<double> ndof(nt);
+  for (int z = 0; z < nt; ++z) {
+    s->type_start[z] = (int)slot_atom.size();
+    int cnt = 0;
+    for (int a = 0; a < N; ++a)
+      if (type_host[a] == z) { seg_slot[a] = (int32_t)slot_atom.size(); slot_atom.push_back(a); ++cnt; }
+    while (slot_atom.size() % 4) slot_atom.push_back(-1);
+    ndof[z] = 3.0 * cnt;
+  }
+  s->type_start[nt] = (int)slot_atom.size();
+  s->n_slots = (int)slot_atom.size();
+  QHP_CUDA_OK(s, cudaMalloc(&s->seg_slot, sizeof(int32_t) * N));
+  QHP_CUDA_OK(s, cudaMemcpy(s->seg_slot, seg_slot.data(), sizeof(int32_t) * N, cudaMemcpyHostToDevice));
+  QHP_CUDA_OK(s, cudaMalloc(&s->slot_atom, sizeof(int32_t) * slot_atom.size()));
+  QHP_CUDA_OK(s, cudaMemcpy(s->slot_atom, slot_atom.data(), sizeof(int32_t) * slot_atom.size(), cudaMemcpyHostToDevice));
+  const size_t seg_bytes = sizeof(double) * 3 * (size_t)s->n_slots * ns;
   if (cudaMalloc(&s->Fc, seg_bytes) != cudaSuccess || cudaMalloc(&s->vseg, seg_bytes) != cudaSuccess) {
     s->err = "adQTB segment buffers: out of device memory";
     return QHP_ENOMEM;
@@ -448,29 +511,19 @@ int qhp_qtb_init(qhp_system *s) {
   QHP_LAUNCH_OK(s);
   k_fill<<<(nt * nf + 255) / 256, 256, 0, s->stream>>>(s->gamma, (long long)nt * nf, s->th.gamma0);
   QHP_LAUNCH_OK(s);
-  // atoms grouped by type; spectra CTAs walk runs of <= chunk atoms of one type
-  std::vector<int32_t> by_type, type_host(N);
-  QHP_CUDA_OK(s, cudaMemcpy(type_host.data(), s->dt_.type, sizeof(int32_t) * N, cudaMemcpyDeviceToHost));
-  s->type_start.assign(nt + 1, 0);
-  for (int z = 0; z < nt; ++z) {
-    s->type_start[z] = (int)by_type.size();
-    for (int a = 0; a < N; ++a) if (type_host[a] == z) by_type.push_back(a);
-  }
-  s->type_start[nt] = (int)by_type.size();
-  int chunk = (N + 148 * 4 - 1) / (148 * 4);
+  // spectra CTAs walk runs of <= chunk slot groups of one type: about two CTAs per SM in all
+  int sms = 148;
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device);
+  const int n_groups = s->n_slots / 4;
+  int chunk = (n_groups + 2 * sms - 1) / (2 * sms);
   if (chunk < 1) chunk = 1;
   std::vector<int32_t> tab;
-  std::vector<double> ndof(nt);
-  for (int z = 0; z < nt; ++z) {
-    ndof[z] = 3.0 * (s->type_start[z + 1] - s->type_start[z]);
-    for (int b = s->type_start[z]; b < s->type_start[z + 1]; b += chunk) {
-      tab.push_back(z); tab.push_back(b); tab.push_back(std::min(b + chunk, s->type_start[z + 1]));
+  for (int z = 0; z < nt; ++z)
+    for (int b = s->type_start[z] / 4; b < s->type_start[z + 1] / 4; b += chunk) {
+      tab.push_back(z); tab.push_back(b); tab.push_back(std::min(b + chunk, s->type_start[z + 1] / 4));
     }
-  }
   s->n_spec_cta = (int)tab.size() / 3;
-  QHP_CUDA_OK(s, cudaMalloc(&s->atoms_by_type, sizeof(int32_t) * N));
-  QHP_CUDA_OK(s, cudaMemcpy(s->atoms_by_type, by_type.data(), sizeof(int32_t) * N, cudaMemcpyHostToDevice));
-  QHP_CUDA_OK(s, cudaMalloc(&s->spec_cta, sizeof(int32_t) * tab.size()));
+  QHP_CUDA_OK(s, cudaMalloc(&s->spec_cta, sizeof(int32_t) * std::max<size_t>(tab.size(), 1)));
   QHP_CUDA_OK(s, cudaMemcpy(s->spec_cta, tab.data(), sizeof(int32_t) * tab.size(), cudaMemcpyHostToDevice));
   QHP_CUDA_OK(s, cudaMalloc(&s->spec_part, sizeof(double) * (size_t)s->n_spec_cta * 2 * nf + sizeof(double) * nt));
   // per-type DOF counts live behind the partials
@@ -488,10 +541,10 @@ int qhp_qtb_generate(qhp_system *s, int64_t seg) {
   k_qtb_spectrum4<<<(nt * 4 * ns + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->hk, (double2 *)s->H4);
   QHP_LAUNCH_OK(s);
   const int n4 = 4 * ns;
-  const size_t smem = sizeof(double2) * n4 + sizeof(double) * 3 * ns;
+  const size_t smem = sizeof(double2) * FPAD_LEN(n4) + sizeof(double) * 2 * 3 * ns;
   QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_noise, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_qtb_noise<<<s->N, fft_threads(n4), smem, s->stream>>>(ns, 3LL * s->N, s->th.seed, seg, s->dt_.type, (const double2 *)s->H4,
-                                                         (const double2 *)s->tw, s->Fc);
+  k_qtb_noise<<<s->n_slots / 2, fft_threads(n4), smem, s->stream>>>(ns, s->th.seed, seg, s->slot_atom, s->dt_.type, (const double2 *)s->H4,
+                                                                   (const double2 *)s->tw, s->Fc);
   QHP_LAUNCH_OK(s);
   s->fc_segment = seg;
   return QHP_OK;
@@ -500,10 +553,17 @@ int qhp_qtb_generate(qhp_system *s, int64_t seg) {
 // Q5-Q7 at the end of a segment
 int qhp_qtb_adapt(qhp_system *s) {
   const int ns = s->n_seg, nf = ns + 1, nt = s->nt, nk = 2 * ns;
-  const size_t smem = sizeof(double2) * 3 * nk;
-  QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_spectra, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_qtb_spectra<<<s->n_spec_cta, 3 * fft_threads(nk), smem, s->stream>>>(ns, 3LL * s->N, s->spec_cta, s->atoms_by_type, s->vseg, s->Fc,
-                                                                        (const double2 *)s->tw, 4 * ns, s->spec_part);
+  // DOFs transformed side by side: 3 (n_seg <= 1024: 384 threads), else 1 (256 threads); every kernel that calls
+  // the shared-memory FFT keeps <= 512 threads per CTA so that the radix-16 butterflies stay in registers
+  const int dpr = ns <= 1024 ? 3 : 1;
+  const size_t smem = sizeof(double2) * 2 * dpr * (nk + 1) + sizeof(double) * 2 * nf;      // two buffers
+  if (dpr == 3) {
+    QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_spectra<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_qtb_spectra<3><<<s->n_spec_cta, 3 * fft_threads(nk), smem, s->stream>>>(ns, s->spec_cta, s->vseg, s->Fc, (const double2 *)s->tw, 4 * ns, s->spec_part);
+  } else {
+    QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_spectra<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_qtb_spectra<1><<<s->n_spec_cta, fft_threads(nk), smem, s->stream>>>(ns, s->spec_cta, s->vseg, s->Fc, (const double2 *)s->tw, 4 * ns, s->spec_part);
+  }
   QHP_LAUNCH_OK(s);
   k_qtb_reduce<<<(nt * nf + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->n_spec_cta, s->spec_cta, s->spec_part,
                                                            s->spec_part + (size_t)s->n_spec_cta * 2 * nf, s->dt, s->Cvv, s->CvF);
