@@ -7,7 +7,9 @@ A "step" is one pass of the whole hot path (SURVEY.md §8(a) rows R1-R12 for RPM
 over the synthetic water box of the chosen BASELINE.json config: one `qhp_step(1)`.
 Default workload C4 = configs[4]: 72,000 waters (216,000 atoms), P = 32 beads, P' = 4 contracted
 beads, dt = 0.25 fs, PILE -- the configuration BASELINE.json's metric (bead-atom-steps/s and ns/day at
-216k atoms) is quoted on.  `--workload C3` times the 216k-atom adQTB configuration.
+216k atoms) is quoted on.  The default run appends an adQTB leg (`adqtb`: C3 = configs[3], 216,000 atoms,
+one whole 1024-step segment with noise generation and adaptation), so that one run measures both halves of
+the metric; `--workload C3` times that configuration alone.
 
 * value     = N_gpus * n_atoms * P * K / (max over ranks of the device time of K steps), state
               resident in HBM.
@@ -17,8 +19,10 @@ beads, dt = 0.25 fs, PILE -- the configuration BASELINE.json's metric (bead-atom
 * roofline  = the dominant kernel (pair forces, FP64-ALU bound): algorithmic flops per launch /
               its average device time, measured with CUDA events recorded by the library on its
               stream around every launch inside the timed region (qhp_profile).
-* cpu_baseline = the oracle (oracle/, plain C, one thread) timed on this box's host on one step of
-              the same workload.
+* kernels   = the same for every hot kernel: {ms, algorithmic units, achieved, peak, frac}; the list-rebuild
+              chain also carries its amortised cost from an untimed 500-step continuation.
+* cpu_baseline = the oracle (oracle/, plain C, one thread) timed on this box's host on 5 steps of a
+              bounded sample (4096 waters) of the same workload.
 N > 1 (torchrun): the path does not shard in this round ("replicas only"): every rank
 runs an independent replica of the workload on its own GPU; barrier + max-over-ranks timing.
 """
@@ -46,10 +50,11 @@ FLOP_PER_PAIR_BEAD = 110.0
 # FP64 ALU peak derived from unit counts: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (max SM clock);
 # bench.py also measures it live with qhp_dfma_probe and reports both.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_staged<false> launch at C4, from the
-# `ncu --set full` capture summarised in profiles/r1c_summary.md (per launch, like `achieved`)
-NCU_TRAFFIC_BYTES = {("C4", "k_pair_staged"): 1.3637e9 + 2.39e7,      # profiles/r1d_summary.md (dram read + write per launch)
-                     ("C3", "k_pair_staged"): 3.409e8 + 9.5e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_staged<false> launch (per launch, like `achieved`) and the
+# `ncu --set full` capture it was read from; refreshed whenever the kernel changes (the value is a property of that
+# capture, not of this run: `traffic_source` says which)
+NCU_TRAFFIC = {("C4", "k_pair_staged"): (1.3637e9 + 2.39e7, "profiles/r1d_summary.md (round-1 kernel; refresh pending)"),
+               ("C3", "k_pair_staged"): (3.409e8 + 9.5e6, "profiles/r1d_summary.md (round-1 kernel; refresh pending)")}
 
 
 def measure_dfma_peak() -> float:
@@ -215,6 +220,124 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def time_workload(sysg, cfg, top, x0, p0, K, args, world, local, dist_barrier):
+    """Warm-up, then the timed region of K steps with the state resident in HBM; returns the measurements."""
+    import torch
+    N, P = top["n_atoms"], cfg["P"]
+    xd, pd = torch.as_tensor(x0).cuda(), torch.as_tensor(p0).cuda()
+    sysg.set_state(xd, pd, 0)
+    sysg.step(args.warmup)
+    sysg.check()
+    c0 = sysg.counters()
+    sysg.profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        dist_barrier()
+        e0.record()
+        sysg.step(K)
+        e1.record()
+        dist_barrier()
+    ms = e0.elapsed_time(e1)
+    prof = sysg.profile_read()
+    sysg.profile(False)
+    c1 = sysg.counters()
+    ms = max_over_ranks(ms, world)
+    out = dict(ms=ms, prof=prof, c0=c0, c1=c1, clocks=clk.summary(), launches=int(c1["launches"] - c0["launches"]),
+               value=job_throughput(world, N, P, K, ms * 1e-3), ns_day=K * cfg["dt_fs"] * 1e-6 / (ms * 1e-3) * 86400.0)
+    return out
+
+
+def e2e_workload(sysg, cfg, top, x0, p0, K, args, world, dist_barrier):
+    """The same K steps through the host entry points of the C ABI, copies inside the timed region."""
+    import torch
+    N, P = top["n_atoms"], cfg["P"]
+    xh, ph = torch.as_tensor(x0).pin_memory(), torch.as_tensor(p0).pin_memory()
+    xo, po = torch.empty_like(xh).pin_memory(), torch.empty_like(ph).pin_memory()
+    sysg.set_state_host(xh, ph, 0)          # untimed pass: allocates the staging buffers
+    sysg.step(3 * args.n_alt)
+    sysg.get_state_host(xo, po)
+    sysg.observables_host()                 # every call of the timed region has run once (lazy module loading, buffers)
+    dist_barrier()
+    t0 = time.perf_counter()
+    sysg.set_state_host(xh, ph, 0)
+    t1 = time.perf_counter()
+    sysg.step(K)
+    sysg.get_state_host(xo, po)             # synchronises: the host buffers are valid on return
+    t2 = time.perf_counter()
+    obs = sysg.observables_host()
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    parts = dict(set_state_host=1e3 * (t1 - t0), steps_and_get_state_host=1e3 * (t2 - t1), observables_host=1e3 * (t0 + t_e2e - t2))
+    t_e2e = max_over_ranks(t_e2e, world)
+    nbytes = xh.numel() * 8
+    return dict(value=job_throughput(world, N, P, K, t_e2e), unit="bead-atom-steps/s",
+                h2d_bytes_per_step=2 * nbytes / K, d2h_bytes_per_step=(2 * nbytes + 32) / K,
+                ms_total=1e3 * t_e2e, ms_parts=parts, what="set_state_host + qhp_step(K) + get_state_host + observables_host",
+                observables=[float(v) for v in obs])
+
+
+def kernel_blocks(cfg, N, m, pk, dfma_tf, amortised=None):
+    """Per-kernel roofline blocks {ms, units, achieved, peak, frac} from the library's per-phase CUDA events."""
+    P, Pc, prof, c1, c0 = cfg["P"], cfg["P_contract"], m["prof"], m["c1"], m["c0"]
+    per = lambda k: prof[k]["ms"] / max(prof[k]["n"], 1)
+    pair_ms, int_ms = per("pair"), per("integrate")
+    pair_beads = c1["pair_beads_in_cutoff"]             # ordered (full list): each pair from both sides
+    flops = 0.5 * pair_beads * FLOP_PER_PAIR_BEAD       # algorithmic: every unordered pair-bead once
+    ach = flops / (pair_ms * 1e-3) / 1e12 if pair_ms > 0 else 0.0
+    kname = "k_pair_staged" if c1.get("staged") else "k_pair"
+    tr = NCU_TRAFFIC.get((cfg["name"], kname))
+    pair = dict(kernel=kname, bound="alu", ms_per_launch=pair_ms, units=0.5 * pair_beads, unit_name="unordered in-cutoff pair-beads",
+                flop_per_unit=FLOP_PER_PAIR_BEAD, achieved=ach, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s", frac=ach / FP64_PEAK_TFLOPS,
+                peak_source="derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz", peak_measured=dfma_tf,
+                frac_of_measured=ach / dfma_tf if dfma_tf > 0 else None, executed_tflops=2.0 * ach,
+                traffic=tr[0] if tr else None, traffic_source=tr[1] if tr else None)
+    if P == 1:      # adQTB / classical step (Q1): 7 x 8 B per DOF + 56 B per atom (pos4 write, Fs read)
+        int_bytes, iname = 7.0 * 8 * 3 * N + 56.0 * N, "k_integrate_mol1"
+    else:           # fused RPMD pass: 4 x 8 B per (DOF, bead) + (32 + 24) B x P' per atom
+        int_bytes, iname = 4.0 * 8 * 3 * N * P + (32.0 + 24.0) * N * Pc, "k_integrate"
+    int_gbs = int_bytes / (int_ms * 1e-3) / 1e9 if int_ms > 0 else 0.0
+    ks = {kname: pair,
+          iname: dict(bound="hbm", ms_per_launch=int_ms, units=int_bytes, unit_name="algorithmic bytes", achieved=int_gbs,
+                      peak=pk["hbm_gbs"], unit="GB/s", frac=int_gbs / pk["hbm_gbs"], peak_source=pk["source"]),
+          "rebuild_chain": dict(ms_per_step=per("rebuild"), rebuilds=int(c1["rebuilds"] - c0["rebuilds"]),
+                                what="cells + contraction + list kernels, enqueued every step (early exit unless a rebuild is due)")}
+    if amortised:
+        ks["rebuild_chain"]["amortised"] = amortised
+    if cfg["thermostat"] == "adqtb" and prof["qtb_generate"]["n"] > 0:
+        ns, dof = cfg["n_seg"], 3.0 * N
+        gen_ms, ad_ms = per("qtb_generate"), per("qtb_adapt")
+        # Q2-Q4 per DOF and segment: 3 n_seg Box-Muller normals (~100 flop) + forward and inverse 4 n_seg-point complex
+        # transform (5 n log2 n flop each) shared by the two real sequences of one complex transform
+        n4 = 4 * ns
+        gflop = dof * (3 * ns * 100.0 + 2 * 5.0 * n4 * np.log2(n4) / 2.0)
+        gtf = gflop / (gen_ms * 1e-3) / 1e12 if gen_ms > 0 else 0.0
+        ks["k_qtb_noise"] = dict(bound="alu", ms_per_segment=gen_ms, units=gflop, unit_name="flop (SURVEY 8(d): normals + FFT convolution)",
+                                 achieved=gtf, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s", frac=gtf / FP64_PEAK_TFLOPS,
+                                 bytes_written=dof * ns * 8.0, what="filter + kernel + k_qtb_noise, once per segment")
+        sbytes = 2.0 * dof * ns * 8
+        sgbs = sbytes / (ad_ms * 1e-3) / 1e9 if ad_ms > 0 else 0.0
+        ks["k_qtb_spectra"] = dict(bound="hbm", ms_per_segment=ad_ms, units=sbytes, unit_name="algorithmic bytes (v_seg + F_c read once)",
+                                   achieved=sgbs, peak=pk["hbm_gbs"], unit="GB/s", frac=sgbs / pk["hbm_gbs"], peak_source=pk["source"],
+                                   what="k_qtb_spectra + reduce + adaptation, once per segment")
+    return ks
+
+
+def cpu_baseline(cfg, n_steps=5, budget_mol=4096):
+    """The oracle as it stands, one thread, >= 5 steps of a bounded sample of the workload (the same force field,
+    density, P, P', thermostat on a box of at most `budget_mol` waters); setup (initial forces) not timed."""
+    import oracle as O
+    O.build()
+    n_mol = min(cfg["n_mol"], budget_mol)
+    top = W.water_box(n_mol)
+    x0, p0 = W.initial_state(top, cfg["P"], W.T_KELVIN)
+    _, s_per_step = oracle_steps(dict(cfg, n_mol=n_mol), top, x0, p0, n_steps)
+    N = 3 * n_mol
+    return dict(value=N * cfg["P"] / s_per_step, unit="bead-atom-steps/s", cores=1, kind="oracle",
+                sample=f"{n_steps} steps of a {n_mol}-water ({N}-atom) box of the {cfg['name']} workload (P={cfg['P']}, "
+                       f"P'={cfg['P_contract']}, {cfg['thermostat']}), {s_per_step:.3f} s/step, setup (initial forces) not timed",
+                host_cores_available=os.cpu_count())
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -227,6 +350,8 @@ def main():
     ap.add_argument("--n-mol", type=int, default=0, help="profiling aid: the same workload on a box of this many waters (0 = the BASELINE.json size)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-adqtb", action="store_true", help="skip the adQTB (C3) leg that the default C4 run appends")
+    ap.add_argument("--no-amortised", action="store_true", help="skip the untimed 500-step run that measures the list-rebuild rate")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -247,102 +372,66 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         dist.barrier()
 
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    pk = peaks()
+    dfma_tf = measure_dfma_peak()
+
+    # ---- primary workload (default C4: the configuration BASELINE.json's metric is quoted on) ------------
     cfg = workload(args.workload)
     if args.n_mol > 0:
         cfg["n_mol"] = args.n_mol
     top, sysg, x0, p0 = build_system(cfg)
     N, P, K = top["n_atoms"], cfg["P"], args.steps
-    xd = torch.as_tensor(x0).cuda()
-    pd = torch.as_tensor(p0).cuda()
     if args.a_block != "exact":
         sysg.set_a_block(args.a_block)
     if args.n_alt > 1:
         sysg.set_respa(args.n_alt)
         args.warmup = -(-args.warmup // args.n_alt) * args.n_alt
         args.steps = K = -(-args.steps // args.n_alt) * args.n_alt
-    sysg.set_state(xd, pd, 0)
-    sysg.step(args.warmup)
+    m = time_workload(sysg, cfg, top, x0, p0, K, args, world, local, barrier)
+    amortised = None
+    if not args.no_amortised and cfg["thermostat"] != "adqtb":
+        # list rebuilds are rare events: their rate and cost come from a longer untimed run of the same system
+        n_long = -(-500 // args.n_alt) * args.n_alt
+        ca = sysg.counters()
+        sysg.profile(True)
+        sysg.step(n_long)
+        pa = sysg.profile_read()
+        sysg.profile(False)
+        cb = sysg.counters()
+        nreb = int(cb["rebuilds"] - ca["rebuilds"])
+        amortised = dict(steps=n_long, rebuilds=nreb, rebuilds_per_step=nreb / n_long,
+                         ms_per_step=pa["rebuild"]["ms"] / max(pa["rebuild"]["n"], 1),
+                         ms_per_step_whole_run=sum(pa[k]["ms"] for k in ("integrate", "rebuild", "pair")) / n_long,
+                         what=f"untimed {n_long}-step continuation: rebuild-chain time per step including the rebuilds that fell inside")
+    kernels = kernel_blocks(cfg, N, m, pk, dfma_tf, amortised)
+    e2e = None if args.no_e2e else e2e_workload(sysg, cfg, top, x0, p0, K, args, world, barrier)
     sysg.check()
+    del sysg
+    torch.cuda.empty_cache()
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    # ---- timed region: K steps, state resident in HBM ------------------------------------------
-    c0 = sysg.counters()
-    sysg.profile(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local) as clk:
-        barrier()
-        e0.record()
-        sysg.step(K)
-        e1.record()
-        barrier()
-    ms = e0.elapsed_time(e1)
-    prof = sysg.profile_read()
-    sysg.profile(False)
-    c1 = sysg.counters()
-    launches = c1["launches"] - c0["launches"]          # kernels the library launched inside the timed region
-    ms = max_over_ranks(ms, world)
-    value = job_throughput(world, N, P, K, ms * 1e-3)
-    ns_day = K * cfg["dt_fs"] * 1e-6 / (ms * 1e-3) * 86400.0
-
-    # ---- roofline of the dominant kernel (pair forces) ------------------------------------------
-    pair_ms = prof["pair"]["ms"] / max(prof["pair"]["n"], 1)
-    int_ms = prof["integrate"]["ms"] / max(prof["integrate"]["n"], 1)
-    pair_beads = c1["pair_beads_in_cutoff"]             # ordered (full list): each pair from both sides
-    flops_algo = 0.5 * pair_beads * FLOP_PER_PAIR_BEAD  # algorithmic: every unordered pair-bead once
-    ach = flops_algo / (pair_ms * 1e-3) / 1e12 if pair_ms > 0 else 0.0
-    pk = peaks()
-    kname = "k_pair_staged" if c1.get("staged") else "k_pair"
-    dfma_tf = measure_dfma_peak()
-    roofline = dict(kernel=kname, bound="alu", achieved=ach, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
-                    frac=ach / FP64_PEAK_TFLOPS, traffic=NCU_TRAFFIC_BYTES.get((cfg["name"], kname)),
-                    peak_source="derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz",
-                    peak_measured=dfma_tf, frac_of_measured=ach / dfma_tf if dfma_tf > 0 else None,
-                    executed_tflops=2.0 * ach, ms_per_launch=pair_ms,
-                    note="achieved counts each unordered in-cutoff pair-bead once (110 flop); the kernel "
-                         "evaluates both directions (full list, no atomics), see executed_tflops; "
-                         "peak_measured = live qhp_dfma_probe")
-    # second kernel: fused integrator pass, HBM-bound: 4 x 8 B per (DOF, bead) + 2 x 24 B * P'/P ... per atom-bead
-    int_bytes = 4.0 * 8 * 3 * N * P + (32.0 + 24.0) * N * cfg["P_contract"]
-    int_gbs = int_bytes / (int_ms * 1e-3) / 1e9 if int_ms > 0 else 0.0
-    kernels = dict(k_integrate=dict(bound="hbm", ms_per_launch=int_ms, achieved=int_gbs, peak=pk["hbm_gbs"], unit="GB/s",
-                                    frac=int_gbs / pk["hbm_gbs"], peak_source=pk["source"]),
-                   rebuild_chain=dict(ms_per_step=prof["rebuild"]["ms"] / max(prof["rebuild"]["n"], 1),
-                                      rebuilds=c1["rebuilds"] - c0["rebuilds"]),
-                   qtb_generate=dict(ms_per_segment=prof["qtb_generate"]["ms"] / max(prof["qtb_generate"]["n"], 1), n=prof["qtb_generate"]["n"]),
-                   qtb_adapt=dict(ms_per_segment=prof["qtb_adapt"]["ms"] / max(prof["qtb_adapt"]["n"], 1), n=prof["qtb_adapt"]["n"]))
-
-    # ---- e2e through the host entry points ----------------------------------------------------------
-    e2e = None
-    if not args.no_e2e:
-        xh = torch.as_tensor(x0).pin_memory()
-        ph = torch.as_tensor(p0).pin_memory()
-        xo, po = torch.empty_like(xh).pin_memory(), torch.empty_like(ph).pin_memory()
-        sysg.set_state_host(xh, ph, 0)          # untimed pass: allocates the staging buffers
-        sysg.step(3 * args.n_alt)
-        sysg.get_state_host(xo, po)
-        sysg.observables_host()                 # every call of the timed region has run once (lazy module loading, buffers)
-        barrier()
-        t0 = time.perf_counter()
-        sysg.set_state_host(xh, ph, 0)
-        t1 = time.perf_counter()
-        sysg.step(K)
-        sysg.get_state_host(xo, po)             # synchronises: the host buffers are valid on return
-        t2 = time.perf_counter()
-        obs = sysg.observables_host()
-        torch.cuda.synchronize()
-        t_e2e = time.perf_counter() - t0
-        parts = dict(set_state_host=1e3 * (t1 - t0), steps_and_get_state_host=1e3 * (t2 - t1), observables_host=1e3 * (t0 + t_e2e - t2))
-        t_e2e = max_over_ranks(t_e2e, world)
-        nbytes = xh.numel() * 8
-        e2e = dict(value=job_throughput(world, N, P, K, t_e2e), unit="bead-atom-steps/s",
-                   h2d_bytes_per_step=2 * nbytes / K, d2h_bytes_per_step=(2 * nbytes + 32) / K,
-                   ms_total=1e3 * t_e2e, ms_parts=parts, what="set_state_host + qhp_step(K) + get_state_host + observables_host",
-                   observables=[float(v) for v in obs])
-    sysg.check()
+    # ---- adQTB leg (C3: 216,000 atoms, one whole 1024-step segment: noise generation, 1024 steps, spectra +
+    #      adaptation), appended to the default run so that one driver run measures both halves of the metric ----
+    adqtb = None
+    if args.workload == "C4" and not args.no_adqtb and args.n_mol == 0 and args.n_alt == 1:
+        c3 = workload("C3")
+        top3, sys3, x3, p3 = build_system(c3)
+        K3 = c3["n_seg"]
+        m3 = time_workload(sys3, c3, top3, x3, p3, K3, args, world, local, barrier)
+        e3 = None if args.no_e2e else e2e_workload(sys3, c3, top3, x3, p3, K3, args, world, barrier)
+        sys3.check()
+        adqtb = dict(workload="C3", n_atoms=top3["n_atoms"], steps=K3, value=m3["value"], unit="bead-atom-steps/s",
+                     ms_per_step=m3["ms"] / K3, ns_per_day=m3["ns_day"], dt_fs=c3["dt_fs"], n_seg=c3["n_seg"],
+                     gpu_launches=m3["launches"], clocks=m3["clocks"], e2e=e3,
+                     kernels=kernel_blocks(c3, top3["n_atoms"], m3, pk, dfma_tf),
+                     what="one whole segment: coloured-noise generation (Q2-Q4), 1024 BAOAB steps with pair forces and list "
+                          "rebuilds (Q1, R7, R8), spectra + gamma adaptation (Q5-Q7)")
+        del sys3
+        torch.cuda.empty_cache()
 
     if rank != 0:
         if world > 1:
@@ -350,27 +439,27 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- oracle on the host cores (bounded sample: one step of the same workload) ----------------
+    # ---- oracle on the host cores (bounded sample of the same workloads) ----------------------------------
     cpu = None
     if not args.no_cpu_baseline:
-        import oracle as O
-        O.build()
-        n_cpu = 1 if N > 20000 else (5 if N > 2000 else 20)
-        _, s_per_step = oracle_steps(cfg, top, x0, p0, n_cpu)
-        cpu = dict(value=N * P / s_per_step, unit="bead-atom-steps/s", cores=1, kind="oracle",
-                   sample=f"{n_cpu} step(s) of the full {cfg['name']} workload ({N} atoms, P={P}, P'={cfg['P_contract']}), "
-                          f"{s_per_step:.2f} s/step, setup (initial forces) not timed",
-                   host_cores_available=os.cpu_count())
+        cpu = cpu_baseline(cfg)
+        if adqtb is not None:
+            adqtb["cpu_baseline"] = cpu_baseline(workload("C3"))
 
-    line = dict(metric="bead_atom_steps_per_s", value=value, unit="bead-atom-steps/s", n_gpus=world, steps=K,
-                warmup=args.warmup, ms_per_step=ms / K, higher_is_better=True, scaling="weak", vs_baseline=None,
+    pair_block = kernels["k_pair_staged"] if "k_pair_staged" in kernels else kernels["k_pair"]
+    roofline = dict(pair_block, note="achieved counts each unordered in-cutoff pair-bead once (110 flop); the kernel "
+                                     "evaluates both directions (full list, no atomics), see executed_tflops; "
+                                     "peak_measured = live qhp_dfma_probe")
+    line = dict(metric="bead_atom_steps_per_s", value=m["value"], unit="bead-atom-steps/s", n_gpus=world, steps=K,
+                warmup=args.warmup, ms_per_step=m["ms"] / K, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f64", data="synthetic",
                 config=dict(workload=cfg["name"], n_atoms=N, P=P, P_contract=cfg["P_contract"], dt_fs=cfg["dt_fs"],
-                            thermostat=cfg["thermostat"], n_alt=args.n_alt, a_block=args.a_block, ns_per_day=ns_day, parallelism="replicas only" if world > 1 else "1 GPU",
+                            thermostat=cfg["thermostat"], n_alt=args.n_alt, a_block=args.a_block, ns_per_day=m["ns_day"],
+                            parallelism="independent replicas (no data-path collective)" if world > 1 else "1 GPU",
                             l2="inputs larger than L2 (state + neighbour table >> 126 MB)" if N > 100000 else "inputs smaller than L2",
-                            pair_beads_in_cutoff=pair_beads, list_entries=c1["list_entries"]),
-                clocks=clk.summary(), e2e=e2e, gpu_launches=int(launches),
-                roofline=roofline, kernels=kernels, cpu_baseline=cpu)
+                            pair_beads_in_cutoff=m["c1"]["pair_beads_in_cutoff"], list_entries=m["c1"]["list_entries"]),
+                clocks=m["clocks"], e2e=e2e, gpu_launches=m["launches"],
+                roofline=roofline, kernels=kernels, adqtb=adqtb, cpu_baseline=cpu)
     print(json.dumps(line))
     if world > 1:
         dist.barrier()

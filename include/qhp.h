@@ -75,7 +75,9 @@ typedef struct {
   int32_t kind;          /* qhp_thermo_kind                                                     */
   double gamma0;         /* 1/ps: PILE centroid friction / adQTB gamma_0 (Eq. 12)*/
   uint64_t seed;         /* Philox4x32-10 key                                                   */
-  int32_t n_seg;         /* adQTB: steps per noise segment, power of two >= 8    */
+  int32_t n_seg;         /* adQTB: steps per noise segment, a power of two in [8, 2048]         */
+                         /* (the 4 n_seg-point transform of the noise lives in    */
+                         /* shared memory: 8192 points = 128 KB is the largest that fits)       */
   double a_gamma;        /* adQTB: adaptation rate A (Eq. 23, reading G15); 0 = no adaptation   */
   double gamma_min_frac; /* adQTB: gamma_z >= gamma_min_frac * gamma0; 0.01      */
   int32_t classical;     /* adQTB: != 0 replaces Theta(omega) by kB T (test hook, hbar -> 0)    */

@@ -61,6 +61,12 @@ def test_create_argument_errors(lib):
     assert _create(lib, top, 8, 8, -1.0, 300.0)[0] == EINVAL
     assert _create(lib, top, 2, 1, 5e-4, 300.0, kind=2, gamma0=20.0, n_seg=64)[0] == EINVAL   # adQTB needs P = 1
     assert _create(lib, top, 1, 1, 5e-4, 300.0, kind=2, gamma0=20.0, n_seg=48)[0] == EINVAL   # n_seg not 2^k
+    # documented limits of include/qhp.h: n_seg a power of two in [8, 2048]; qhp_fft_c2c n a power of two in [8, 8192]
+    assert _create(lib, top, 1, 1, 5e-4, 300.0, kind=2, gamma0=20.0, n_seg=4)[0] == EINVAL
+    assert _create(lib, top, 1, 1, 5e-4, 300.0, kind=2, gamma0=20.0, n_seg=4096)[0] == EINVAL
+    one = C.c_double(0.0)
+    for n in (4, 12, 16384):
+        assert lib.qhp_fft_c2c(C.byref(one), n, 1, -1, None) == EINVAL
     small = dict(top); small["box"] = np.array([17.0, 20.0, 20.0])
     rc, _, msg = _create(lib, small, 8, 8, 2.5e-4, 300.0)
     assert rc == EINVAL and "box" in msg

@@ -195,3 +195,25 @@ def test_kappa_classicalising_factor_is_white_noise_baoab():
     sysg.step(20)
     ref.step(20)
     assert np.abs(sysg.get_state()[0].cpu().numpy() - ref.get_state()[0]).max() < 1e-8
+
+
+def test_n_seg_2048_segment_parity():
+    """The documented upper limit n_seg = 2048 (8192-point noise transform, 4096-point spectra, one DOF per
+    spectra round): F_c of the first segment against the oracle, gamma_z after it from the product's arrays."""
+    import oracle as O
+    top = W.water_box(27)
+    top["box"] = np.array([20.0, 20.0, 20.0])
+    n_seg, g0 = 2048, 20.0
+    sysg, ref, x0, p0 = make_pair(top, 1, 1, 0.5, "adqtb", gamma0=g0, n_seg=n_seg, a_gamma=0.5)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    sysg.step(n_seg)
+    ref.step(1)                                          # generates the oracle's first segment
+    Fc, v = sysg.adqtb_segment()
+    Fc, v = Fc.cpu().numpy(), v.cpu().numpy()
+    assert np.abs(Fc - ref.Fc).max() < 1e-11 * np.sqrt((ref.Fc ** 2).mean())
+    otop = O.Topology(top)
+    g_ref, _ = oracle_adapt_from_segment(otop, n_seg, 0.5e-3, g0, 0.5, 0.01, v, Fc, np.full((otop.n_types, n_seg + 1), g0))
+    g = sysg.adqtb_gamma().cpu().numpy()
+    assert np.abs(g - g_ref).max() < 1e-9 * np.abs(g_ref).max()
+    sysg.check()

@@ -33,7 +33,7 @@ def test_philox_normal_moments():
     assert abs((z ** 4).mean() - 3) < 5 * np.sqrt(96 / n)
 
 
-@pytest.mark.parametrize("n", [8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096])
+@pytest.mark.parametrize("n", [8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192])
 def test_fft_matches_dft(n):
     import torch
     import paper_2212_03137_b200 as qhp
