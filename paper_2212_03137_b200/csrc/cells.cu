@@ -22,7 +22,6 @@ struct CellArgs {
   int N, nc[3], ncell;
   double box[3], inv_box[3], rl2;
   float boxf[3], inv_boxf[3], edgef[3], rl2_lo, rl2_hi;   // fp32 pre-test: d2f < lo surely inside, >= hi surely outside
-  float rn2;                                              // staged lists: d2f < rn2 => centroid distance surely below r_cut - skin ("near" entry)
   const unsigned long long *flag;
   double thresh2;
 };
@@ -195,12 +194,7 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
   uint16_t *row = nbr + (long long)i * stride;
   float lo = a.rl2_lo, hi = a.rl2_hi;
   asm volatile("" : "+r"(lt), "+l"(row));
-  // Row layout (pair_staged.cu): block 0 (256 entries) holds the NEAR entries, centroid distance < r_cut - skin:
-  // such a pair stays inside the cutoff for every bead as long as the list is valid (no bead moves farther
-  // than skin/2 from the centroid it had at the build), so the pair kernel evaluates it without a pre-test;
-  // the other (FAR) entries follow from offset 256.  A near entry that finds block 0 full is filed as far.
-  int cnt = 0, cnear = 0, off = 0;
-  float rn2 = a.rn2;
+  int cnt = 0, off = 0;
   // The 27 stencil cells are walked as 9 (x, y) columns.  The three cells of a column are adjacent in z,
   // hence contiguous in slot order unless the column wraps around the box: they are scanned as one run
   // (fewer ragged 32-candidate chunks, one set of per-run constants).  A cell whose box is out of reach
@@ -239,7 +233,7 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
         while (oz2 < 3 && reach[oz2] && bq[oz2] == e && sz[oz2] == sz[oz]) { e = eq[oz2]; off += eq[oz2] - bq[oz2]; ++oz2; }
         // the inner loop decides the run time of a rebuild: keep its invariants in registers (ptxas
         // otherwise re-derives the image shifts and reloads the thresholds every iteration)
-        asm volatile("" : "+f"(px), "+f"(py), "+f"(pz), "+f"(lo), "+f"(hi), "+f"(rn2), "+r"(idx0), "+r"(e));
+        asm volatile("" : "+f"(px), "+f"(py), "+f"(pz), "+f"(lo), "+f"(hi), "+r"(idx0), "+r"(e));
         const int last = e - 1;
         for (int k = b + lane; k - lane < e; k += 32) {
           const float4 fj = centf[min(k, last)];
@@ -249,48 +243,38 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
           bool hit = (k <= last) & (k != i) & ((wj & 0x0fffffff) != wi) & (d2f < hi);
           if (hit && !(d2f < lo)) hit = list_hit_exact(a, cent4, ci, k);      // the thin shell around r_list
           const unsigned mask = __ballot_sync(0xffffffffu, hit);
-          const bool room = cnear <= 256 - 32;                    // warp-uniform: block 0 can take a whole step
-          const unsigned mnear = __ballot_sync(0xffffffffu, hit && room && d2f < rn2);
           if (FILL && hit) {
-            const uint16_t v = (uint16_t)((idx0 + k) | ((wj >> 28) << 13));
-            if ((mnear >> lane) & 1u) {
-              const int pos = cnear + __popc(mnear & lt);
-              row[((pos & 31) << 3) + (pos >> 5)] = v;
-            } else {
-              const int pos = cnt + __popc(mask & ~mnear & lt);
-              if (pos < stride - 256) row[256 + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = v;
-            }
+            const int pos = cnt + __popc(mask & lt);
+            if (pos < stride) row[(pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)((idx0 + k) | ((wj >> 28) << 13));
           }
-          cnear += __popc(mnear);
-          cnt += __popc(mask & ~mnear);
+          cnt += __popc(mask);
         }
         oz = oz2;
       }
     }
   }
   if (FILL) {
-    // pad the last 32-entry step of both parts with the dummy staged index (pair_staged.cu: no pre-test against it passes)
-    for (int pos = cnear + lane; pos < ((cnear + 31) & ~31); pos += 32) row[((pos & 31) << 3) + (pos >> 5)] = (uint16_t)dummy;
-    const int n = min(cnt, stride - 256), end = min((n + 31) & ~31, stride - 256);
+    // pad the last 32-entry step with the dummy staged index (pair_staged.cu: no pre-test against it passes)
+    const int n = min(cnt, stride), end = min((n + 31) & ~31, stride);
     for (int pos = n + lane; pos < end; pos += 32)
-      row[256 + (pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)dummy;
+      row[(pos & ~255) + ((pos & 31) << 3) + ((pos & 255) >> 5)] = (uint16_t)dummy;
   }
   if (lane == 0) {
     if (FILL) {
-      nbr_count[i] = min(cnt, stride - 256) | (cnear << 16);       // far | near << 16
-      if (cnt > stride - 256) counters[1] = 1;
+      nbr_count[i] = min(cnt, stride);
+      if (cnt > stride) counters[1] = 1;
     } else {
-      nbr_count[i] = cnt + cnear;
+      nbr_count[i] = cnt;
     }
-    atomicMax((unsigned long long *)&counters[2], (unsigned long long)(cnt + cnear));
+    atomicMax((unsigned long long *)&counters[2], (unsigned long long)cnt);
     atomicMax((unsigned long long *)&counters[5], (unsigned long long)off);   // staged-region size
   }
 }
 
 // ---- export in atom indices (parity hook) ---------------------------------------------------------
-__global__ void k_export_count(int N, const int32_t *__restrict__ order, const int32_t *__restrict__ nbr_count, int32_t *count, int staged) {
+__global__ void k_export_count(int N, const int32_t *__restrict__ order, const int32_t *__restrict__ nbr_count, int32_t *count) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < N) count[order[i]] = staged ? (nbr_count[i] & 0xffff) + (nbr_count[i] >> 16) : nbr_count[i];   // staged: far | near << 16
+  if (i < N) count[order[i]] = nbr_count[i];
 }
 __global__ void k_export_fill(int N, const int32_t *__restrict__ order, const int32_t *__restrict__ nbr_count,
                               const int32_t *__restrict__ nbr, long long stride, const int32_t *__restrict__ start,
@@ -312,7 +296,7 @@ __global__ void k_export_fill16(const CellArgs a, const int32_t *__restrict__ ce
   const int lane = threadIdx.x & 31;
   const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (i >= a.N) return;
-  const int at = order[i], nnear = nbr_count[i] >> 16, n = (nbr_count[i] & 0xffff) + nnear;
+  const int at = order[i], n = nbr_count[i];
   const int cell = cell_of[at];
   const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
   int cb = 0, cn = 0;                       // lane s < 27: first slot and size of stencil cell s
@@ -326,8 +310,7 @@ __global__ void k_export_fill16(const CellArgs a, const int32_t *__restrict__ ce
   const long long s0 = start[at];
   for (int k0 = 0; k0 < n; k0 += 32) {
     const int k = k0 + lane;
-    const int q = k < nnear ? k : 256 + k - nnear;           // near entries in block 0, far entries from offset 256
-    const int loc = k < n ? (int)(nbr[i * stride + (q & ~255) + ((q & 31) << 3) + ((q & 255) >> 5)] & 0x1fff) : 0;
+    const int loc = k < n ? (int)(nbr[i * stride + (k & ~255) + ((k & 31) << 3) + ((k & 255) >> 5)] & 0x1fff) : 0;
     int off = 0, slot = -1;
     for (int s = 0; s < 27; ++s) {
       const int b = __shfl_sync(0xffffffffu, cb, s), c = __shfl_sync(0xffffffffu, cn, s);
@@ -353,8 +336,6 @@ static CellArgs cell_args(qhp_system *s, bool force) {
     const double m = 4.0 * (2.0 * sqrt(3.0) * rl * e + 4.0 * ldexp(1.0, -24) * a.rl2);
     a.rl2_lo = (float)(a.rl2 - m) * (1.0f - 1.2e-7f);
     a.rl2_hi = (float)(a.rl2 + m) * (1.0f + 1.2e-7f);
-    const double rn = s->r_cut - s->skin;                     // near entries: surely below r_cut - skin
-    a.rn2 = rn > 0.0 ? (float)fmax(rn * rn - m, 0.0) * (1.0f - 1.2e-7f) : 0.0f;
   }
   a.flag = force ? nullptr : &s->d2max[s->flag_idx];
   const double th = 0.5 * s->skin;
@@ -490,10 +471,9 @@ int qhp_cells_rebuild(qhp_system *s, bool force) {
       s->staged = false;                               // too dense: generic kernel and 32-bit list
     }
     const bool have = s->staged ? (s->nbr16 != nullptr) : (s->nbr != nullptr);
-    if (!have || mx + 8 + (s->staged ? 256 : 0) > s->nbr_stride) {
+    if (!have || mx + 8 > s->nbr_stride) {
       int64_t stride = (int64_t)((double)mx * 1.4) + 32;
       stride = (stride + 255) / 256 * 256;                 // whole 256-entry row blocks (pair_staged.cu)
-      if (s->staged) stride += 256;                        // block 0 holds the near entries
       if (stride < 4) stride = 4;
       if (s->nbr) cudaFree(s->nbr);
       if (s->nbr16) cudaFree(s->nbr16);
@@ -518,7 +498,7 @@ int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, i
   int32_t *cnt = count;
   int32_t *cnt_own = nullptr;
   if (!cnt) { QHP_CUDA_OK(s, cudaMalloc(&cnt_own, sizeof(int32_t) * (size_t)s->N)); cnt = cnt_own; }
-  k_export_count<<<(s->N + tb - 1) / tb, tb, 0, s->stream>>>(s->N, s->order, s->nbr_count, cnt, s->staged ? 1 : 0);
+  k_export_count<<<(s->N + tb - 1) / tb, tb, 0, s->stream>>>(s->N, s->order, s->nbr_count, cnt);
   QHP_LAUNCH_OK(s);
   CellArgs a{};
   a.flag = nullptr;

@@ -9,11 +9,8 @@
 // shared memory, in coordinates relative to the cell centre (so the minimum image is applied per
 // staged atom, not per pair), and the neighbour table holds 16-bit indices into that staged array.
 //
-// Per atom i (one warp); a list row = [near entries | far entries], each entry = staged index | type << 13:
-//   near    centroid distance at the list build < r_cut - skin: inside the cutoff for every bead as
-//           long as the list is valid (no bead is farther than skin/2 from that centroid), so the
-//           entry is evaluated straight from the row: no pre-test, no queue (47 % of the pairs);
-//   check   far entries, 32 at a time: fp32 distance test on a float4 copy (conservative margin,
+// Per atom i (one warp); a list entry = staged index | atom type << 13:
+//   check   32 list entries at a time: fp32 distance test on a float4 copy (conservative margin,
 //           it only rejects pairs that are certainly outside r_c), ballot compaction of the
 //           survivors into a per-warp queue; the record of the next step is requested one step ahead;
 //   eval    whenever the queue holds >= 32 survivors: all 32 lanes evaluate one pair each in fp64
@@ -36,7 +33,7 @@
 #endif
 #define STG_MAX_WARPS (STG_THREADS / 32)
 #define STG_BLOCK 256             // list entries per row block (8 per lane)
-#define STG_QUEUE (STG_BLOCK + 64)   // <= 31 left over + 31 from the near block + 256
+#define STG_QUEUE (STG_BLOCK + 32)   // <= 31 left over + 256
 #define STG_IDX_BITS 13           // list entry = staged index | atom type << 13 (QHP_MAX_TYPES = 8)
 #define STG_IDX_MASK 0x1fffu
 
@@ -189,11 +186,11 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
     if (ii >= nh) break;
     const uint32_t ei = (uint32_t)(h0 + ii);
     const long long slot = slot0 + ii;
-    const int nc2 = a.nbr_count[slot];                   // far | near << 16 (cells.cu k_list_build16)
-    const int n = nc2 & 0xffff, nnear = nc2 >> 16;
+    const int n = a.nbr_count[slot];
     const uint16_t *rowp = a.nbr16 + slot * a.stride;
-    const int nblk = 1 + (n + STG_BLOCK - 1) / STG_BLOCK;  // block 0: near entries, blocks 1..: far entries
-    uint4 cur = *reinterpret_cast<const uint4 *>(rowp + 8 * lane);
+    const int nblk = (n + STG_BLOCK - 1) / STG_BLOCK;
+    uint4 cur = make_uint4(0u, 0u, 0u, 0u);
+    if (nblk > 0) cur = *reinterpret_cast<const uint4 *>(rowp + 8 * lane);
     const double2 xyi = lds_d2(sXY + ei * 16);
     const double zi = lds_d(sZ + ei * 8);
     float4 ci = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -243,22 +240,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       if (m + 1 < nblk) nxt = *reinterpret_cast<const uint4 *>(rowp + STG_BLOCK * (m + 1) + 8 * lane);
       const uint32_t w[4] = {cur.x, cur.y, cur.z, cur.w};
       auto entry = [&](int j) { return (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu); };
-      if (m == 0) {
-        // ---- near entries: inside the cutoff for every bead while the list is valid -> no pre-test, no queue ----
-        const int nfull = nnear >> 5, rem = nnear & 31;
-        // rolled loop (one copy of the evaluation code): entry j of this lane selected from the four words
-#pragma unroll 1
-        for (int j = 0; j <= nfull; ++j) {
-          const uint32_t ww = (j & 4) ? ((j & 2) ? cur.w : cur.z) : ((j & 2) ? cur.y : cur.x);
-          const uint32_t e = (j & 1) ? (ww >> 16) : (ww & 0xffffu);
-          if (j < nfull) eval(e, true);
-          else if (rem) {                                // the partial last step joins the queue of the far survivors
-            if (lane < rem) sts_u(qa + lane * 4, e);
-            qa += rem * 4;
-          }
-        }
-      } else {
-      const int nst = min(8, (n - STG_BLOCK * (m - 1) + 31) >> 5);
+      const int nst = min(8, (n - STG_BLOCK * m + 31) >> 5);
       // ---- check: pre-test of 32 entries per step, survivors compacted into the queue; the staged record
       //      of the next step is requested before this step's compaction store ------------------------------
       float4 cj = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -283,7 +265,6 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
         const unsigned mask = __ballot_sync(0xffffffffu, hit);
         if (hit) sts_u(qa + __popc(mask & lt) * 4, e);
         qa += __popc(mask) * 4;
-      }
       }
       __syncwarp();
       // ---- eval: full warps of survivors ---------------------------------------------------------------
