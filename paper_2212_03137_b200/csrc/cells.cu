@@ -17,6 +17,7 @@
 #include <cooperative_groups.h>
 
 #include "qhp_internal.cuh"
+#include "contract.cuh"
 
 struct CellArgs {
   int N, nc[3], ncell;
@@ -122,16 +123,10 @@ __device__ __forceinline__ bool list_hit(const CellArgs &a, const double *__rest
   return list_hit_exact(a, cent4, ci, k);
 }
 
-// one warp per slot; nbr == NULL: count only
-__global__ void __launch_bounds__(256) k_list_build(const CellArgs a, const double *__restrict__ cent4,
-                                                    const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
-                                                    const int32_t *__restrict__ cell_start, int32_t *nbr,
-                                                    int32_t *nbr_count, long long stride, long long *counters) {
-  if (cells_skip(a)) return;
-  const int lane = threadIdx.x & 31;
-  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (i >= a.N) return;
-  if (i == 0 && lane == 0 && nbr) counters[0] += 1;
+// one warp per slot (row i of the table); nbr == NULL: count only
+__device__ __forceinline__ void list_row32(const CellArgs &a, const double *__restrict__ cent4, const int32_t *__restrict__ cell_of,
+                                           const int32_t *__restrict__ order, const int32_t *__restrict__ cell_start, int32_t *nbr,
+                                           int32_t *nbr_count, long long stride, long long *counters, long long i, int lane) {
   const float4 *centf = reinterpret_cast<const float4 *>(cent4 + 4LL * a.N);   // fp32 copies live behind cent4
   const double4 ci = reinterpret_cast<const double4 *>(cent4)[i];
   const float4 fi = centf[i];
@@ -171,19 +166,26 @@ __global__ void __launch_bounds__(256) k_list_build(const CellArgs a, const doub
   }
 }
 
+__global__ void __launch_bounds__(256) k_list_build(const CellArgs a, const double *__restrict__ cent4,
+                                                    const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
+                                                    const int32_t *__restrict__ cell_start, int32_t *nbr,
+                                                    int32_t *nbr_count, long long stride, long long *counters) {
+  if (cells_skip(a)) return;
+  const int lane = threadIdx.x & 31;
+  const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i >= a.N) return;
+  if (i == 0 && lane == 0 && nbr) counters[0] += 1;
+  list_row32(a, cent4, cell_of, order, cell_start, nbr, nbr_count, stride, counters, i, lane);
+}
+
 // Same pair set, written as 16-bit indices into the staged array of the row's cell (pair_staged.cu):
 // index = (number of atoms in the stencil cells before this one, in the stencil order below) + (k - b).
 // Requires nc >= 4 in every dimension (27 distinct stencil cells).
 template <bool FILL>
-__global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const double *__restrict__ cent4,
-                                                      const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
-                                                      const int32_t *__restrict__ cell_start, uint16_t *nbr,
-                                                      int32_t *nbr_count, int stride, int dummy, long long *counters) {
-  if (cells_skip(a)) return;
-  const int lane = threadIdx.x & 31;
-  const int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
-  if (i >= a.N) return;
-  if (i == 0 && lane == 0 && FILL) counters[0] += 1;
+__device__ __forceinline__ void list_row16(const CellArgs &a, const double *__restrict__ cent4,
+                                           const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
+                                           const int32_t *__restrict__ cell_start, uint16_t *nbr,
+                                           int32_t *nbr_count, int stride, int dummy, long long *counters, int i, int lane) {
   const float4 *centf = reinterpret_cast<const float4 *>(cent4 + 4LL * a.N);   // fp32 copies live behind cent4
   const double4 ci = reinterpret_cast<const double4 *>(cent4)[i];
   const float4 fi = centf[i];
@@ -271,6 +273,19 @@ __global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const do
   }
 }
 
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_list_build16(const CellArgs a, const double *__restrict__ cent4,
+                                                      const int32_t *__restrict__ cell_of, const int32_t *__restrict__ order,
+                                                      const int32_t *__restrict__ cell_start, uint16_t *nbr,
+                                                      int32_t *nbr_count, int stride, int dummy, long long *counters) {
+  if (cells_skip(a)) return;
+  const int lane = threadIdx.x & 31;
+  const int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  if (i >= a.N) return;
+  if (i == 0 && lane == 0 && FILL) counters[0] += 1;
+  list_row16<FILL>(a, cent4, cell_of, order, cell_start, nbr, nbr_count, stride, dummy, counters, i, lane);
+}
+
 // ---- export in atom indices (parity hook) ---------------------------------------------------------
 __global__ void k_export_count(int N, const int32_t *__restrict__ order, const int32_t *__restrict__ nbr_count, int32_t *count) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -347,9 +362,24 @@ static CellArgs cell_args(qhp_system *s, bool force) {
 // The four cell kernels as one cooperative kernel (grid-wide barriers between the phases): inside
 // qhp_step the chain is enqueued every step and returns at once unless a rebuild is due, so one launch
 // instead of four takes 3 kernel boundaries off every step (they dominate the small boxes).
+// Rest of the rebuild chain inside the same cooperative kernel (ra.on): contraction of the current modes into the
+// new slot order (+ sorted centroids, fp32 copy, reference centroids) and the list build, its rows handed to the
+// warps through a work counter -- one launch per step, which returns at once unless a rebuild is due.
+struct RebuildArgs {
+  int on, Pc, staged, stride, dummy;
+  BoxArg bx;
+  const double *Q, *Tc;
+  const int32_t *type, *molid;
+  double *pos4, *cent4, *cref;
+  uint16_t *nbr16;
+  int32_t *nbr;
+  int32_t *nbr_count;
+  long long stride32;
+  long long *counters;           // [4] = work counter of the list phase
+};
 __global__ void __launch_bounds__(256) k_cells_fused(const CellArgs a, const double *__restrict__ Q0, int32_t *cell_of,
                                                      int32_t *cell_count, int32_t *cell_start, int32_t *cursor,
-                                                     int32_t *tmp, int32_t *order, int32_t *rank) {
+                                                     int32_t *tmp, int32_t *order, int32_t *rank, const RebuildArgs ra) {
   if (cells_skip(a)) return;                       // uniform over the grid: nobody reaches a barrier
   namespace cg = cooperative_groups;
   cg::grid_group grid = cg::this_grid();
@@ -402,16 +432,35 @@ __global__ void __launch_bounds__(256) k_cells_fused(const CellArgs a, const dou
     order[b + cnt] = i;
     rank[i] = b + cnt;
   }
+  if (!ra.on) return;
+  grid.sync();
+  if (t0 == 0) { ra.counters[4] = 0; ra.counters[0] += 1; }
+  for (long long d = t0; d < 3LL * a.N; d += nthreads)
+    qhp_contract_dof(ra.bx, ra.Q, a.N, ra.Pc, ra.Tc, rank, ra.type, ra.molid, ra.pos4, ra.cent4, ra.cref, nullptr, 0,
+                     a.thresh2, ra.counters, d);
+  grid.sync();
+  const int lane = threadIdx.x & 31;
+  for (;;) {
+    long long i = 0;
+    if (lane == 0) i = (long long)atomicAdd((unsigned long long *)&ra.counters[4], 1ull);
+    i = __shfl_sync(0xffffffffu, i, 0);
+    if (i >= a.N) break;
+    if (ra.staged) list_row16<true>(a, ra.cent4, cell_of, order, cell_start, ra.nbr16, ra.nbr_count, ra.stride, ra.dummy, ra.counters, (int)i, lane);
+    else list_row32(a, ra.cent4, cell_of, order, cell_start, ra.nbr, ra.nbr_count, ra.stride32, ra.counters, i, lane);
+  }
 }
 
-static int cells_only(qhp_system *s, const CellArgs &a) {
+static int cells_only(qhp_system *s, const CellArgs &a, const RebuildArgs *fused = nullptr) {
   if (s->coop_blocks > 0) {
     const int tb = 256;
     int grid = (s->N + tb - 1) / tb;
+    if (fused) grid = s->coop_blocks;                  // the list phase wants every resident warp
     if (grid > s->coop_blocks) grid = s->coop_blocks;
     CellArgs ac = a;
     const double *q0 = s->Q;
-    void *args[] = {&ac, &q0, &s->cell_of, &s->cell_count, &s->cell_start, &s->cell_cursor, &s->cell_tmp, &s->order, &s->rank};
+    RebuildArgs ra{};
+    if (fused) ra = *fused;
+    void *args[] = {&ac, &q0, &s->cell_of, &s->cell_count, &s->cell_start, &s->cell_cursor, &s->cell_tmp, &s->order, &s->rank, &ra};
     QHP_CUDA_OK(s, cudaLaunchCooperativeKernel((const void *)k_cells_fused, dim3(grid), dim3(tb), args, 0, s->stream));
     s->n_launch++;
     return QHP_OK;
@@ -448,6 +497,17 @@ static int list_build(qhp_system *s, const CellArgs &a, bool count_only) {
 
 int qhp_cells_rebuild(qhp_system *s, bool force) {
   const CellArgs a = cell_args(s, force);
+  if (!force && s->coop_blocks > 0 && (s->staged ? s->nbr16 != nullptr : s->nbr != nullptr)) {
+    // the per-step path: the whole chain (cells, contraction, list) as one cooperative launch
+    RebuildArgs ra{};
+    ra.on = 1; ra.Pc = s->Pc; ra.staged = s->staged ? 1 : 0; ra.stride = (int)s->nbr_stride; ra.dummy = s->staged_cap - 1;
+    for (int d = 0; d < 3; ++d) { ra.bx.box[d] = s->box[d]; ra.bx.inv_box[d] = s->inv_box[d]; }
+    ra.Q = s->Q; ra.Tc = s->d_Tc; ra.type = s->dt_.type; ra.molid = s->dt_.molid;
+    ra.pos4 = s->pos4; ra.cent4 = s->cent4; ra.cref = s->cref;
+    ra.nbr16 = s->nbr16; ra.nbr = s->nbr; ra.nbr_count = s->nbr_count; ra.stride32 = s->nbr_stride;
+    ra.counters = (long long *)s->counters;
+    return cells_only(s, a, &ra);
+  }
   int rc = cells_only(s, a);
   if (rc) return rc;
   rc = qhp_nm_contract(s, true, force);

@@ -15,6 +15,7 @@
 #include <algorithm>
 
 #include "qhp_internal.cuh"
+#include "contract.cuh"
 #include "philox.cuh"
 
 template <int P> struct NmTab { double T[P * P]; };   // T[i*P+n], Eq. 2 eigenvectors
@@ -617,52 +618,15 @@ __global__ void k_to_beads(const double *__restrict__ Q, const double *__restric
 // mode 1: write xc_out [Pc][N][3] in atom order (parity hook).
 // `need` (may be NULL): device flag words; the kernel returns at once unless forced or the
 // list-validity statistic exceeds the threshold.
-struct BoxArg { double box[3], inv_box[3]; };
 __global__ void k_contract(const BoxArg bx, const double *__restrict__ Q, int N, int Pc, const double *__restrict__ Tc,
                            const int32_t *__restrict__ rank, const int32_t *__restrict__ type,
                            const int32_t *__restrict__ molid, double *pos4, double *cent4, double *cref,
                            double *xc_out, int mode, const unsigned long long *d2max, double thresh2,
                            long long *counters) {
   if (d2max && __longlong_as_double((long long)*d2max) < thresh2) return;
-  const long long ND = 3LL * N;
   const long long d = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (d >= ND) return;
-  const int atom = (int)(d / 3), c = (int)(d % 3);
-  const double spc = sqrt((double)Pc);
-  const long long slot = rank ? rank[atom] : atom;
-  for (int j = 0; j < Pc; ++j) {
-    double s = 0.0;
-    for (int n = 0; n < Pc; ++n) s += Tc[j * Pc + n] * Q[n * ND + d];
-    const double xc = spc * s;
-    if (mode == 0) {
-      // a list built on the centroids can only cover beads closer than skin/2 to their centroid: the
-      // thread of component 0 tests the NORM of the bead's offset (all three components)
-      if (cent4 && c == 0) {
-        double n2 = (xc - Q[d]) * (xc - Q[d]);
-        for (int cc = 1; cc < 3; ++cc) {
-          double sc = 0.0;
-          for (int n = 0; n < Pc; ++n) sc += Tc[j * Pc + n] * Q[n * ND + d + cc];
-          n2 += (spc * sc - Q[d + cc]) * (spc * sc - Q[d + cc]);
-        }
-        if (n2 > thresh2) counters[6] = 1;
-      }
-      pos4[((long long)j * N + slot) * 4 + c] = xc;
-      if (c == 0) reinterpret_cast<long long *>(pos4)[((long long)j * N + slot) * 4 + 3] = type[atom];
-    } else {
-      xc_out[(long long)j * ND + d] = xc;
-    }
-  }
-  if (mode == 0 && cent4) {
-    const double q0 = Q[d];
-    cent4[slot * 4 + c] = q0;
-    if (c == 0) reinterpret_cast<long long *>(cent4)[slot * 4 + 3] = molid[atom];
-    // fp32 copy: w = molecule id | atom type << 28 (the list entries of the staged pair kernel carry the type)
-    // single-precision copy, wrapped into [0, L), for the pre-test of the list build (cells.cu)
-    float *centf = reinterpret_cast<float *>(cent4 + 4LL * N);
-    centf[slot * 4 + c] = (float)(q0 - bx.box[c] * floor(q0 * bx.inv_box[c]));
-    if (c == 0) reinterpret_cast<int *>(centf)[slot * 4 + 3] = molid[atom] | (type[atom] << 28);
-    cref[d] = q0;
-  }
+  if (d >= 3LL * N) return;
+  qhp_contract_dof(bx, Q, N, Pc, Tc, rank, type, molid, pos4, cent4, cref, xc_out, mode, thresh2, counters, d);
 }
 
 // ---------------------------------------------------------------------------------------------
