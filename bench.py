@@ -350,6 +350,8 @@ def main():
     ap.add_argument("--n-mol", type=int, default=0, help="profiling aid: the same workload on a box of this many waters (0 = the BASELINE.json size)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--shard-beads", action="store_true", help="N > 1: bead-sharded V_s over the ranks (qhp_set_comm, NCCL all-gather of F_s; N must divide P'); "
+                    "strong scaling of ONE replica instead of N independent replicas.  Unmeasured on hardware in this round.")
     ap.add_argument("--no-adqtb", action="store_true", help="skip the adQTB (C3) leg that the default C4 run appends")
     ap.add_argument("--no-amortised", action="store_true", help="skip the untimed 500-step run that measures the list-rebuild rate")
     args = ap.parse_args()
@@ -386,6 +388,9 @@ def main():
         cfg["n_mol"] = args.n_mol
     top, sysg, x0, p0 = build_system(cfg)
     N, P, K = top["n_atoms"], cfg["P"], args.steps
+    sharded = args.shard_beads and world > 1 and cfg["P_contract"] % world == 0
+    if sharded:
+        sysg.set_comm(rank, world)
     if args.a_block != "exact":
         sysg.set_a_block(args.a_block)
     if args.n_alt > 1:
@@ -417,7 +422,7 @@ def main():
     # ---- adQTB leg (C3: 216,000 atoms, one whole 1024-step segment: noise generation, 1024 steps, spectra +
     #      adaptation), appended to the default run so that one driver run measures both halves of the metric ----
     adqtb = None
-    if args.workload == "C4" and not args.no_adqtb and args.n_mol == 0 and args.n_alt == 1:
+    if args.workload == "C4" and not args.no_adqtb and args.n_mol == 0 and args.n_alt == 1 and not sharded:
         c3 = workload("C3")
         top3, sys3, x3, p3 = build_system(c3)
         K3 = c3["n_seg"]
@@ -450,12 +455,14 @@ def main():
     roofline = dict(pair_block, note="achieved counts each unordered in-cutoff pair-bead once (110 flop); the kernel "
                                      "evaluates both directions (full list, no atomics), see executed_tflops; "
                                      "peak_measured = live qhp_dfma_probe")
+    if sharded:                                   # one replica on all ranks: the job advanced N*P bead-atoms per step, not world times that
+        m["value"] /= world
     line = dict(metric="bead_atom_steps_per_s", value=m["value"], unit="bead-atom-steps/s", n_gpus=world, steps=K,
-                warmup=args.warmup, ms_per_step=m["ms"] / K, higher_is_better=True, scaling="weak", vs_baseline=None,
+                warmup=args.warmup, ms_per_step=m["ms"] / K, higher_is_better=True, scaling="strong" if sharded else "weak", vs_baseline=None,
                 dtype="f64", data="synthetic",
                 config=dict(workload=cfg["name"], n_atoms=N, P=P, P_contract=cfg["P_contract"], dt_fs=cfg["dt_fs"],
                             thermostat=cfg["thermostat"], n_alt=args.n_alt, a_block=args.a_block, ns_per_day=m["ns_day"],
-                            parallelism="independent replicas (no data-path collective)" if world > 1 else "1 GPU",
+                            parallelism=("bead-sharded V_s, all-gather of F_s per step" if sharded else "independent replicas (no data-path collective)") if world > 1 else "1 GPU",
                             l2="inputs larger than L2 (state + neighbour table >> 126 MB)" if N > 100000 else "inputs smaller than L2",
                             pair_beads_in_cutoff=m["c1"]["pair_beads_in_cutoff"], list_entries=m["c1"]["list_entries"]),
                 clocks=m["clocks"], e2e=e2e, gpu_launches=m["launches"],

@@ -26,6 +26,7 @@
 #ifndef QHP_H
 #define QHP_H
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -134,6 +135,26 @@ int qhp_set_contraction(qhp_system *sys, int variant);
 #define QHP_ABLOCK_EXACT 0
 #define QHP_ABLOCK_CAYLEY 1
 int qhp_set_a_block(qhp_system *sys, int kind);
+
+/* Bead-parallel evaluation of V_s over several processes, one GPU each (Sec. III.C: the beads of
+ * the -- contracted -- ring polymer are distributed over the ranks of a "polymer" communicator, each rank evaluates
+ * the forces of its beads, the forces are gathered and then projected on the normal modes, l.192, l.195).  Every rank
+ * holds the whole system and runs the same qhp_* calls (the integrator pass is replicated, so the copies stay
+ * bit-identical); after qhp_set_comm(sys, rank, world, fn, ctx) the pair kernel of rank r evaluates the contracted
+ * beads [r P'/world, (r + 1) P'/world) only, and the library calls
+ *     fn(ctx, Fs, bytes_per_rank, rank, world, cuda_stream)
+ * once per V_s evaluation: an IN-PLACE all-gather of the DEVICE buffer Fs (world consecutive blocks of bytes_per_rank
+ * bytes, block r valid on rank r on entry, all blocks valid on every rank on return), enqueued on cuda_stream (the
+ * stream of qhp_create); return 0 on success.  The caller owns the communicator (NCCL all-gather over NVLink in
+ * the Python binding: torch.distributed.all_gather_into_tensor).  world must divide P_contract; world = 1 (or fn =
+ * NULL) restores the single-process path.  Observables and the counters hook evaluate every bead locally.  Call before
+ * qhp_set_state.  QHP_EINVAL for rank/world out of range or world not dividing P_contract. */
+typedef int (*qhp_allgather_fn)(void *ctx, void *device_buf, size_t bytes_per_rank, int rank, int world, void *cuda_stream);
+int qhp_set_comm(qhp_system *sys, int rank, int world, qhp_allgather_fn fn, void *ctx);
+/* Test hook of the bead slicing: overwrites the slow forces F_s with NaN, then evaluates them in n_slices bead
+ * slices, one launch after the other (the launches ranks 0..n_slices-1 would make); F_s, hence qhp_forces, must
+ * afterwards equal the unsliced result bit for bit.  n_slices must divide P_contract. */
+int qhp_pair_slices(qhp_system *sys, int n_slices);
 
 /* Bead-space forces at the current positions, device [P][n_atoms][3]:
  * G_i = -grad V_f(x_i) + (P/P') sum_j C_ji (-grad V_s(xc_j))  (Eq. 10-11 and chain rule on Eq. 20). */

@@ -18,7 +18,32 @@ SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_respa", "qhp_set_a_block", "qhp
            "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
            "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma", "qhp_adqtb_ratio", "qhp_adqtb_kappa",
            "qhp_adqtb_segment", "qhp_counters", "qhp_profile", "qhp_profile_read", "qhp_check", "qhp_last_error", "qhp_philox_normals",
-           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar"]
+           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar", "qhp_set_comm", "qhp_pair_slices"]
+
+
+# int fn(void *ctx, void *device_buf, size_t bytes_per_rank, int rank, int world, void *cuda_stream)  (include/qhp.h)
+ALLGATHER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_size_t, C.c_int, C.c_int, C.c_void_p)
+
+
+def allgather_inplace(buf, rank: int, world: int, group=None):
+    """In-place all-gather of a flat tensor of `world` equal blocks (block `rank` valid on entry) over
+    torch.distributed: NCCL for CUDA tensors (the data-path collective of the bead-sharded V_s), gloo for the
+    host-side tests.  Argument marshalling only."""
+    import torch.distributed as dist
+    n = buf.numel() // world
+    dist.all_gather_into_tensor(buf, buf[rank * n:(rank + 1) * n].clone(), group=group)
+    return buf
+
+
+class _DevMem:
+    """A raw device allocation of the library seen through __cuda_array_interface__ (no copy)."""
+
+    def __init__(self, ptr: int, n: int):
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (int(ptr), False), "version": 2}
+
+
+def _wrap_device_f64(ptr: int, n: int):
+    return _torch().as_tensor(_DevMem(ptr, n), device="cuda")
 
 
 class QhpError(RuntimeError):
@@ -68,6 +93,8 @@ def lib():
         L.qhp_set_a_block.argtypes = [vp, i32]
         L.qhp_set_contraction.argtypes = [vp, i32]
         L.qhp_forces.argtypes = [vp, vp]
+        L.qhp_set_comm.argtypes = [vp, i32, i32, ALLGATHER_FN, vp]
+        L.qhp_pair_slices.argtypes = [vp, i32]
         L.qhp_observables.argtypes = [vp, vp, i32]
         L.qhp_observables_host.argtypes = [vp, vp, i32]
         L.qhp_neighbor_lists.argtypes = [vp, vp, vp, vp, vp]
@@ -220,6 +247,32 @@ class System:
         if k.shape != (self.n_seg + 1,):
             raise ValueError("kappa: one value per frequency omega_j, j = 0..n_seg")
         self._ok(self._L.qhp_adqtb_kappa(self._h, k.ctypes.data_as(C.c_void_p)))
+
+    def set_comm(self, rank: int, world: int, group=None):
+        """Bead-sharded V_s over `world` processes: this rank evaluates P'/world contracted beads,
+        the slow forces are all-gathered through torch.distributed (NCCL) on the library's stream.  Before set_state."""
+        torch = _torch()
+        if world <= 1:
+            self._ok(self._L.qhp_set_comm(self._h, 0, 1, ALLGATHER_FN(0), None))
+            self._comm_cb = None
+            return
+        stream = self.stream
+
+        def cb(ctx, ptr, nbytes, rk, wd, cuda_stream):
+            try:
+                n = nbytes * wd // 8
+                buf = _wrap_device_f64(ptr, n)
+                with torch.cuda.stream(stream):
+                    allgather_inplace(buf, rk, wd, group)
+                return 0
+            except Exception:
+                return 1
+        self._comm_cb = ALLGATHER_FN(cb)          # keep the callback alive as long as the system
+        self._ok(self._L.qhp_set_comm(self._h, int(rank), int(world), self._comm_cb, None))
+
+    def pair_slices(self, n_slices: int):
+        """Test hook: F_s re-evaluated in n_slices bead slices (include/qhp.h)."""
+        self._ok(self._L.qhp_pair_slices(self._h, int(n_slices)))
 
     def set_respa(self, n_alt: int):
         self._ok(self._L.qhp_set_respa(self._h, int(n_alt)))

@@ -14,6 +14,7 @@
 
 struct PairArgs {
   int N, Pc, nt;
+  int bead0, bead_end;      // this launch evaluates the contracted beads [bead0, bead_end)
   const double *pos4;       // [Pc][N] (x, y, z, type bits)
   double *Fs;               // [Pc][N][3]
   const int32_t *nbr, *nbr_count;
@@ -33,7 +34,7 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs a) {
   const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long i = gid / L;
   const int sub = (int)(gid % L);
-  const int b0 = blockIdx.y * NB;
+  const int b0 = a.bead0 + blockIdx.y * NB;
   const bool active = i < a.N;
 
   double xi[NB][3], F[NB][3];
@@ -44,7 +45,7 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs a) {
   for (int b = 0; b < NB; ++b) {
     F[b][0] = F[b][1] = F[b][2] = 0.0;
     xi[b][0] = xi[b][1] = xi[b][2] = 0.0;
-    if (active && b0 + b < a.Pc) {
+    if (active && b0 + b < a.bead_end) {
       const double4 p = reinterpret_cast<const double4 *>(a.pos4)[(long long)(b0 + b) * a.N + i];
       xi[b][0] = p.x; xi[b][1] = p.y; xi[b][2] = p.z;
       ti = (int)__double_as_longlong(p.w);
@@ -57,7 +58,7 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs a) {
       const int j = row[k];
 #pragma unroll
       for (int b = 0; b < NB; ++b) {
-        if (b0 + b < a.Pc) {
+        if (b0 + b < a.bead_end) {
           const double4 pj = reinterpret_cast<const double4 *>(a.pos4)[(long long)(b0 + b) * a.N + j];
           double dx = xi[b][0] - pj.x, dy = xi[b][1] - pj.y, dz = xi[b][2] - pj.z;
           dx = fma(-a.box[0], rint(dx * a.inv_box[0]), dx);
@@ -96,7 +97,7 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs a) {
   if (active && sub == 0) {
 #pragma unroll
     for (int b = 0; b < NB; ++b)
-      if (b0 + b < a.Pc) {
+      if (b0 + b < a.bead_end) {
         double *o = a.Fs + ((long long)(b0 + b) * a.N + i) * 3;
         o[0] = F[b][0]; o[1] = F[b][1]; o[2] = F[b][2];
       }
@@ -150,7 +151,7 @@ int qhp_pair_geometry(const qhp_system *s, int *NB_out, int *L_out, unsigned *gx
 }
 
 int qhp_pair_staged_partials(const qhp_system *s);
-int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned long long *count);
+int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned long long *count, int bead0, int nbeads);
 
 // upper bound of the per-CTA energy partials of either kernel (sizes s->red)
 int qhp_pair_partials(const qhp_system *s) {
@@ -160,15 +161,15 @@ int qhp_pair_partials(const qhp_system *s) {
   return n > m ? n : m;
 }
 
-int qhp_pair_forces(qhp_system *s, bool energy) {
+int qhp_pair_forces_beads(qhp_system *s, bool energy, int bead0, int nbeads) {
   if (energy) {
     QHP_CUDA_OK(s, cudaMemsetAsync(&s->counters[3], 0, sizeof(int64_t), s->stream));
     QHP_CUDA_OK(s, cudaMemsetAsync(s->red + 4 * (size_t)s->n_tiles, 0, sizeof(double) * (size_t)qhp_pair_partials(s), s->stream));
   }
   if (s->staged)
-    return qhp_pair_staged_forces(s, energy, s->red + 4 * (size_t)s->n_tiles, (unsigned long long *)&s->counters[3]);
+    return qhp_pair_staged_forces(s, energy, s->red + 4 * (size_t)s->n_tiles, (unsigned long long *)&s->counters[3], bead0, nbeads);
   PairArgs a{};
-  a.N = s->N; a.Pc = s->Pc; a.nt = s->nt;
+  a.N = s->N; a.Pc = s->Pc; a.nt = s->nt; a.bead0 = bead0; a.bead_end = bead0 + nbeads;
   a.pos4 = s->pos4; a.Fs = s->Fs; a.nbr = s->nbr; a.nbr_count = s->nbr_count; a.stride = s->nbr_stride;
   a.pair_tab = s->pair_tab;
   for (int d = 0; d < 3; ++d) { a.box[d] = s->box[d]; a.inv_box[d] = s->inv_box[d]; }
@@ -179,6 +180,7 @@ int qhp_pair_forces(qhp_system *s, bool energy) {
   a.fshift = erfc(al * rc) / (rc * rc) + a.two_a_sqrtpi * exp(-al * al * rc * rc) / rc;
   int NB, L; unsigned gx, gy;
   qhp_pair_geometry(s, &NB, &L, &gx, &gy);
+  gy = (unsigned)((nbeads + NB - 1) / NB);           // bead chunks of this slice
   a.part = s->red + 4 * (size_t)s->n_tiles;
   a.count = (unsigned long long *)&s->counters[3];
   const dim3 grid(gx, gy);
@@ -189,5 +191,22 @@ int qhp_pair_forces(qhp_system *s, bool energy) {
     default: launch_pair_L<1>(L, a, grid, 128, smem, s->stream, energy); break;
   }
   QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+// V_s forces of all contracted beads.  After qhp_set_comm (world > 1) this rank evaluates its own bead slice and the
+// ranks exchange the slices: F_s is bead-major, so every rank's slice is one contiguous block and the exchange is one
+// in-place all-gather on the library's stream (forces gathered over the polymer communicator, then
+// projected).  The energy variant (observables, counters) always evaluates every bead locally.
+int qhp_pair_forces(qhp_system *s, bool energy) {
+  if (energy || s->shard_world <= 1) return qhp_pair_forces_beads(s, energy, 0, s->Pc);
+  const int nb = s->Pc / s->shard_world;
+  int rc = qhp_pair_forces_beads(s, false, s->shard_rank * nb, nb);
+  if (rc) return rc;
+  const size_t bytes = sizeof(double) * 3 * (size_t)s->N * nb;
+  if (s->shard_allgather(s->shard_ctx, s->Fs, bytes, s->shard_rank, s->shard_world, (void *)s->stream) != 0) {
+    s->err = "qhp_set_comm: the all-gather callback failed";
+    return QHP_ECUDA;
+  }
   return QHP_OK;
 }

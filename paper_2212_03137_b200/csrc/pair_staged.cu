@@ -39,6 +39,7 @@
 
 struct StagedArgs {
   int N, Pc, nt, split, cap;     // cap - 1 = dummy staged atom (infinitely far): target of the row padding
+  int bead0;                     // first contracted bead of this launch (grid.y beads from here: bead slices, qhp_set_comm)
   int nc[3];
   double box[3], inv_box[3], cell_edge[3];
   const double *pos4;            // [Pc][N] (x, y, z, type bits), slot order
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   __shared__ double su[STG_MAX_WARPS];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = blockDim.x;
-  const int cell = blockIdx.x / a.split, part = blockIdx.x % a.split, bead = blockIdx.y;
+  const int cell = blockIdx.x / a.split, part = blockIdx.x % a.split, bead = a.bead0 + blockIdx.y;
   const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
 
   for (int k = tid; k < a.nt * a.nt * 4; k += nthr) {      // (qq, 4 eps, sigma^2, shift) -> (24 eps, sigma^2, qq, shift)
@@ -421,8 +422,9 @@ bool qhp_pair_staged_fit(qhp_system *s, long long region) {
   return false;
 }
 
-int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned long long *count) {
+int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned long long *count, int bead0, int nbeads) {
   StagedArgs a{};
+  a.bead0 = bead0;
   a.N = s->N; a.Pc = s->Pc; a.nt = s->nt; a.split = s->staged_split; a.cap = s->staged_cap;
   for (int d = 0; d < 3; ++d) {
     a.nc[d] = s->nc[d]; a.box[d] = s->box[d]; a.inv_box[d] = s->inv_box[d];
@@ -450,7 +452,7 @@ int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned lo
       if (s->lj_eps[t] > 0 && s->lj_eps[u] > 0) a.lj_mask[t] |= 1u << u;
   }
   a.part = part; a.count = count; a.counters = (long long *)s->counters;
-  const dim3 grid((unsigned)(s->ncell * s->staged_split), (unsigned)s->Pc);
+  const dim3 grid((unsigned)(s->ncell * s->staged_split), (unsigned)nbeads);
   const size_t smem = staged_smem_bytes(s->staged_cap, s->staged_warps, s->staged_f32);
   const int threads = 32 * s->staged_warps;
   if (s->staged_f32) {

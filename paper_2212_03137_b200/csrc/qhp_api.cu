@@ -481,6 +481,35 @@ extern "C" int qhp_set_a_block(qhp_system *s, int kind) {
   return QHP_OK;
 }
 
+extern "C" int qhp_set_comm(qhp_system *s, int rank, int world, qhp_allgather_fn fn, void *ctx) {
+  if (!s) return QHP_EINVAL;
+  if (world < 1 || rank < 0 || rank >= world || s->Pc % world != 0) { s->err = "qhp_set_comm: 0 <= rank < world and world must divide P_contract"; return QHP_EINVAL; }
+  if (s->have_state) { s->err = "qhp_set_comm: call before qhp_set_state"; return QHP_ESTATE; }
+  if (world == 1 || !fn) { s->shard_rank = 0; s->shard_world = 1; s->shard_allgather = nullptr; s->shard_ctx = nullptr; return QHP_OK; }
+  s->shard_rank = rank; s->shard_world = world; s->shard_allgather = fn; s->shard_ctx = ctx;
+  return QHP_OK;
+}
+
+__global__ void k_fill_nan(double *p, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = __longlong_as_double(0x7ff8000000000000LL);
+}
+
+extern "C" int qhp_pair_slices(qhp_system *s, int n_slices) {
+  if (!s) return QHP_EINVAL;
+  if (!s->have_state) { s->err = "no state"; return QHP_ESTATE; }
+  if (n_slices < 1 || s->Pc % n_slices != 0) { s->err = "n_slices must divide P_contract"; return QHP_EINVAL; }
+  const long long n = 3LL * s->N * s->Pc;
+  k_fill_nan<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(s->Fs, n);
+  QHP_LAUNCH_OK(s);
+  const int nb = s->Pc / n_slices;
+  for (int r = 0; r < n_slices; ++r) {
+    const int rc = qhp_pair_forces_beads(s, false, r * nb, nb);
+    if (rc) return rc;
+  }
+  return QHP_OK;
+}
+
 extern "C" int qhp_forces(qhp_system *s, double *f_beads) {
   if (!s || !f_beads) return QHP_EINVAL;
   if (!s->have_state) { s->err = "no state"; return QHP_ESTATE; }

@@ -129,6 +129,12 @@ struct qhp_system {
   double *kappa = nullptr;                 // [n_seg+1] kernel-correction factor on H (reading G11); NULL: 1
   bool ratio_started = false;
 
+  // ---- bead-sharded V_s (qhp_set_comm): this rank evaluates the contracted beads
+  //      [rank Pc/world, (rank + 1) Pc/world) and the ranks all-gather F_s (bead-major: one contiguous block each) ----
+  int shard_rank = 0, shard_world = 1;
+  qhp_allgather_fn shard_allgather = nullptr;
+  void *shard_ctx = nullptr;
+
   // ---- per-phase profiling (qhp_profile) ----
   bool prof = false;
   std::vector<cudaEvent_t> prof_ev;      // flat list of (begin, end) pairs
@@ -158,7 +164,8 @@ int qhp_cells_rebuild(qhp_system *s, bool force);   // early-exits on device unl
 int qhp_cells_setup(qhp_system *s);                 // cooperative-launch capacity of the fused cell kernel
 int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, int64_t *total_host);
 // pair.cu
-int qhp_pair_forces(qhp_system *s, bool energy);     // pos4 -> Fs (+ U_s, count into obs/counters)
+int qhp_pair_forces(qhp_system *s, bool energy);     // pos4 -> Fs (+ U_s, count into obs/counters); bead-sharded if qhp_set_comm
+int qhp_pair_forces_beads(qhp_system *s, bool energy, int bead0, int nbeads);   // the launch of one bead slice
 int qhp_pair_setup(qhp_system *s);                   // polynomial tables, staged-kernel geometry
 bool qhp_pair_staged_fit(qhp_system *s, long long region);  // CTA size / capacity for a neighbourhood size
 int qhp_pair_partials(const qhp_system *s);          // upper bound of per-CTA energy partials

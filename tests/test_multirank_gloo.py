@@ -64,3 +64,39 @@ def test_reference_arm_only_rank0_prints():
     line = json.loads(p.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+SHARD_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch
+import torch.distributed as dist
+from paper_2212_03137_b200.binding import allgather_inplace
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:{port}", rank=int(sys.argv[1]), world_size=2)
+rank, world = dist.get_rank(), 2
+# F_s is bead-major [P'][N][3]: with P' = 4 beads on 2 ranks, rank r owns beads 2r, 2r+1 = one contiguous block
+Pc, N = 4, 5
+full = torch.arange(Pc * N * 3, dtype=torch.float64) * 0.5 + 1.0
+buf = torch.full((Pc * N * 3,), float("nan"), dtype=torch.float64)
+n = buf.numel() // world
+buf[rank * n:(rank + 1) * n] = full[rank * n:(rank + 1) * n]        # the slice this rank "computed"
+allgather_inplace(buf, rank, world)
+dist.barrier()
+print(json.dumps(dict(rank=rank, equal=bool(torch.equal(buf, full)))))
+dist.destroy_process_group()
+"""
+
+
+def test_bead_slice_allgather_two_processes(tmp_path):
+    """The exchange step of the bead-sharded V_s (qhp_set_comm): every rank contributes the contiguous
+    bead-major block of its contracted beads, afterwards every rank holds all of F_s.  Host buffers, gloo; on GPUs
+    the same call runs over NCCL inside the callback of the library."""
+    port = 31500 + os.getpid() % 2000
+    script = tmp_path / "shard_worker.py"
+    script.write_text(SHARD_WORKER.format(root=ROOT, port=port))
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)
+             for r in range(2)]
+    for p in procs:
+        out, err = p.communicate(timeout=120)
+        assert p.returncode == 0, err
+        assert json.loads(out.strip().splitlines()[-1])["equal"]
