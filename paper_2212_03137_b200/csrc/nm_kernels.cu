@@ -448,38 +448,63 @@ __global__ void __launch_bounds__(128) k_integrate_mol1(const IntArgs a, int n_m
         const double k = a.tether_k[a.type[s0 + al]];
         acc4(f, al, -k * x[3 * al], -k * x[3 * al + 1], -k * x[3 * al + 2]);
       }
-    // every position of the molecule has been read: update its atoms in place
+    // every position of the molecule has been read: update its atoms in place.  Two sweeps: all loads of the
+    // molecule first (independent, so their latencies overlap; the kernel has one thread per molecule and is
+    // latency-bound), then the arithmetic and the stores.
+    int ty_[4];
+    long long slot_[4], segb_[4];
+    double q_[4][3], p_[4][3], fs_[4][3], fc_[4][3], cr_[4][3];
 #pragma unroll
     for (int al = 0; al < 4; ++al) {
       if (al >= na) break;
       const int atom = s0 + al;
-      const int ty = a.type[atom];
-      const double mass = a.mass[ty];
-      const long long slot = a.rank[atom];
+      ty_[al] = __ldg(a.type + atom);
+      slot_[al] = __ldg(a.rank + atom);
+      segb_[al] = THERMO == 2 ? qhp_seg_addr(__ldg(a.seg_slot + atom), a.n_seg, a.n_loc) : 0;
+    }
+#pragma unroll
+    for (int al = 0; al < 4; ++al) {
+      if (al >= na) break;
+      const int atom = s0 + al;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const long long dof = 3LL * atom + c;
+        q_[al][c] = a.Q[dof]; p_[al][c] = a.Pm[dof];
+        fs_[al][c] = __ldg(a.Fs + slot_[al] * 3 + c);
+        fc_[al][c] = (THERMO == 2 && a.do_step) ? __ldg(a.Fc + segb_[al] + c) : 0.0;
+        cr_[al][c] = a.do_step ? __ldg(a.cref + dof) : 0.0;
+      }
+    }
+#pragma unroll
+    for (int al = 0; al < 4; ++al) {
+      if (al >= na) break;
+      const int atom = s0 + al;
+      const int ty = ty_[al];
+      const double mass = __ldg(a.mass + ty);
+      const long long slot = slot_[al];
       const double *cf = a.coef + ty * QHP_NCOEF;
       double z[3] = {0.0, 0.0, 0.0};
       if (THERMO == 1 && a.do_step) qhp_normals3(a.seed, (uint32_t)atom, 0u, QHP_TAG_PILE, (uint64_t)a.step, z);
       double dsum = 0.0;
-      const long long segb = THERMO == 2 ? qhp_seg_addr(a.seg_slot[atom], a.n_seg, a.n_loc) : 0;
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         const long long dof = 3LL * atom + c;
-        double q = a.Q[dof], p = a.Pm[dof];
-        p += a.w_fast * f[al][c] + a.w_slow * a.Fs[slot * 3 + c];
+        double q = q_[al][c], p = p_[al][c];
+        p += a.w_fast * f[al][c] + a.w_slow * fs_[al][c];
         if (a.do_step) {
           q += a.hdt * p / mass;
           if (THERMO == 1) {
             p = __ldg(cf + 3) * p + __ldg(cf + 4) * z[c];
           } else if (THERMO == 2) {
-            const long long k = segb + c;
-            const double pn = a.qa * p + a.qbA * a.Fc[k];
+            const long long k = segb_[al] + c;
+            const double pn = a.qa * p + a.qbA * fc_[al][c];
             a.vseg[k] = (p + pn) / (2.0 * mass);
             p = pn;
           }
           q += a.hdt * p / mass;
           a.Q[dof] = q;
           a.pos4[slot * 4 + c] = q;
-          const double dd = q - a.cref[dof];
+          const double dd = q - cr_[al][c];
           dsum += dd * dd;
         }
         a.Pm[dof] = p;
