@@ -24,9 +24,6 @@
 // consecutive elements (all other accesses) inside one aligned 128-byte row.  No extra memory.
 #define FPAD(i) ((i) ^ ((((i) >> 3) ^ ((i) >> 6)) & 7))
 #define FPAD_LEN(n) (n)
-#ifndef NOISE_LB
-#define NOISE_LB 1
-#endif
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
   return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
@@ -248,9 +245,8 @@ __global__ void k_qtb_spectrum4(int nt, int n_seg, const double *__restrict__ hk
   H4[idx] = make_double2(re, im);
 }
 
-// white noise of one pass of k_qtb_noise into the transform buffer (own function: the constants of the
-// Box-Muller evaluation must not stay live across the transforms, which need every register)
-__device__ __noinline__ void qtb_fill_noise(double2 *nbuf, double *zb, int nf, int nw, int n_seg, int pass, int atom,
+// white noise of one pass of k_qtb_noise into the transform buffer
+__device__ __forceinline__ void qtb_fill_noise(double2 *nbuf, double *zb, int nf, int nw, int n_seg, int pass, int atom,
                                             unsigned long long seed, long long seg, int t, int nthr) {
   for (int m = t; m < nf; m += nthr) {
     double2 v = make_double2(0.0, 0.0);
@@ -275,7 +271,7 @@ __device__ __noinline__ void qtb_fill_noise(double2 *nbuf, double *zb, int nf, i
 //   F_c[dof][n] = sum_k h_z[k] r(dof, seg*n_seg + n - k + n_seg),  n = 0..n_seg-1
 // Output: the 48-byte half row of the pair in the segment layout [group][n_seg][12].
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NOISE_LB == 1 ? 512 : 256, 1) k_qtb_noise(int n_seg, unsigned long long seed, long long seg, const int32_t *__restrict__ slot_atom,
+__global__ void __launch_bounds__(512, 1) k_qtb_noise(int n_seg, unsigned long long seed, long long seg, const int32_t *__restrict__ slot_atom,
                                                    const int32_t *__restrict__ type, const double2 *__restrict__ H4,
                                                    const double2 *__restrict__ tw, double *Fc) {
   extern __shared__ double2 nbuf[];
