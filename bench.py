@@ -53,8 +53,8 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_staged<false> launch (per launch, like `achieved`) and the
 # `ncu --set full` capture it was read from; refreshed whenever the kernel changes (the value is a property of that
 # capture, not of this run: `traffic_source` says which)
-NCU_TRAFFIC = {("C4", "k_pair_staged"): (1.3637e9 + 2.39e7, "profiles/r1d_summary.md (round-1 kernel; refresh pending)"),
-               ("C3", "k_pair_staged"): (3.409e8 + 9.5e6, "profiles/r1d_summary.md (round-1 kernel; refresh pending)")}
+NCU_TRAFFIC = {("C4", "k_pair_staged"): (1.363542e9 + 2.4354e7, "profiles/r2_summary.md (prof_r2_hot, ncu --set full)"),
+               ("C3", "k_pair_staged"): (3.409152e8 + 7.760e6, "profiles/r2_summary.md (prof_r2_c3, ncu --set full)")}
 
 
 def measure_dfma_peak() -> float:
