@@ -31,21 +31,37 @@ __device__ __forceinline__ bool cells_skip(const CellArgs &a) {
   return a.flag && __longlong_as_double((long long)*a.flag) < a.thresh2;
 }
 
-__global__ void k_cells_assign(const CellArgs a, const double *__restrict__ Q0, int32_t *cell_of, int32_t *cell_count) {
+// Order INSIDE a cell (internal slot order only; the canonical `order` of the parity hook breaks ties by atom index):
+// 9-bit Morton code of the atom's position within its cell (8 x 8 x 8 sub-cells), then atom index.  Atoms that are
+// neighbours in space become neighbours in slot order, so the staged records a warp of the pair kernel gathers for
+// one atom come in runs of consecutive 16-byte records instead of scattered ones (shared-memory bank conflicts).
+__device__ __forceinline__ int cell_subkey(double fx, double fy, double fz) {   // fractions in [0, 1)
+  const int a = min((int)(fx * 8.0), 7), b = min((int)(fy * 8.0), 7), c = min((int)(fz * 8.0), 7);
+  int k = 0;
+#pragma unroll
+  for (int bit = 0; bit < 3; ++bit) k |= (((a >> bit) & 1) << (3 * bit + 2)) | (((b >> bit) & 1) << (3 * bit + 1)) | (((c >> bit) & 1) << (3 * bit));
+  return k;
+}
+
+__global__ void k_cells_assign(const CellArgs a, const double *__restrict__ Q0, int32_t *cell_of, int32_t *cell_count, int32_t *cell_key) {
   if (cells_skip(a)) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= a.N) return;
   int q[3];
+  double fr[3];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     double s = __dmul_rn(Q0[3LL * i + d], a.inv_box[d]);
     s = __dsub_rn(s, floor(s));
-    int v = (int)__dmul_rn(s, (double)a.nc[d]);
+    const double sn = __dmul_rn(s, (double)a.nc[d]);
+    int v = (int)sn;
     if (v > a.nc[d] - 1) v = a.nc[d] - 1;
     q[d] = v;
+    fr[d] = fmin(fmax(sn - v, 0.0), 0.999999);
   }
   const int cell = (q[0] * a.nc[1] + q[1]) * a.nc[2] + q[2];
   cell_of[i] = cell;
+  cell_key[i] = cell_subkey(fr[0], fr[1], fr[2]);
   atomicAdd(&cell_count[cell], 1);
 }
 
@@ -86,16 +102,21 @@ __global__ void k_cells_fill(const CellArgs a, const int32_t *__restrict__ cell_
 }
 
 // stable order inside each cell: slot = cell_start + #{members with a smaller atom index}
+// key == NULL: the canonical order (ties by atom index; parity hook), rank may be NULL then
 __global__ void k_cells_rank(const CellArgs a, const int32_t *__restrict__ cell_of, const int32_t *__restrict__ cell_start,
-                             const int32_t *__restrict__ tmp, int32_t *order, int32_t *rank) {
+                             const int32_t *__restrict__ tmp, const int32_t *__restrict__ key, int32_t *order, int32_t *rank) {
   if (cells_skip(a)) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= a.N) return;
   const int c = cell_of[i], b = cell_start[c], e = cell_start[c + 1];
+  const int ki = key ? key[i] : 0;
   int cnt = 0;
-  for (int k = b; k < e; ++k) cnt += (tmp[k] < i);
+  for (int k = b; k < e; ++k) {
+    const int j = tmp[k], kj = key ? key[j] : 0;
+    cnt += (kj < ki) || (kj == ki && j < i);
+  }
   order[b + cnt] = i;
-  rank[i] = b + cnt;
+  if (rank) rank[i] = b + cnt;
 }
 
 // Is slot k a list neighbour of the slot whose centroid is ci / fi?  The decision is the canonical
@@ -379,23 +400,27 @@ struct RebuildArgs {
 };
 __global__ void __launch_bounds__(256) k_cells_fused(const CellArgs a, const double *__restrict__ Q0, int32_t *cell_of,
                                                      int32_t *cell_count, int32_t *cell_start, int32_t *cursor,
-                                                     int32_t *tmp, int32_t *order, int32_t *rank, const RebuildArgs ra) {
+                                                     int32_t *tmp, int32_t *order, int32_t *rank, int32_t *cell_key, const RebuildArgs ra) {
   if (cells_skip(a)) return;                       // uniform over the grid: nobody reaches a barrier
   namespace cg = cooperative_groups;
   cg::grid_group grid = cg::this_grid();
   const int nthreads = gridDim.x * blockDim.x, t0 = blockIdx.x * blockDim.x + threadIdx.x;
   for (int i = t0; i < a.N; i += nthreads) {       // assign
     int q[3];
+    double fr[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
       double sc = __dmul_rn(Q0[3LL * i + d], a.inv_box[d]);
       sc = __dsub_rn(sc, floor(sc));
-      int v = (int)__dmul_rn(sc, (double)a.nc[d]);
+      const double sn = __dmul_rn(sc, (double)a.nc[d]);
+      int v = (int)sn;
       if (v > a.nc[d] - 1) v = a.nc[d] - 1;
       q[d] = v;
+      fr[d] = fmin(fmax(sn - v, 0.0), 0.999999);
     }
     const int cell = (q[0] * a.nc[1] + q[1]) * a.nc[2] + q[2];
     cell_of[i] = cell;
+    cell_key[i] = cell_subkey(fr[0], fr[1], fr[2]);
     atomicAdd(&cell_count[cell], 1);
   }
   grid.sync();
@@ -426,9 +451,12 @@ __global__ void __launch_bounds__(256) k_cells_fused(const CellArgs a, const dou
   for (int i = t0; i < a.N; i += nthreads) tmp[atomicAdd(&cursor[cell_of[i]], 1)] = i;   // fill
   grid.sync();
   for (int i = t0; i < a.N; i += nthreads) {       // stable order inside each cell
-    const int c = cell_of[i], b = cell_start[c], e = cell_start[c + 1];
+    const int c = cell_of[i], b = cell_start[c], e = cell_start[c + 1], ki = cell_key[i];
     int cnt = 0;
-    for (int k = b; k < e; ++k) cnt += (tmp[k] < i);
+    for (int k = b; k < e; ++k) {
+      const int j = tmp[k], kj = cell_key[j];
+      cnt += (kj < ki) || (kj == ki && j < i);
+    }
     order[b + cnt] = i;
     rank[i] = b + cnt;
   }
@@ -460,19 +488,19 @@ static int cells_only(qhp_system *s, const CellArgs &a, const RebuildArgs *fused
     const double *q0 = s->Q;
     RebuildArgs ra{};
     if (fused) ra = *fused;
-    void *args[] = {&ac, &q0, &s->cell_of, &s->cell_count, &s->cell_start, &s->cell_cursor, &s->cell_tmp, &s->order, &s->rank, &ra};
+    void *args[] = {&ac, &q0, &s->cell_of, &s->cell_count, &s->cell_start, &s->cell_cursor, &s->cell_tmp, &s->order, &s->rank, &s->cell_key, &ra};
     QHP_CUDA_OK(s, cudaLaunchCooperativeKernel((const void *)k_cells_fused, dim3(grid), dim3(tb), args, 0, s->stream));
     s->n_launch++;
     return QHP_OK;
   }
   const int tb = 256, grid = (s->N + tb - 1) / tb;
-  k_cells_assign<<<grid, tb, 0, s->stream>>>(a, s->Q, s->cell_of, s->cell_count);
+  k_cells_assign<<<grid, tb, 0, s->stream>>>(a, s->Q, s->cell_of, s->cell_count, s->cell_key);
   QHP_LAUNCH_OK(s);
   k_scan_excl<<<1, 1024, 0, s->stream>>>(a, s->cell_count, s->cell_start, s->cell_cursor, s->ncell, 1);
   QHP_LAUNCH_OK(s);
   k_cells_fill<<<grid, tb, 0, s->stream>>>(a, s->cell_of, s->cell_cursor, s->cell_tmp);
   QHP_LAUNCH_OK(s);
-  k_cells_rank<<<grid, tb, 0, s->stream>>>(a, s->cell_of, s->cell_start, s->cell_tmp, s->order, s->rank);
+  k_cells_rank<<<grid, tb, 0, s->stream>>>(a, s->cell_of, s->cell_start, s->cell_tmp, s->cell_key, s->order, s->rank);
   QHP_LAUNCH_OK(s);
   return QHP_OK;
 }
@@ -582,6 +610,15 @@ int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, i
   if (total_host) *total_host = tot;
   cudaFree(start);
   if (cnt_own) cudaFree(cnt_own);
+  return QHP_OK;
+}
+
+// canonical order (cells, ties by atom index) of the current cell assignment into `order_out` (parity hook)
+int qhp_cells_canonical_order(qhp_system *s, int32_t *order_out) {
+  CellArgs a = cell_args(s, true);
+  const int tb = 256, grid = (s->N + tb - 1) / tb;
+  k_cells_rank<<<grid, tb, 0, s->stream>>>(a, s->cell_of, s->cell_start, s->cell_tmp, nullptr, order_out, nullptr);
+  QHP_LAUNCH_OK(s);
   return QHP_OK;
 }
 

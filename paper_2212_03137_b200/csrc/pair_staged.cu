@@ -173,7 +173,8 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   const uint32_t sXY = (uint32_t)__cvta_generic_to_shared(XY), sZ = (uint32_t)__cvta_generic_to_shared(Z),
                  sC = (uint32_t)__cvta_generic_to_shared(C), sTab = (uint32_t)__cvta_generic_to_shared(tab), sQt = (uint32_t)__cvta_generic_to_shared(qtab),
                  sQ = (uint32_t)__cvta_generic_to_shared(queue) + warp * (STG_QUEUE * 4);
-  const unsigned lt = (1u << lane) - 1u;
+  unsigned lt;
+  asm volatile("mov.u32 %0, %%lanemask_lt;" : "=r"(lt));   // volatile: kept in a register (ptxas re-derives (1 << lane) - 1 per use)
   double U = 0.0;
   unsigned long long hits = 0;
 
@@ -263,7 +264,8 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
           hit = fma(dz, dz, fma(dy, dy, dx * dx)) < a.rc2;
           if (j < 7) { xyj = lds_d2(sXY + (entry(j + 1) & STG_IDX_MASK) * 16); zj = lds_d(sZ + (entry(j + 1) & STG_IDX_MASK) * 8); }
         }
-        const unsigned mask = __ballot_sync(0xffffffffu, hit);
+        unsigned mask;
+        asm volatile("{ .reg .pred p; setp.ne.u32 p, %1, 0; vote.sync.ballot.b32 %0, p, 0xffffffff; }" : "=r"(mask) : "r"((unsigned)hit));
         if (hit) sts_u(qa + __popc(mask & lt) * 4, e);
         qa += __popc(mask) * 4;
       }

@@ -248,6 +248,7 @@ extern "C" int qhp_create(const qhp_topology *top, int P, int P_contract, double
   CREATE_CUDA(cudaMalloc(&s->cell_start, sizeof(int32_t) * (s->ncell + 1)));
   CREATE_CUDA(cudaMalloc(&s->cell_cursor, sizeof(int32_t) * (s->ncell + 1)));
   CREATE_CUDA(cudaMalloc(&s->cell_tmp, sizeof(int32_t) * N));
+  CREATE_CUDA(cudaMalloc(&s->cell_key, sizeof(int32_t) * N));
   CREATE_CUDA(cudaMalloc(&s->order, sizeof(int32_t) * N));
   CREATE_CUDA(cudaMalloc(&s->rank, sizeof(int32_t) * N));
   CREATE_CUDA(cudaMalloc(&s->nbr_count, sizeof(int32_t) * N));
@@ -283,7 +284,7 @@ extern "C" int qhp_destroy(qhp_system *s) {
   void *ptrs[] = {d.type, d.molid, d.mol_atom_start, d.mol_bond_start, d.mol_angle_start, d.bond_idx, d.bond_k,
                   d.bond_r0, d.angle_idx, d.angle_k, d.angle_th0, d.mass, d.tether_k, d.tiles, s->Q, s->Pm, s->coef,
                   s->d_Tc, s->pos4, s->Fs, s->cent4, s->cref, s->pair_tab, s->cell_of, s->cell_count, s->cell_start,
-                  s->cell_cursor, s->cell_tmp, s->order, s->rank, s->nbr, s->nbr16, s->nbr_count, s->d2max, s->counters,
+                  s->cell_cursor, s->cell_tmp, s->cell_key, s->order, s->rank, s->nbr, s->nbr16, s->nbr_count, s->d2max, s->counters,
                   s->red, s->obs, s->gamma, s->Hf, s->hk, s->H4, s->Fc, s->vseg, s->tw, s->seg_slot, s->slot_atom,
                   s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p, s->ratio_tau, s->ratio_avv, s->ratio_avf, s->kappa};
   for (void *p : ptrs) if (p) cudaFree(p);
@@ -549,7 +550,7 @@ extern "C" int qhp_neighbor_lists(qhp_system *s, int32_t *cell_of, int32_t *orde
   int rc = rebuild_and_forces(s, true);
   if (rc) return rc;
   if (cell_of) QHP_CUDA_OK(s, cudaMemcpyAsync(cell_of, s->cell_of, sizeof(int32_t) * s->N, cudaMemcpyDeviceToDevice, s->stream));
-  if (order) QHP_CUDA_OK(s, cudaMemcpyAsync(order, s->order, sizeof(int32_t) * s->N, cudaMemcpyDeviceToDevice, s->stream));
+  if (order) { rc = qhp_cells_canonical_order(s, order); if (rc) return rc; }   // the internal slot order is Morton-sorted inside cells
   if (cell_start) QHP_CUDA_OK(s, cudaMemcpyAsync(cell_start, s->cell_start, sizeof(int32_t) * (s->ncell + 1), cudaMemcpyDeviceToDevice, s->stream));
   if (n_cells3) {
     const int32_t h[3] = {s->nc[0], s->nc[1], s->nc[2]};

@@ -84,6 +84,7 @@ struct qhp_system {
   int nc[3]{1, 1, 1}, ncell = 1;
   int32_t *cell_of = nullptr, *cell_count = nullptr, *cell_start = nullptr, *cell_cursor = nullptr;
   int32_t *cell_tmp = nullptr, *order = nullptr, *rank = nullptr;
+  int32_t *cell_key = nullptr;             // [N] sub-cell Morton key of the atom inside its cell (internal slot order)
   int coop_blocks = 0;                     // resident CTAs of the fused (cooperative) cell kernel; 0 = four separate kernels
   int32_t *nbr = nullptr, *nbr_count = nullptr;
   int64_t nbr_stride = 0;
@@ -162,6 +163,7 @@ int qhp_nm_contracted_out(qhp_system *s, double *xc);
 // cells.cu
 int qhp_cells_rebuild(qhp_system *s, bool force);   // early-exits on device unless needed/forced
 int qhp_cells_setup(qhp_system *s);                 // cooperative-launch capacity of the fused cell kernel
+int qhp_cells_canonical_order(qhp_system *s, int32_t *order_out);   // parity hook: ties by atom index
 int qhp_cells_export(qhp_system *s, int32_t *count, int32_t *nbr, int64_t cap, int64_t *total_host);
 // pair.cu
 int qhp_pair_forces(qhp_system *s, bool energy);     // pos4 -> Fs (+ U_s, count into obs/counters); bead-sharded if qhp_set_comm
