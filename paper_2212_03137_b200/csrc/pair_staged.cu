@@ -10,7 +10,7 @@
 // staged atom, not per pair), and the neighbour table holds 16-bit indices into that staged array.
 //
 // Per atom i (one warp); a list entry = staged index | atom type << 13:
-//   check   32 list entries at a time: fp32 distance test on a float4 copy (conservative margin,
+//   check   32 list entries at a time: packed-half distance test on an 8-byte fp16 copy (conservative margin,
 //           it only rejects pairs that are certainly outside r_c), ballot compaction of the
 //           survivors into a per-warp queue; the record of the next step is requested one step ahead;
 //   eval    whenever the queue holds >= 32 survivors: all 32 lanes evaluate one pair each in fp64
@@ -25,6 +25,7 @@
 // from the Taylor series of S, qhp_pair_setup) sit in the kernel's constant bank.
 // Full list (each ordered pair evaluated from its own side): no atomics, fixed summation order.
 #include <math.h>
+#include <cuda_fp16.h>
 
 #include "qhp_internal.cuh"
 
@@ -51,7 +52,7 @@ struct StagedArgs {
   double qs[QHP_MAX_TYPES];      // sqrt(Coulomb constant) * charge per type: qq = qs_i * qs_j
   unsigned lj_mask[QHP_MAX_TYPES]; // bit tj: types (ti, tj) have a Lennard-Jones term
   double rc, rc2, u_scale, fshift, erfc_rc;
-  float rc2f;
+  unsigned rc2h;                 // fp16 pre-test threshold (r_c^2 + error bound, rounded up), both halves of a half2
   double cS[QHP_NPOLY], cE[QHP_NPOLY];
   double *part;                  // ENERGY: per-CTA partial sums of U_s
   unsigned long long *count;     // ENERGY: in-cutoff pair-bead counter
@@ -77,24 +78,38 @@ __device__ __forceinline__ double poly_eval(const double *c, double u) {
 }
 
 // shared-memory accesses through 32-bit shared addresses (no generic pointers, no 64-bit address arithmetic)
-__device__ __forceinline__ float4 lds_f4(uint32_t a) { float4 v; asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a)); return v; }
+__device__ __forceinline__ uint2 lds_u2(uint32_t a) { uint2 v; asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v; }
 __device__ __forceinline__ double2 lds_d2(uint32_t a) { double2 v; asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a)); return v; }
 __device__ __forceinline__ double lds_d(uint32_t a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
 __device__ __forceinline__ uint32_t lds_u(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ void sts_u(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
 
+// fp16 pre-test record of a staged atom: (x, y) and (z, 0) as two half2 words, round to nearest
+__device__ __forceinline__ uint2 half_record(double x, double y, double z) {
+  const __half2 xy = __floats2half2_rn((float)x, (float)y), zw = __floats2half2_rn((float)z, 0.f);
+  return make_uint2(*reinterpret_cast<const unsigned *>(&xy), *reinterpret_cast<const unsigned *>(&zw));
+}
+// packed-half squared distance of two records against the threshold (qhp_pair_staged_forces derives the error bound
+// that makes this test conservative: it never rejects a pair whose fp64 r^2 is below r_c^2)
+__device__ __forceinline__ bool half_test(uint2 ci, uint2 cj, unsigned thr) {
+  const __half2 dxy = __hsub2(*reinterpret_cast<const __half2 *>(&ci.x), *reinterpret_cast<const __half2 *>(&cj.x));
+  const __half2 dzw = __hsub2(*reinterpret_cast<const __half2 *>(&ci.y), *reinterpret_cast<const __half2 *>(&cj.y));
+  const __half2 s = __hfma2(dzw, dzw, __hmul2(dxy, dxy));              // (dx^2 + dz^2, dy^2)
+  return __hlt(__hadd(__low2half(s), __high2half(s)), __low2half(*reinterpret_cast<const __half2 *>(&thr)));
+}
+
 // Row layout of the 16-bit table (written by k_list_build16, cells.cu): the entry of rank `pos` in a
 // row sits at (pos / 256) * 256 + (pos % 32) * 8 + (pos % 256) / 32, i.e. one 16-byte load per lane
 // brings entries pos = 256 m + 32 j + lane, j = 0..7; a row is padded with the dummy index up to a
 // multiple of 32 entries, so a check step never needs a per-lane tail predicate.
-// Shared memory: XY[cap] (x, y) and Z[cap] fp64, cell-centred; F32: C[cap] float4 copy (x, y, z, type bits)
-// for the fp32 pre-test.  !F32 (neighbourhoods too large for 40 B per atom): 24 B per atom, fp64 pre-test.
+// Shared memory: XY[cap] (x, y) and Z[cap] fp64, cell-centred; F32: C[cap] 8-byte fp16 copy (x, y | z, 0)
+// for the packed-half pre-test.  !F32 (neighbourhoods too large for 32 B per atom): 24 B per atom, fp64 pre-test.
 template <bool ENERGY, bool F32>
 __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double2 *XY = reinterpret_cast<double2 *>(smem_raw);
   double *Z = reinterpret_cast<double *>(XY + a.cap);
-  float4 *C = reinterpret_cast<float4 *>(Z + a.cap);
+  uint2 *C = reinterpret_cast<uint2 *>(Z + a.cap);
   double *tab = F32 ? reinterpret_cast<double *>(C + a.cap) : reinterpret_cast<double *>(Z + a.cap);
   double *qtab = tab + QHP_MAX_TYPES * QHP_MAX_TYPES * 4;             // sqrt(Coulomb constant) * charge per type
   uint32_t *queue = reinterpret_cast<uint32_t *>(qtab + QHP_MAX_TYPES);
@@ -158,13 +173,13 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
           ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
           lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
           XY[g] = make_double2(lx, ly); Z[g] = lz;
-          if (F32) C[g] = make_float4((float)lx, (float)ly, (float)lz, __int_as_float((int)__double_as_longlong(p[u].w)));
+          if (F32) C[g] = half_record(lx, ly, lz);
         }
       }
     }
     if (tid == 0) {                                      // the dummy: every pre-test against it fails
       XY[a.cap - 1] = make_double2(1e9, 1e9); Z[a.cap - 1] = 1e9;
-      if (F32) C[a.cap - 1] = make_float4(1e9f, 1e9f, 1e9f, 0.f);
+      if (F32) C[a.cap - 1] = half_record(1e9, 1e9, 1e9);     // +inf: inf - x = inf, inf - inf = NaN, neither is < the threshold
     }
   }
   __syncthreads();
@@ -195,10 +210,9 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
     if (nblk > 0) cur = *reinterpret_cast<const uint4 *>(rowp + 8 * lane);
     const double2 xyi = lds_d2(sXY + ei * 16);
     const double zi = lds_d(sZ + ei * 8);
-    float4 ci = make_float4(0.f, 0.f, 0.f, 0.f);
-    int ti;
-    if (F32) { ci = lds_f4(sC + ei * 16); ti = __float_as_int(ci.w); }
-    else ti = (int)__double_as_longlong(pos[slot].w);
+    uint2 ci = make_uint2(0u, 0u);
+    if (F32) ci = lds_u2(sC + ei * 8);
+    const int ti = (int)__double_as_longlong(pos[slot].w);
     const uint32_t sTi = sTab + (uint32_t)(ti * a.nt) * 32u;
     const double qi = lds_d(sQt + ti * 8);
     const unsigned lj_mask = a.lj_mask[ti];
@@ -245,10 +259,10 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
       const int nst = min(8, (n - STG_BLOCK * m + 31) >> 5);
       // ---- check: pre-test of 32 entries per step, survivors compacted into the queue; the staged record
       //      of the next step is requested before this step's compaction store ------------------------------
-      float4 cj = make_float4(0.f, 0.f, 0.f, 0.f);
+      uint2 cj = make_uint2(0u, 0u);
       double2 xyj = make_double2(0.0, 0.0);
       double zj = 0.0;
-      if (F32) cj = lds_f4(sC + (entry(0) & STG_IDX_MASK) * 16);
+      if (F32) cj = lds_u2(sC + (entry(0) & STG_IDX_MASK) * 8);
       else { xyj = lds_d2(sXY + (entry(0) & STG_IDX_MASK) * 16); zj = lds_d(sZ + (entry(0) & STG_IDX_MASK) * 8); }
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
@@ -256,9 +270,8 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
         const uint32_t e = entry(j);
         bool hit;
         if (F32) {
-          const float dxf = ci.x - cj.x, dyf = ci.y - cj.y, dzf = ci.z - cj.z;
-          hit = fmaf(dzf, dzf, fmaf(dyf, dyf, dxf * dxf)) < a.rc2f;
-          if (j < 7) cj = lds_f4(sC + (entry(j + 1) & STG_IDX_MASK) * 16);
+          hit = half_test(ci, cj, a.rc2h);
+          if (j < 7) cj = lds_u2(sC + (entry(j + 1) & STG_IDX_MASK) * 8);
         } else {
           const double dx = xyi.x - xyj.x, dy = xyi.y - xyj.y, dz = zi - zj;
           hit = fma(dz, dz, fma(dy, dy, dx * dx)) < a.rc2;
@@ -365,7 +378,7 @@ static long double fit_poly(int which, long double wmax, long double scale, doub
   return worst;
 }
 
-static size_t staged_atom_bytes(bool f32) { return 3 * sizeof(double) + (f32 ? sizeof(float4) : 0); }
+static size_t staged_atom_bytes(bool f32) { return 3 * sizeof(double) + (f32 ? sizeof(uint2) : 0); }
 static size_t staged_smem_bytes(int cap, int warps, bool f32) {
   return (size_t)cap * staged_atom_bytes(f32) + 16 + sizeof(double) * (QHP_MAX_TYPES * QHP_MAX_TYPES * 4 + QHP_MAX_TYPES) +
          sizeof(uint32_t) * (size_t)warps * STG_QUEUE;
@@ -410,7 +423,7 @@ int qhp_pair_staged_partials(const qhp_system *s) { return s->ncell * 8 * s->Pc;
 bool qhp_pair_staged_fit(qhp_system *s, long long region) {
   static const int tries[] = {STG_MAX_WARPS, 24, 16};
   const long long need = region + region / 16 + 32 + 1;               // + the dummy at cap - 1
-  // first choice: the fp32 pre-test copy with the largest CTA; then the same CTA sizes without the copy
+  // first choice: the fp16 pre-test copy with the largest CTA; then the same CTA sizes without the copy
   for (int f32 = 1; f32 >= 0; --f32)
     for (int w : tries) {
       if (w > STG_MAX_WARPS) continue;
@@ -439,12 +452,27 @@ int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned lo
   a.erfc_rc = erfc(al * rc) / rc;
   a.fshift = erfc(al * rc) / (rc * rc) + 2.0 * al / sqrt(QHP_PI) * exp(-al * al * rc * rc) / rc;
   {
-    // fp32 pre-test margin: 4x a bound on the fp32 error of r^2 (two roundings of coordinates up to
-    // 1.5 cell edges + skin, one of each difference, three of the sum of squares)
+    // fp16 pre-test threshold = r_c^2 + a bound on the error of the packed-half r^2, rounded UP to a half.
+    // Staged coordinates reach 1.5 cell edges + skin: rounding them to half moves each by <= ulp(cmax)/2; the half
+    // difference of two records adds <= ulp(r_c + 1)/2; so each component of d is off by e_d, r^2 by
+    // <= 2 sqrt(3) r_c' e_d + 3 e_d^2 (r_c' = r_c + 1 covers the margin itself); the product, the fma, the sum and the
+    // rounding of the threshold add <= 4 half-ulps at r_c^2 + margin.  The float -> half double rounding of the
+    // staging adds 2^-13 relative to the half-ulp (the 1.01).  Pairs certainly outside r_c are the only ones rejected.
+    auto ulp16 = [](double v) { int e; frexp(v, &e); return ldexp(1.0, e - 11); };   // spacing of halves just below 2^e >= v
     double cmax = 0.0;
     for (int d = 0; d < 3; ++d) cmax = fmax(cmax, 1.5 * a.cell_edge[d] + s->skin + 1.0);
-    const double err = 2.0 * sqrt(3.0) * rc * (cmax * ldexp(1.0, -23) + rc * ldexp(1.0, -24)) + 4.0 * ldexp(1.0, -24) * rc * rc;
-    a.rc2f = (float)(rc * rc + 4.0 * err) * (1.0f + 1.2e-7f);
+    const double e_d = 1.01 * (ulp16(cmax) + 0.5 * ulp16(rc + 1.0));
+    double thr = rc * rc + 2.0 * sqrt(3.0) * (rc + 1.0) * e_d + 3.0 * e_d * e_d;
+    thr += 2.0 * ulp16(thr + 4.0);
+    __half h = __double2half(thr);                                      // round to nearest, then step up if it fell below
+    if (__half2float(h) < thr) {
+      unsigned short b = *reinterpret_cast<unsigned short *>(&h);
+      ++b;
+      h = *reinterpret_cast<__half *>(&b);
+    }
+    const unsigned short hb = *reinterpret_cast<unsigned short *>(&h);
+    a.rc2h = (unsigned)hb | ((unsigned)hb << 16);
+    s->staged_thr = (double)__half2float(h);
   }
   for (int k = 0; k < QHP_NPOLY; ++k) { a.cS[k] = s->polyS[k]; a.cE[k] = s->polyE[k]; }
   for (int t = 0; t < s->nt; ++t) {

@@ -95,7 +95,8 @@ struct qhp_system {
   uint16_t *nbr16 = nullptr;               // [N][nbr_stride]
   int staged_cap = 0;                      // staged atoms that fit in shared memory
   int staged_warps = 0, staged_smem_max = 0; // CTA size in use, dynamic shared memory available
-  bool staged_f32 = true;                  // the staged kernel keeps a float4 copy for the fp32 pre-test (else fp64 pre-test)
+  bool staged_f32 = true;                  // the staged kernel keeps an 8-byte fp16 copy for the packed-half pre-test (else fp64 pre-test)
+  double staged_thr = 0.0;                 // threshold of that pre-test (r_c^2 + its error bound, a half)
   int staged_split = 1;                    // CTAs per (cell, bead)
   double polyS[QHP_NPOLY]{}, polyE[QHP_NPOLY]{};   // alpha^3 S(w), alpha E(w) in u = 2 r^2/rc^2 - 1
   unsigned long long *d2max = nullptr;     // [2] double bits, max |xc - cref|^2, double-buffered by step parity

@@ -199,6 +199,31 @@ def test_harmonic_oscillators_single_atom_molecules():
     assert np.abs(obs - ref.observables()).max() < 1e-9 * np.abs(ref.observables()).max()
 
 
+def test_staged_pretest_rejects_no_pair_inside_the_cutoff():
+    """The staged kernel drops list entries by a packed-half distance pre-test before the fp64 test.  A pair it
+    wrongly dropped near r_c would be invisible in the forces (the shifted force vanishes at r_c), so the
+    pre-test is pinned by the integer it must not change: the number of in-cutoff (ordered) pair-beads equals
+    a KD-tree count on the oracle's contracted beads (Eq. 20), intramolecular pairs excluded."""
+    import oracle as O
+    from scipy.spatial import cKDTree
+    top = W.water_box(5832)
+    sysg, _, x0, p0 = make_pair(top, 4, 2, 0.25, "pile", sigma_bead=0.05)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    c = sysg.counters()
+    assert c["staged"] == 1 and c["overflow"] == 0
+    xc = O.contract(O.beads_to_nm(x0), 2)
+    L = top["box"]
+    want = 0
+    for b in range(2):
+        pr = cKDTree(np.mod(xc[b], L), boxsize=L).query_pairs(top["r_cut"], output_type="ndarray")
+        d = xc[b][pr[:, 0]] - xc[b][pr[:, 1]]
+        d -= L * np.rint(d / L)
+        r2 = (d * d).sum(1)
+        assert np.abs(r2 - top["r_cut"] ** 2).min() > 1e-9          # no decision rests on the last bits
+        want += 2 * int((top["mol"][pr[:, 0]] != top["mol"][pr[:, 1]]).sum())
+    assert c["pair_beads_in_cutoff"] == want
+
+
 def test_staged_pair_kernel_mid_size():
     """5832 waters (17,496 atoms, 5 x 5 x 5 cells): the smallest water box the shared-memory staged pair
     kernel serves (>= 4 cells per dimension and the 27-cell neighbourhood fits); lists, forces,
