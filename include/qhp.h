@@ -214,7 +214,8 @@ int qhp_profile(qhp_system *sys, int enable);
 int qhp_profile_read(qhp_system *sys, double *ms_host, int64_t *n_host);
 /* Synchronise the stream and report sticky CUDA / overflow errors. */
 int qhp_check(qhp_system *sys);
-const char *qhp_last_error(const qhp_system *sys); /* sys may be NULL: last create error */
+const char *qhp_last_error(const qhp_system *sys); /* sys may be NULL: last error of a call without a handle
+                                                     * (qhp_create, qhp_pibar_noalloc) */
 
 /* ---- stand-alone primitives of the path (device pointers), for parity tests ------------- */
 /* Philox4x32-10 words and the three Box-Muller normals of counter (atom0+i, mode | tag<<24,
@@ -240,6 +241,31 @@ int qhp_dfma_probe(double *sink, int grid, int block, int64_t iters, void *cuda_
  * pointers.  The inputs are not modified.  QHP_EINVAL for empty series or beta <= 0. */
 int qhp_pibar(const double *wA, int64_t n_A, const double *wB, int64_t n_B, double beta, int max_iter,
               double tol, void *cuda_stream, double *dF_host, int *iters_host);
+
+/* The same estimator for callers that may not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc).  qhp_pibar allocates and frees its per-CTA partial sums on
+ * every call and copies the result to the host; this entry point calls no cudaMalloc, cudaFree, memcpy or
+ * allocating library routine and does NOT synchronise: it enqueues one cooperative kernel on cuda_stream.
+ *   scratch   the per-CTA partial sums live in a file-scope static __device__ array of the library
+ *             (QHP_PIBAR_NOALLOC_SCRATCH_BYTES = 16 KiB, held by every GPU that loads the library until
+ *             exit): room for QHP_PIBAR_NOALLOC_MAX_CTAS CTAs.
+ *   limit     n_A, n_B <= QHP_PIBAR_NOALLOC_MAX_N (= MAX_CTAS CTAs x 256 threads x 64 samples per thread and
+ *             iteration); longer series, or a device whose grid would need more CTAs than the array holds,
+ *             are rejected with QHP_EINVAL and a text in qhp_last_error(NULL).  Use qhp_pibar for those.
+ *   out_dev   DEVICE pointer, 2 doubles, caller-owned: out_dev[0] = dF (kcal/mol), out_dev[1] = number of
+ *             iterations; valid once the work enqueued on cuda_stream has finished.
+ *   sharing   every call on a device uses the same array and finds the previous call's partial sums in it.
+ *             Nothing has to start at zero: each iteration writes all of its partial sums before the grid
+ *             barrier that precedes their reads.  Calls that overlap on the GPU (two streams, two host
+ *             threads, two graphs in flight) RACE on the array: serialise them (one stream, or events).
+ *   set-up    the first call on each device resolves the array's device address (cudaGetSymbolAddress with
+ *             that device current) and the launch geometry; make that first call outside stream capture.
+ * Same arguments, arithmetic, grid and summation order as qhp_pibar otherwise: the two agree bit for bit. */
+#define QHP_PIBAR_NOALLOC_MAX_CTAS 512
+#define QHP_PIBAR_NOALLOC_SCRATCH_BYTES (4 * QHP_PIBAR_NOALLOC_MAX_CTAS * 8)
+#define QHP_PIBAR_NOALLOC_MAX_N (QHP_PIBAR_NOALLOC_MAX_CTAS * 256 * 64)
+int qhp_pibar_noalloc(const double *wA, int64_t n_A, const double *wB, int64_t n_B, double beta, int max_iter,
+                      double tol, void *cuda_stream, double *out_dev);
 
 #ifdef __cplusplus
 }

@@ -6,7 +6,9 @@ device memory and streams.  There is no CPU fallback: importing `binding` withou
 libqhp.so raises, and every call needs a CUDA device.
 """
 from .binding import (QHP_THERMO_ADQTB, QHP_THERMO_NONE, QHP_THERMO_PILE, QhpError, System, lib,
-                      lib_path, qhp_dfma_probe, qhp_fft_c2c, qhp_philox_normals, qhp_pibar)
+                      lib_path, qhp_dfma_probe, qhp_fft_c2c, qhp_philox_normals, qhp_pibar, qhp_pibar_noalloc,
+                      PIBAR_NOALLOC_MAX_N)
 
 __all__ = ["System", "QhpError", "lib", "lib_path", "QHP_THERMO_NONE", "QHP_THERMO_PILE",
-           "QHP_THERMO_ADQTB", "qhp_philox_normals", "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar"]
+           "QHP_THERMO_ADQTB", "qhp_philox_normals", "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar",
+           "qhp_pibar_noalloc", "PIBAR_NOALLOC_MAX_N"]

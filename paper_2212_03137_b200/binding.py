@@ -18,7 +18,7 @@ SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_respa", "qhp_set_a_block", "qhp
            "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
            "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma", "qhp_adqtb_ratio", "qhp_adqtb_kappa",
            "qhp_adqtb_segment", "qhp_counters", "qhp_profile", "qhp_profile_read", "qhp_check", "qhp_last_error", "qhp_philox_normals",
-           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar", "qhp_set_comm", "qhp_pair_slices"]
+           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar", "qhp_pibar_noalloc", "qhp_set_comm", "qhp_pair_slices"]
 
 
 # int fn(void *ctx, void *device_buf, size_t bytes_per_rank, int rank, int world, void *cuda_stream)  (include/qhp.h)
@@ -114,6 +114,7 @@ def lib():
         L.qhp_fft_c2c.argtypes = [vp, i32, i64, i32, vp]
         L.qhp_dfma_probe.argtypes = [vp, i32, i32, i64, vp]
         L.qhp_pibar.argtypes = [vp, i64, vp, i64, C.c_double, i32, C.c_double, vp, C.POINTER(C.c_double), C.POINTER(i32)]
+        L.qhp_pibar_noalloc.argtypes = [vp, i64, vp, i64, C.c_double, i32, C.c_double, vp, vp]
         for name in SYMBOLS:
             if name != "qhp_last_error":
                 getattr(L, name).restype = C.c_int
@@ -416,3 +417,21 @@ def qhp_pibar(wA, wB, beta: float, max_iter: int = 1000, tol: float = 1e-13, str
     if rc != 0:
         raise QhpError(rc, "qhp_pibar")
     return dF.value, it.value
+
+
+PIBAR_NOALLOC_MAX_N = 512 * 256 * 64      # QHP_PIBAR_NOALLOC_MAX_N of include/qhp.h
+
+
+def qhp_pibar_noalloc(wA, wB, beta: float, out, max_iter: int = 1000, tol: float = 1e-13, stream=None):
+    """qhp_pibar without any allocation, copy or synchronisation (include/qhp.h): enqueues the estimator on the
+    stream; `out` is a caller-owned CUDA tensor of 2 doubles that receives (dF, iterations) once the stream
+    has run.  Series longer than PIBAR_NOALLOC_MAX_N are rejected.  Calls overlapping on the GPU race on the
+    library's static scratch array: keep them on one stream."""
+    torch = _torch()
+    _chk_dev(wA, torch.float64, None, "wA")
+    _chk_dev(wB, torch.float64, None, "wB")
+    _chk_dev(out, torch.float64, 2, "out")
+    rc = lib().qhp_pibar_noalloc(_ptr(wA), int(wA.numel()), _ptr(wB), int(wB.numel()), float(beta), int(max_iter),
+                                 float(tol), _stream_ptr(stream), _ptr(out))
+    if rc != 0:
+        raise QhpError(rc, (lib().qhp_last_error(None) or b"qhp_pibar_noalloc").decode())

@@ -293,6 +293,8 @@ extern "C" int qhp_destroy(qhp_system *s) {
 }
 
 extern "C" const char *qhp_last_error(const qhp_system *s) { return s ? s->err.c_str() : g_create_err.c_str(); }
+// text of a failed call that has no system handle (read back by qhp_last_error(NULL))
+void qhp_global_error(const char *msg) { g_create_err = msg; }
 
 // list (re)build on the current centroids followed by the slow forces in the new slot order
 static int rebuild_and_forces(qhp_system *s, bool force) {

@@ -202,3 +202,5 @@ int qhp_fft_launch(double *data, int n, int64_t batch, int sign, const double *t
 __host__ __device__ __forceinline__ long long qhp_seg_addr(int slot, int n_seg, int n) {
   return ((long long)(slot >> 2) * n_seg + n) * 12 + (slot & 3) * 3;
 }
+
+void qhp_global_error(const char *msg);   // qhp_api.cu: error text of a call without a system handle (qhp_last_error(NULL))
