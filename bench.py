@@ -154,6 +154,9 @@ def job_throughput(world: int, n_atoms: int, P: int, steps: int, seconds: float)
     return world * n_atoms * P * steps / seconds
 
 
+PRUNE_SKIN = None       # --prune-skin: None = the library's default (include/qhp.h qhp_set_pair_prune)
+
+
 def build_system(cfg: dict):
     import paper_2212_03137_b200 as qhp
     top = W.water_box(cfg["n_mol"])
@@ -162,6 +165,8 @@ def build_system(cfg: dict):
         kw = dict(n_seg=cfg["n_seg"], a_gamma=cfg["a_gamma"])
     sysg = qhp.System(top, cfg["P"], cfg["P_contract"], cfg["dt_fs"] * 1e-3, W.T_KELVIN, cfg["thermostat"],
                       gamma0=cfg["gamma0"], seed=W.MASTER_SEED, **kw)
+    if PRUNE_SKIN is not None:
+        sysg.set_pair_prune(PRUNE_SKIN)
     x0, p0 = W.initial_state(top, cfg["P"], W.T_KELVIN)
     return top, sysg, x0, p0
 
@@ -348,6 +353,7 @@ def main():
     ap.add_argument("--a-block", choices=["exact", "cayley"], default="exact", help="cayley = BCOCB (PAPER.md:151); exact = the BASELINE.json configs")
     ap.add_argument("--n-alt", type=int, default=1, help="BAOAB-RESPA inner steps per V_s evaluation (PAPER.md Eq. 19); 1 = the BASELINE.json configs")
     ap.add_argument("--n-mol", type=int, default=0, help="profiling aid: the same workload on a box of this many waters (0 = the BASELINE.json size)")
+    ap.add_argument("--prune-skin", type=float, default=None, help="qhp_set_pair_prune: A; <= 0 = the unpruned pre-test pair kernel; default = the library's (0.5)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--shard-beads", action="store_true", help="N > 1: bead-sharded V_s over the ranks (qhp_set_comm, NCCL all-gather of F_s; N must divide P'); "
@@ -355,6 +361,8 @@ def main():
     ap.add_argument("--no-adqtb", action="store_true", help="skip the adQTB (C3) leg that the default C4 run appends")
     ap.add_argument("--no-amortised", action="store_true", help="skip the untimed 500-step run that measures the list-rebuild rate")
     args = ap.parse_args()
+    global PRUNE_SKIN
+    PRUNE_SKIN = args.prune_skin
     if args.impl == "reference":
         return run_reference(args)
     if args.warmup < 3:

@@ -127,6 +127,25 @@ int qhp_set_respa(qhp_system *sys, int n_alt);
 #define QHP_CONTRACT_TRIG 1
 int qhp_set_contraction(qhp_system *sys, int variant);
 
+/* Pruned per-bead rows of the staged pair kernel (an acceleration structure of R8; the centroid
+ * table of R7 -- the list the paper describes and the oracle is compared with -- is unchanged).  With
+ * prune_skin > 0 (default 0.5 A; must be < the list skin) every contracted bead keeps a second table holding the
+ * entries of the centroid table within r_cut + prune_skin of the bead's own positions; V_s is then evaluated on
+ * those rows without a per-step pre-test.  A bead's rows are renewed on the device, without a host round trip,
+ * when one of its atoms has moved more than prune_skin / 2 since they were made or the centroid table was
+ * rebuilt, so the evaluated pair set always contains every pair inside r_cut: forces equal those of the unpruned
+ * path up to the summation order.  Costs 2 B x P_contract x N x row stride of device memory.  prune_skin <= 0:
+ * off (every step walks the centroid table with the packed-half pre-test).  Before qhp_set_state
+ * (QHP_ESTATE afterwards). */
+int qhp_set_pair_prune(qhp_system *sys, double prune_skin);
+/* Parity hook of the pruned rows.  Makes the rows current for the present state exactly as a step does (displacement
+ * check, prune if due), evaluates V_s through them and reports, out_host[4] (HOST): [0] 1 if the pruned-row path serves
+ * this system (else the other entries are 0), [1] number of prunes so far (summed over the contracted beads; a step
+ * without a prune leaves it unchanged), [2] entries in the pruned rows, [3] ordered pair-beads of those rows that pass
+ * the fp64 test r^2 < r_cut^2 -- equal to qhp_counters' pair_beads_in_cutoff (centroid table) iff no pair inside the
+ * cutoff is missing.  Synchronises.  After qhp_set_state. */
+int qhp_pair_prune_stats(qhp_system *sys, int64_t *out_host);
+
 /* A block of the splitting: QHP_ABLOCK_EXACT (default) = exact harmonic evolution of the
  * fluctuation modes over dt/2 (Eq. 17); QHP_ABLOCK_CAYLEY = the BCOCB variant, whose half-step is the
  * square root of the Cayley transform of the free ring-polymer generator,

@@ -18,7 +18,7 @@ SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_respa", "qhp_set_a_block", "qhp
            "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
            "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma", "qhp_adqtb_ratio", "qhp_adqtb_kappa",
            "qhp_adqtb_segment", "qhp_counters", "qhp_profile", "qhp_profile_read", "qhp_check", "qhp_last_error", "qhp_philox_normals",
-           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar", "qhp_pibar_noalloc", "qhp_set_comm", "qhp_pair_slices"]
+           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar", "qhp_pibar_noalloc", "qhp_set_comm", "qhp_pair_slices", "qhp_set_pair_prune", "qhp_pair_prune_stats"]
 
 
 # int fn(void *ctx, void *device_buf, size_t bytes_per_rank, int rank, int world, void *cuda_stream)  (include/qhp.h)
@@ -114,6 +114,8 @@ def lib():
         L.qhp_fft_c2c.argtypes = [vp, i32, i64, i32, vp]
         L.qhp_dfma_probe.argtypes = [vp, i32, i32, i64, vp]
         L.qhp_pibar.argtypes = [vp, i64, vp, i64, C.c_double, i32, C.c_double, vp, C.POINTER(C.c_double), C.POINTER(i32)]
+        L.qhp_set_pair_prune.argtypes = [vp, C.c_double]
+        L.qhp_pair_prune_stats.argtypes = [vp, C.POINTER(C.c_int64)]
         L.qhp_pibar_noalloc.argtypes = [vp, i64, vp, i64, C.c_double, i32, C.c_double, vp, vp]
         for name in SYMBOLS:
             if name != "qhp_last_error":
@@ -281,6 +283,17 @@ class System:
     def set_contraction(self, variant: str):
         """"literal" (default, Eq. 20 as printed) or "trig" (Fourier interpolation; reading G3); before set_state."""
         self._ok(self._L.qhp_set_contraction(self._h, {"literal": 0, "trig": 1}[variant]))
+
+    def set_pair_prune(self, prune_skin: float):
+        """Pruned per-bead rows of the staged pair kernel (include/qhp.h): prune_skin in A (default 0.5), <= 0 off.
+        Before set_state."""
+        self._ok(self._L.qhp_set_pair_prune(self._h, float(prune_skin)))
+
+    def pair_prune_stats(self) -> dict:
+        """Parity hook (include/qhp.h qhp_pair_prune_stats)."""
+        out = (C.c_int64 * 4)()
+        self._ok(self._L.qhp_pair_prune_stats(self._h, out))
+        return dict(zip(["active", "prunes", "entries", "pair_beads_in_cutoff"], [int(v) for v in out]))
 
     def set_a_block(self, kind: str):
         """"exact" (default) or "cayley" = BCOCB (PAPER.md:151)."""

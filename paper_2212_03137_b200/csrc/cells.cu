@@ -545,7 +545,7 @@ int qhp_cells_rebuild(qhp_system *s, bool force) {
     // the staged pair kernel serves the system if its geometry allows it (qhp_pair_setup) and the
     // densest 27-cell neighbourhood fits in shared memory with some room for drift between rebuilds
     s->staged = s->staged_ok;
-    int64_t mx = 0;
+    int64_t mx = 0, region_max = 0;
     for (int attempt = 0; attempt < 2; ++attempt) {
       QHP_CUDA_OK(s, cudaMemsetAsync(&s->counters[2], 0, sizeof(int64_t), s->stream));
       QHP_CUDA_OK(s, cudaMemsetAsync(&s->counters[5], 0, sizeof(int64_t), s->stream));
@@ -555,6 +555,7 @@ int qhp_cells_rebuild(qhp_system *s, bool force) {
       QHP_CUDA_OK(s, cudaMemcpyAsync(&mx, &s->counters[2], sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
       QHP_CUDA_OK(s, cudaMemcpyAsync(&region, &s->counters[5], sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
       QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
+      region_max = region;
       if (!s->staged || qhp_pair_staged_fit(s, region)) break;
       s->staged = false;                               // too dense: generic kernel and 32-bit list
     }
@@ -575,6 +576,8 @@ int qhp_cells_rebuild(qhp_system *s, bool force) {
         return QHP_ENOMEM;
       }
     }
+    rc = qhp_pair_dense_prepare(s, region_max);          // pruned per-bead rows (pair_staged.cu): decide, allocate, mark stale
+    if (rc) return rc;
   }
   return list_build(s, a, false);
 }

@@ -57,6 +57,11 @@ struct StagedArgs {
   double *part;                  // ENERGY: per-CTA partial sums of U_s
   unsigned long long *count;     // ENERGY: in-cutoff pair-bead counter
   long long *counters;           // [7] = staged-region overflow flag
+  // k_pair_dense: rows of the table it walks ([bead][N][stride] pruned rows, or the shared table with bead strides 0)
+  long long list_bead_stride;    // entries between the tables of two beads
+  long long count_bead_stride;   // row counts between two beads
+  int dcap;                      // staged atoms of the dense kernel (dummy at dcap - 1)
+  long long *pruned_at;          // [Pc] or NULL: written with the rebuild count by CTA (0, bead)
 };
 
 // 1/sqrt(s): hardware seed (upper-word approximation, ~2^-20) + one third-order step -> ~1 ulp
@@ -324,6 +329,404 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
 }
 
 // ---------------------------------------------------------------------------------------------
+// k_pair_dense: evaluation without pre-test.  Same CTA-per-(cell, bead) staging, but only the fp64 records
+// (24 B per staged atom: two CTAs per SM) and no queue: every entry of the row is evaluated, the exact fp64
+// r^2 < r_c^2 test masks the result.  Pays when the rows are dense (the pruned per-bead rows: >= 85 % of the
+// entries inside r_c).  COUNT (parity hook qhp_pair_prune_stats only) also counts the pairs that pass the fp64 test.
+// ---------------------------------------------------------------------------------------------
+#ifndef DNS_THREADS
+#define DNS_THREADS 448          // 14 warps x 2 CTAs per SM at 72 registers (512: 64 registers, spills)
+#endif
+#ifndef DNS_CTAS
+#define DNS_CTAS 2
+#endif
+template <bool COUNT>
+__global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const StagedArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double2 *XY = reinterpret_cast<double2 *>(smem_raw);
+  double *Z = reinterpret_cast<double *>(XY + a.dcap);
+  double *tab = reinterpret_cast<double *>(Z + a.dcap);
+  double *qtab = tab + a.nt * a.nt * 4;                     // tables sized by the number of types: room for staged atoms
+  __shared__ int off[28], cbeg[27], next_atom;
+
+  const int tid = threadIdx.x, lane = tid & 31, nthr = blockDim.x;
+  const int cell = blockIdx.x / a.split, part = blockIdx.x % a.split, bead = a.bead0 + blockIdx.y;
+  const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
+  // the rows of this bead were made current by the k_prune launch in front of this one: record their rebuild count
+  if (a.pruned_at && blockIdx.x == 0 && tid == 0) a.pruned_at[bead] = a.counters[0];
+
+  for (int k = tid; k < a.nt * a.nt * 4; k += nthr) {      // (qq, 4 eps, sigma^2, shift) -> (24 eps, sigma^2, qq, shift)
+    const int f = k & 3;
+    tab[(k & ~3) + (f == 0 ? 2 : (f == 1 ? 0 : (f == 2 ? 1 : 3)))] = (f == 1 ? 6.0 : 1.0) * a.pair_tab[k];
+  }
+  if (tid < a.nt) qtab[tid] = a.qs[tid];
+  if (tid < 27) {
+    const int ox = tid / 9, oy = (tid / 3) % 3, oz = tid % 3;
+    const int qx = (cx - 1 + ox + a.nc[0]) % a.nc[0], qy = (cy - 1 + oy + a.nc[1]) % a.nc[1],
+              qz = (cz - 1 + oz + a.nc[2]) % a.nc[2];
+    const int c2 = (qx * a.nc[1] + qy) * a.nc[2] + qz;
+    cbeg[tid] = a.cell_start[c2];
+    off[tid + 1] = a.cell_start[c2 + 1] - a.cell_start[c2];
+  }
+  __syncthreads();
+  if (tid == 0) {
+    next_atom = 0;
+    off[0] = 0;
+    for (int s = 0; s < 27; ++s) off[s + 1] += off[s];
+  }
+  __syncthreads();
+  const int total = off[27];
+  if (off[14] == off[13]) return;
+  if (total > a.dcap - 1) {
+    if (tid == 0) a.counters[7] = 1;
+    return;
+  }
+  const double4 *pos = reinterpret_cast<const double4 *>(a.pos4) + (long long)bead * a.N;
+  const int h0 = off[13], nh = off[14] - off[13], slot0 = cbeg[13];
+  const uint16_t *table = a.nbr16 + (long long)bead * a.list_bead_stride;
+  const int32_t *counts = a.nbr_count + (long long)bead * a.count_bead_stride;
+  // Rows are dealt to the warps round-robin (rows of one cell have near-equal lengths); the next row's count, type
+  // and first block are requested before the current row is evaluated (the first one before the staging), so a row
+  // never starts on a global-load wait.
+  // (the broadcast tells the compiler that the row loop is warp-uniform: polynomial coefficients stay in uniform registers)
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0), istep = a.split * (nthr >> 5);
+  int ii = part + a.split * warp;
+  int n_nx = 0, ti_nx = 0;
+  uint4 cur = make_uint4(0u, 0u, 0u, 0u);                  // the block being evaluated; its successor (same row or next row) in flight
+  if (ii < nh) {
+    n_nx = counts[slot0 + ii];
+    ti_nx = (int)__double_as_longlong(pos[slot0 + ii].w);
+    cur = *reinterpret_cast<const uint4 *>(table + (long long)(slot0 + ii) * a.stride + 8 * lane);
+  }
+  {
+    const double ctr[3] = {(cx + 0.5) * a.cell_edge[0], (cy + 0.5) * a.cell_edge[1], (cz + 0.5) * a.cell_edge[2]};
+    const double MAGIC = 6755399441055744.0;
+    constexpr int UN = 4;
+    for (int g0 = tid; g0 < total; g0 += UN * nthr) {
+      double4 p[UN];
+      int s = 0;
+#pragma unroll
+      for (int u = 0; u < UN; ++u) {
+        const int g = g0 + u * nthr;
+        if (g < total) {
+          while (g >= off[s + 1]) ++s;
+          p[u] = pos[cbeg[s] + g - off[s]];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < UN; ++u) {
+        const int g = g0 + u * nthr;
+        if (g < total) {
+          double lx = p[u].x - ctr[0], ly = p[u].y - ctr[1], lz = p[u].z - ctr[2];
+          lx = fma(-a.box[0], (lx * a.inv_box[0] + MAGIC) - MAGIC, lx);
+          ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
+          lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
+          XY[g] = make_double2(lx, ly); Z[g] = lz;
+        }
+      }
+    }
+    if (tid == 0) { XY[a.dcap - 1] = make_double2(1e9, 1e9); Z[a.dcap - 1] = 1e9; }
+  }
+  __syncthreads();
+
+  const uint32_t sXY = (uint32_t)__cvta_generic_to_shared(XY), sZ = (uint32_t)__cvta_generic_to_shared(Z),
+                 sTab = (uint32_t)__cvta_generic_to_shared(tab), sQt = (uint32_t)__cvta_generic_to_shared(qtab);
+  unsigned long long hits = 0;
+
+  for (; ii < nh; ii += istep) {
+    const uint32_t ei = (uint32_t)(h0 + ii);
+    const long long slot = slot0 + ii;
+    const int n = n_nx, ti = ti_nx;
+    const uint16_t *rowp = table + slot * a.stride;
+    const int nblk = max(1, (n + STG_BLOCK - 1) / STG_BLOCK);
+    const bool more = ii + istep < nh;
+    if (more) {
+      n_nx = counts[slot + istep];
+      ti_nx = (int)__double_as_longlong(pos[slot + istep].w);
+    }
+    const double2 xyi = lds_d2(sXY + ei * 16);
+    const double zi = lds_d(sZ + ei * 8);
+    const uint32_t sTi = sTab + (uint32_t)(ti * a.nt) * 32u;
+    const double qi = lds_d(sQt + ti * 8);
+    const unsigned lj_mask = a.lj_mask[ti];
+    const bool lj_row = lj_mask != 0u;
+    double Fx = 0.0, Fy = 0.0, Fz = 0.0;
+
+    auto eval = [&](uint32_t entry) {
+      const uint32_t sj = entry & STG_IDX_MASK, tj = entry >> STG_IDX_BITS;
+      const double2 xyj = lds_d2(sXY + sj * 16);
+      const double zj = lds_d(sZ + sj * 8);
+      const double qq = qi * lds_d(sQt + tj * 8);
+      const double dx = xyi.x - xyj.x, dy = xyi.y - xyj.y, dz = zi - zj;
+      const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+      const bool in = r2 < a.rc2;
+      const double y = rsqrt_seeded(r2), y2 = y * y;
+      const double u = fma(r2, a.u_scale, -1.0);
+      double fr = qq * fma(y, y2 - a.fshift, -poly_eval(a.cS, u));
+      if (lj_row && __any_sync(0xffffffffu, (lj_mask >> tj) & 1u)) {
+        const double2 lj = lds_d2(sTi + tj * 32);        // 24 eps, sigma^2
+        const double s2 = lj.y * y2;
+        const double s6 = s2 * s2 * s2;
+        fr = fma(lj.x * y2, fma(s6 + s6, s6, -s6), fr);
+      }
+      fr = in ? fr : 0.0;
+      Fx = fma(fr, dx, Fx); Fy = fma(fr, dy, Fy); Fz = fma(fr, dz, Fz);
+      if (COUNT) hits += in ? 1ull : 0ull;
+    };
+
+    for (int m = 0; m < nblk; ++m) {
+      uint4 nxt = cur;
+      if (m + 1 < nblk) nxt = *reinterpret_cast<const uint4 *>(rowp + STG_BLOCK * (m + 1) + 8 * lane);
+      else if (more) nxt = *reinterpret_cast<const uint4 *>(rowp + (long long)istep * a.stride + 8 * lane);   // first block of the next row
+      const uint32_t w[4] = {cur.x, cur.y, cur.z, cur.w};
+      const int nst = min(8, (n - STG_BLOCK * m + 31) >> 5);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        if (j >= nst) break;
+        eval((j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu));
+      }
+      cur = nxt;
+    }
+    // (Fx, Fy, Fz) over the 32 lanes in 6 exchanges instead of 15: the halves of the warp first swap what the other
+    // one keeps (lower: x, y; upper: z), then quarters split x | y, then a plain butterfly; fixed order -> reproducible
+    {
+      const bool up = lane & 16, q = lane & 8;
+      const double r1 = __shfl_xor_sync(0xffffffffu, up ? Fx : Fz, 16);
+      const double r2 = __shfl_xor_sync(0xffffffffu, up ? Fy : 0.0, 16);
+      const double A = (up ? Fz : Fx) + r1, B = up ? 0.0 : Fy + r2;
+      double V = (q ? B : A) + __shfl_xor_sync(0xffffffffu, q ? A : B, 8);
+      V += __shfl_xor_sync(0xffffffffu, V, 4);
+      V += __shfl_xor_sync(0xffffffffu, V, 2);
+      V += __shfl_xor_sync(0xffffffffu, V, 1);
+      if ((lane & 7) == 0 && lane < 24) a.Fs[((long long)bead * a.N + slot) * 3 + (lane >> 3)] = V;
+    }
+  }
+  if (COUNT) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) hits += __shfl_xor_sync(0xffffffffu, hits, o);
+    if (lane == 0) atomicAdd(a.count, hits);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Pruned per-bead rows for k_pair_dense.  The centroid table (skin 2 A, shared by all beads, the list the
+// oracle is compared with) holds ~1.8x the pairs inside r_c.  k_prune copies, per contracted bead, the entries
+// within r_c + prune_skin of the bead's CURRENT positions into a second table (same blocked 16-bit row format,
+// dummy = dcap - 1) and records those positions (pref4).  The pruned rows of a bead stay complete while no atom
+// of that bead has moved by more than prune_skin / 2 since (k_prune_check, every step) and the centroid table has
+// not been rebuilt (pruned_at[bead] == rebuild count): both are tested on the device, no host round trip.
+// The prune test is the packed-half pre-test (conservative: it keeps every pair inside its radius).
+// ---------------------------------------------------------------------------------------------
+#define PRUNE_CHECK_CTAS 296
+#ifndef PRUNE_THREADS
+#define PRUNE_THREADS 512
+#endif
+#define PRUNE_WARPS (PRUNE_THREADS / 32)
+#define PRUNE_QUEUE (2 * STG_BLOCK)      // < 256 left over + 256 new entries per warp
+
+struct PruneArgs {
+  int N, Pc, nt, cap, bead0;     // cap = dcap of the dense kernel (dummy at cap - 1)
+  int nc[3];
+  double box[3], inv_box[3], cell_edge[3];
+  const double *pos4;            // [Pc][N][4] current contracted beads, slot order
+  double *pref4;                 // [Pc][N][4] positions the pruned rows were made from
+  const uint16_t *nbr16;         // centroid table [N][stride]
+  const int32_t *nbr_count, *cell_start;
+  uint16_t *nbr16p;              // [Pc][N][stride] pruned rows
+  int32_t *nbr_count_p;          // [Pc][N]
+  long long stride;
+  double *part;                  // [Pc][PRUNE_CHECK_CTAS] per-CTA maxima of |pos - pref|^2
+  long long *pruned_at;          // [Pc] rebuild count the pruned rows of the bead belong to (-1: none)
+  int *work;                     // [Pc] next cell of k_prune (zeroed by k_prune_check every step)
+  long long *nprune;             // [Pc] number of prunes of the bead so far (statistics)
+  const long long *counters;     // [0] = rebuild count
+  double move2;                  // (prune_skin / 2)^2
+  unsigned thr_h;                // packed-half threshold for r_c + prune_skin
+};
+
+// every step: per-bead maximum of the squared displacement since the last prune (fixed order, no atomics)
+__global__ void __launch_bounds__(256) k_prune_check(const PruneArgs a) {
+  __shared__ double red[8];
+  const int bead = a.bead0 + blockIdx.y;
+  const double4 *p = reinterpret_cast<const double4 *>(a.pos4) + (long long)bead * a.N;
+  const double4 *r = reinterpret_cast<const double4 *>(a.pref4) + (long long)bead * a.N;
+  double m = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < a.N; i += gridDim.x * blockDim.x) {
+    const double4 u = p[i], v = r[i];
+    const double dx = u.x - v.x, dy = u.y - v.y, dz = u.z - v.z;
+    const double d2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    m = (d2 > m || d2 != d2) ? d2 : m;                   // a NaN sticks: the comparison in k_prune then fails towards "prune"
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const double t = __shfl_xor_sync(0xffffffffu, m, o);
+    m = (t > m || t != t) ? t : m;
+  }
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) m = (red[w] > m || red[w] != red[w]) ? red[w] : m;
+    a.part[(long long)bead * PRUNE_CHECK_CTAS + blockIdx.x] = m;
+    if (blockIdx.x == 0) a.work[bead] = 0;
+  }
+}
+
+// the rows of bead `bead` must be pruned again (uniform over the grid: read-only inputs of this launch); all threads
+// of the CTA call it
+__device__ __forceinline__ bool prune_due(const PruneArgs &a, int bead) {
+  const int t = threadIdx.x;
+  int f = (t == 0) && (a.pruned_at[bead] != a.counters[0]);
+  if (t < PRUNE_CHECK_CTAS) f |= !(a.part[(long long)bead * PRUNE_CHECK_CTAS + t] < a.move2);   // NaN: prune
+  return __syncthreads_or(f) != 0;
+}
+
+__global__ void __launch_bounds__(PRUNE_THREADS, 2) k_prune(const PruneArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint2 *C = reinterpret_cast<uint2 *>(smem_raw);
+  uint32_t *queue = reinterpret_cast<uint32_t *>(C + a.cap);
+  __shared__ int off[28], cbeg[27], next_atom;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = blockDim.x;
+  const int bead = a.bead0 + blockIdx.y;
+  if (!prune_due(a, bead)) return;
+  if (blockIdx.x == 0 && tid == 0) a.nprune[bead] += 1;
+  // a small grid (the launch returns at once on most steps) takes the cells from a work counter
+  __shared__ int cell_s;
+  for (;;) {
+  __syncthreads();                                         // the previous cell's shared arrays are no longer read
+  if (tid == 0) cell_s = atomicAdd(&a.work[bead], 1);
+  __syncthreads();
+  const int cell = cell_s;
+  if (cell >= a.nc[0] * a.nc[1] * a.nc[2]) break;
+  const int cz = cell % a.nc[2], cy = (cell / a.nc[2]) % a.nc[1], cx = cell / (a.nc[2] * a.nc[1]);
+  if (tid < 27) {
+    const int ox = tid / 9, oy = (tid / 3) % 3, oz = tid % 3;
+    const int qx = (cx - 1 + ox + a.nc[0]) % a.nc[0], qy = (cy - 1 + oy + a.nc[1]) % a.nc[1],
+              qz = (cz - 1 + oz + a.nc[2]) % a.nc[2];
+    const int c2 = (qx * a.nc[1] + qy) * a.nc[2] + qz;
+    cbeg[tid] = a.cell_start[c2];
+    off[tid + 1] = a.cell_start[c2 + 1] - a.cell_start[c2];
+  }
+  __syncthreads();
+  if (tid == 0) {
+    next_atom = 0;
+    off[0] = 0;
+    for (int s = 0; s < 27; ++s) off[s + 1] += off[s];
+  }
+  __syncthreads();
+  const int total = off[27];
+  if (off[14] == off[13] || total > a.cap - 1) continue;   // the dense kernel reports the overflow
+  const double4 *pos = reinterpret_cast<const double4 *>(a.pos4) + (long long)bead * a.N;
+  {
+    const double ctr[3] = {(cx + 0.5) * a.cell_edge[0], (cy + 0.5) * a.cell_edge[1], (cz + 0.5) * a.cell_edge[2]};
+    const double MAGIC = 6755399441055744.0;
+    constexpr int UN = 4;
+    for (int g0 = tid; g0 < total; g0 += UN * nthr) {
+      double4 p[UN];
+      int s = 0;
+#pragma unroll
+      for (int u = 0; u < UN; ++u) {
+        const int g = g0 + u * nthr;
+        if (g < total) {
+          while (g >= off[s + 1]) ++s;
+          p[u] = pos[cbeg[s] + g - off[s]];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < UN; ++u) {
+        const int g = g0 + u * nthr;
+        if (g < total) {
+          double lx = p[u].x - ctr[0], ly = p[u].y - ctr[1], lz = p[u].z - ctr[2];
+          lx = fma(-a.box[0], (lx * a.inv_box[0] + MAGIC) - MAGIC, lx);
+          ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
+          lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
+          C[g] = half_record(lx, ly, lz);
+          if (g >= off[13] && g < off[14])               // home atoms: the reference of the displacement check
+            reinterpret_cast<double4 *>(a.pref4)[(long long)bead * a.N + cbeg[13] + g - off[13]] = p[u];
+        }
+      }
+    }
+  }
+  if (tid == 0) C[a.cap - 1] = half_record(1e9, 1e9, 1e9);  // the dummy: no test against it passes
+  __syncthreads();
+  const int h0 = off[13], nh = off[14] - off[13], slot0 = cbeg[13];
+  const uint32_t sC = (uint32_t)__cvta_generic_to_shared(C),
+                 sQ = (uint32_t)__cvta_generic_to_shared(queue) + warp * (PRUNE_QUEUE * 4);
+  unsigned lt;
+  asm volatile("mov.u32 %0, %%lanemask_lt;" : "=r"(lt));
+  const uint32_t dummy = (uint32_t)(a.cap - 1);
+  for (;;) {
+    int t = 0;
+    if (lane == 0) t = atomicAdd(&next_atom, 1);
+    const int ii = __shfl_sync(0xffffffffu, t, 0);
+    if (ii >= nh) break;
+    const long long slot = slot0 + ii;
+    const int n = a.nbr_count[slot];
+    const uint16_t *rowp = a.nbr16 + slot * a.stride;
+    uint16_t *outp = a.nbr16p + ((long long)bead * a.N + slot) * a.stride;
+    const int nblk = (n + STG_BLOCK - 1) / STG_BLOCK;
+    uint4 cur = make_uint4(0u, 0u, 0u, 0u);
+    if (nblk > 0) cur = *reinterpret_cast<const uint4 *>(rowp + 8 * lane);
+    const uint2 ci = lds_u2(sC + (uint32_t)(h0 + ii) * 8);
+    uint32_t qa = sQ;
+    int written = 0;
+    // one 256-entry block of the pruned row from the first 256 queue slots (lane l: entries 32 j + l, j = 0..7)
+    auto flush = [&]() {
+      uint32_t e[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) e[j] = lds_u(sQ + (32 * j + lane) * 4);
+      *reinterpret_cast<uint4 *>(outp + written + 8 * lane) =
+          make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
+    };
+    for (int m = 0; m < nblk; ++m) {
+      uint4 nxt = cur;
+      if (m + 1 < nblk) nxt = *reinterpret_cast<const uint4 *>(rowp + STG_BLOCK * (m + 1) + 8 * lane);
+      const uint32_t w[4] = {cur.x, cur.y, cur.z, cur.w};
+      auto entry = [&](int j) { return (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu); };
+      const int nst = min(8, (n - STG_BLOCK * m + 31) >> 5);
+      // the centroid table pads its rows with the dummy of the LARGER staged array of k_pair_staged: clamp to ours
+      auto rec = [&](int j) { return sC + min(entry(j) & STG_IDX_MASK, dummy) * 8; };
+      uint2 cj = lds_u2(rec(0));
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        if (j >= nst) break;
+        const uint32_t e = entry(j);
+        const bool hit = half_test(ci, cj, a.thr_h);
+        if (j < 7) cj = lds_u2(rec(j + 1));
+        unsigned mask;
+        asm volatile("{ .reg .pred p; setp.ne.u32 p, %1, 0; vote.sync.ballot.b32 %0, p, 0xffffffff; }" : "=r"(mask) : "r"((unsigned)hit));
+        if (hit) sts_u(qa + __popc(mask & lt) * 4, e);
+        qa += __popc(mask) * 4;
+      }
+      __syncwarp();
+      if (qa >= sQ + STG_BLOCK * 4) {
+        flush();
+        written += STG_BLOCK;
+        qa -= STG_BLOCK * 4;
+        uint32_t v[8];                                     // < 256 entries left over: to the front of the queue
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = lds_u(sQ + (STG_BLOCK + 32 * k + lane) * 4);
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+          if (sQ + (32 * k + lane) * 4 < qa) sts_u(sQ + (32 * k + lane) * 4, v[k]);
+        __syncwarp();
+      }
+      cur = nxt;
+    }
+    const int cnt = (int)(qa - sQ) >> 2;                   // < 256
+    if (cnt > 0) {
+      const int pad = (cnt + 31) & ~31;
+      if (cnt + lane < pad) sts_u(qa + lane * 4, dummy);   // the last 32-entry step is completed with the dummy
+      __syncwarp();
+      flush();                                             // entries behind `pad` are never read (row count)
+      __syncwarp();
+    }
+    if (lane == 0) a.nbr_count_p[(long long)bead * a.N + slot] = written + cnt;
+  }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
 // S(w) = (4/sqrt(pi)) sum_k (-1)^k w^k / (k! (2k+3)),  E(w) = (2/sqrt(pi)) sum_k (-1)^k w^k / (k! (2k+1)):
@@ -376,6 +779,30 @@ static long double fit_poly(int which, long double wmax, long double scale, doub
     if (err > worst) worst = err;
   }
   return worst;
+}
+
+// fp16 pre-test threshold for radius r: r^2 + a bound on the error of the packed-half r^2, rounded UP to a half,
+// both halves of a half2.  Staged coordinates reach 1.5 cell edges + skin: rounding them to half moves each by
+// <= ulp(cmax)/2; the half difference of two records adds <= ulp(r + 1)/2; so each component of d is off by e_d,
+// r^2 by <= 2 sqrt(3) r' e_d + 3 e_d^2 (r' = r + 1 covers the margin itself); the product, the fma, the sum and
+// the rounding of the threshold add <= 4 half-ulps at r^2 + margin.  The float -> half double rounding of the
+// staging adds 2^-13 relative to the half-ulp (the 1.01).  Only pairs certainly outside r are rejected.
+static unsigned half_threshold(const qhp_system *s, double r, double *thr_out) {
+  auto ulp16 = [](double v) { int e; frexp(v, &e); return ldexp(1.0, e - 11); };   // spacing of halves just below 2^e >= v
+  double cmax = 0.0;
+  for (int d = 0; d < 3; ++d) cmax = fmax(cmax, 1.5 * s->box[d] / s->nc[d] + s->skin + 1.0);
+  const double e_d = 1.01 * (ulp16(cmax) + 0.5 * ulp16(r + 1.0));
+  double thr = r * r + 2.0 * sqrt(3.0) * (r + 1.0) * e_d + 3.0 * e_d * e_d;
+  thr += 2.0 * ulp16(thr + 4.0);
+  __half h = __double2half(thr);                                        // round to nearest, then step up if it fell below
+  if (__half2float(h) < thr) {
+    unsigned short b = *reinterpret_cast<unsigned short *>(&h);
+    ++b;
+    h = *reinterpret_cast<__half *>(&b);
+  }
+  const unsigned short hb = *reinterpret_cast<unsigned short *>(&h);
+  if (thr_out) *thr_out = (double)__half2float(h);
+  return (unsigned)hb | ((unsigned)hb << 16);
 }
 
 static size_t staged_atom_bytes(bool f32) { return 3 * sizeof(double) + (f32 ? sizeof(uint2) : 0); }
@@ -437,8 +864,90 @@ bool qhp_pair_staged_fit(qhp_system *s, long long region) {
   return false;
 }
 
-int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned long long *count, int bead0, int nbeads) {
-  StagedArgs a{};
+static size_t dense_tab_bytes(const qhp_system *s) { return sizeof(double) * ((size_t)s->nt * s->nt * 4 + (size_t)s->nt + 1); }
+
+void qhp_pair_dense_free(qhp_system *s) {
+  if (s->nbr16p) cudaFree(s->nbr16p);
+  if (s->nbr_count_p) cudaFree(s->nbr_count_p);
+  if (s->pref4) cudaFree(s->pref4);
+  if (s->prune_part) cudaFree(s->prune_part);
+  if (s->pruned_at) cudaFree(s->pruned_at);
+  if (s->prune_work) cudaFree(s->prune_work);
+  s->nbr16p = nullptr; s->nbr_count_p = nullptr; s->pref4 = nullptr; s->prune_part = nullptr; s->pruned_at = nullptr; s->prune_work = nullptr;
+  s->nbr16p_stride = 0;
+}
+
+// Called at every synchronising list build (after the table and its stride are final): the pruned-row path serves
+// the system when the staged kernel does, prune_skin > 0, and the densest neighbourhood leaves room for TWO
+// k_pair_dense CTAs per SM (24 B per staged atom); allocates the per-bead tables and marks them stale.
+int qhp_pair_dense_prepare(qhp_system *s, long long region) {
+  s->dense = false;
+  if (!s->staged || !s->staged_f32 || !(s->prune_skin > 0.0) || s->prune_skin >= s->skin) return QHP_OK;
+  int sm_bytes = 0;
+  QHP_CUDA_OK(s, cudaDeviceGetAttribute(&sm_bytes, cudaDevAttrMaxSharedMemoryPerMultiprocessor, s->device));
+  const long long dyn = (long long)sm_bytes / DNS_CTAS - 1024 - 256;   // per-CTA reserve + the static shared variables
+  long long cap = (dyn - (long long)dense_tab_bytes(s)) / 24;
+  if (cap > (1 << STG_IDX_BITS)) cap = 1 << STG_IDX_BITS;
+  cap &= ~3LL;
+  if (cap < region + region / 32 + 32 + 1) return QHP_OK;               // one CTA per SM: the pre-test kernel is the better one
+  s->dense_cap = (int)cap;
+  const size_t PcN = (size_t)s->Pc * (size_t)s->N;
+  if (!s->nbr16p || s->nbr16p_stride != s->nbr_stride) {
+    qhp_pair_dense_free(s);
+    cudaError_t e = cudaMalloc(&s->nbr16p, sizeof(uint16_t) * PcN * (size_t)s->nbr_stride);
+    if (e == cudaSuccess) e = cudaMalloc(&s->nbr_count_p, sizeof(int32_t) * PcN);
+    if (e == cudaSuccess) e = cudaMalloc(&s->pref4, sizeof(double) * 4 * PcN);
+    if (e == cudaSuccess) e = cudaMalloc(&s->prune_part, sizeof(double) * (size_t)s->Pc * PRUNE_CHECK_CTAS);
+    if (e == cudaSuccess) e = cudaMalloc(&s->pruned_at, sizeof(long long) * 2 * (size_t)s->Pc);      // + [Pc] prune counts
+    if (e == cudaSuccess) e = cudaMalloc(&s->prune_work, sizeof(int) * (size_t)s->Pc);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      qhp_pair_dense_free(s);                                          // not fatal: the pre-test kernel serves the system
+      return QHP_OK;
+    }
+    s->nbr16p_stride = s->nbr_stride;
+    QHP_CUDA_OK(s, cudaMemsetAsync(s->pref4, 0, sizeof(double) * 4 * PcN, s->stream));
+    QHP_CUDA_OK(s, cudaMemsetAsync(s->prune_part, 0, sizeof(double) * (size_t)s->Pc * PRUNE_CHECK_CTAS, s->stream));
+    QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_dense<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+    QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_dense<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+    QHP_CUDA_OK(s, cudaFuncSetAttribute(k_prune, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+  }
+  QHP_CUDA_OK(s, cudaMemsetAsync(s->pruned_at, 0xff, sizeof(long long) * (size_t)s->Pc, s->stream));   // -1: stale
+  QHP_CUDA_OK(s, cudaMemsetAsync(s->pruned_at + s->Pc, 0, sizeof(long long) * (size_t)s->Pc, s->stream));
+  s->dense = true;
+  return QHP_OK;
+}
+
+// check (every step) -> prune (returns at once unless due) -> evaluation of the pruned rows
+static int pair_dense_forces(qhp_system *s, StagedArgs &a, int bead0, int nbeads, bool count = false) {
+  PruneArgs p{};
+  p.N = s->N; p.Pc = s->Pc; p.nt = s->nt; p.cap = s->dense_cap; p.bead0 = bead0;
+  for (int d = 0; d < 3; ++d) {
+    p.nc[d] = s->nc[d]; p.box[d] = s->box[d]; p.inv_box[d] = s->inv_box[d]; p.cell_edge[d] = s->box[d] / s->nc[d];
+  }
+  p.pos4 = s->pos4; p.pref4 = s->pref4; p.nbr16 = s->nbr16; p.nbr_count = s->nbr_count; p.cell_start = s->cell_start;
+  p.nbr16p = s->nbr16p; p.nbr_count_p = s->nbr_count_p; p.stride = s->nbr_stride;
+  p.part = s->prune_part; p.pruned_at = s->pruned_at; p.work = s->prune_work; p.nprune = s->pruned_at + s->Pc; p.counters = (const long long *)s->counters;
+  p.move2 = 0.25 * s->prune_skin * s->prune_skin;
+  p.thr_h = half_threshold(s, s->r_cut + s->prune_skin, nullptr);
+  k_prune_check<<<dim3(PRUNE_CHECK_CTAS, (unsigned)nbeads), 256, 0, s->stream>>>(p);
+  QHP_LAUNCH_OK(s);
+  const size_t psm = (size_t)s->dense_cap * sizeof(uint2) + sizeof(uint32_t) * PRUNE_WARPS * PRUNE_QUEUE;
+  k_prune<<<dim3((unsigned)(s->ncell < PRUNE_CHECK_CTAS ? s->ncell : PRUNE_CHECK_CTAS), (unsigned)nbeads), PRUNE_THREADS, psm, s->stream>>>(p);
+  QHP_LAUNCH_OK(s);
+  a.dcap = s->dense_cap;
+  a.nbr16 = s->nbr16p; a.nbr_count = s->nbr_count_p;
+  a.list_bead_stride = (long long)s->N * s->nbr_stride; a.count_bead_stride = s->N;
+  a.pruned_at = s->pruned_at;
+  const size_t sm = (size_t)s->dense_cap * 24 + dense_tab_bytes(s);
+  const dim3 grid((unsigned)(s->ncell * s->staged_split), (unsigned)nbeads);
+  if (count) k_pair_dense<true><<<grid, DNS_THREADS, sm, s->stream>>>(a);
+  else k_pair_dense<false><<<grid, DNS_THREADS, sm, s->stream>>>(a);
+  QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+static int staged_args(qhp_system *s, StagedArgs &a, double *part, unsigned long long *count, int bead0) {
   a.bead0 = bead0;
   a.N = s->N; a.Pc = s->Pc; a.nt = s->nt; a.split = s->staged_split; a.cap = s->staged_cap;
   for (int d = 0; d < 3; ++d) {
@@ -451,29 +960,7 @@ int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned lo
   a.rc = rc; a.rc2 = rc * rc; a.u_scale = 2.0 / (rc * rc);
   a.erfc_rc = erfc(al * rc) / rc;
   a.fshift = erfc(al * rc) / (rc * rc) + 2.0 * al / sqrt(QHP_PI) * exp(-al * al * rc * rc) / rc;
-  {
-    // fp16 pre-test threshold = r_c^2 + a bound on the error of the packed-half r^2, rounded UP to a half.
-    // Staged coordinates reach 1.5 cell edges + skin: rounding them to half moves each by <= ulp(cmax)/2; the half
-    // difference of two records adds <= ulp(r_c + 1)/2; so each component of d is off by e_d, r^2 by
-    // <= 2 sqrt(3) r_c' e_d + 3 e_d^2 (r_c' = r_c + 1 covers the margin itself); the product, the fma, the sum and the
-    // rounding of the threshold add <= 4 half-ulps at r_c^2 + margin.  The float -> half double rounding of the
-    // staging adds 2^-13 relative to the half-ulp (the 1.01).  Pairs certainly outside r_c are the only ones rejected.
-    auto ulp16 = [](double v) { int e; frexp(v, &e); return ldexp(1.0, e - 11); };   // spacing of halves just below 2^e >= v
-    double cmax = 0.0;
-    for (int d = 0; d < 3; ++d) cmax = fmax(cmax, 1.5 * a.cell_edge[d] + s->skin + 1.0);
-    const double e_d = 1.01 * (ulp16(cmax) + 0.5 * ulp16(rc + 1.0));
-    double thr = rc * rc + 2.0 * sqrt(3.0) * (rc + 1.0) * e_d + 3.0 * e_d * e_d;
-    thr += 2.0 * ulp16(thr + 4.0);
-    __half h = __double2half(thr);                                      // round to nearest, then step up if it fell below
-    if (__half2float(h) < thr) {
-      unsigned short b = *reinterpret_cast<unsigned short *>(&h);
-      ++b;
-      h = *reinterpret_cast<__half *>(&b);
-    }
-    const unsigned short hb = *reinterpret_cast<unsigned short *>(&h);
-    a.rc2h = (unsigned)hb | ((unsigned)hb << 16);
-    s->staged_thr = (double)__half2float(h);
-  }
+  a.rc2h = half_threshold(s, rc, &s->staged_thr);
   for (int k = 0; k < QHP_NPOLY; ++k) { a.cS[k] = s->polyS[k]; a.cE[k] = s->polyE[k]; }
   for (int t = 0; t < s->nt; ++t) {
     a.qs[t] = sqrt(QHP_COUL) * s->charge[t];
@@ -482,7 +969,15 @@ int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned lo
       if (s->lj_eps[t] > 0 && s->lj_eps[u] > 0) a.lj_mask[t] |= 1u << u;
   }
   a.part = part; a.count = count; a.counters = (long long *)s->counters;
+  return QHP_OK;
+}
+
+int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned long long *count, int bead0, int nbeads) {
+  StagedArgs a{};
+  const int rc0 = staged_args(s, a, part, count, bead0);
+  if (rc0) return rc0;
   const dim3 grid((unsigned)(s->ncell * s->staged_split), (unsigned)nbeads);
+  if (!energy && s->dense) return pair_dense_forces(s, a, bead0, nbeads);
   const size_t smem = staged_smem_bytes(s->staged_cap, s->staged_warps, s->staged_f32);
   const int threads = 32 * s->staged_warps;
   if (s->staged_f32) {
@@ -493,5 +988,42 @@ int qhp_pair_staged_forces(qhp_system *s, bool energy, double *part, unsigned lo
     else k_pair_staged<false, false><<<grid, threads, smem, s->stream>>>(a);
   }
   QHP_LAUNCH_OK(s);
+  return QHP_OK;
+}
+
+__global__ void k_sum_counts(const int32_t *__restrict__ c, long long n, unsigned long long *out) {
+  unsigned long long v = 0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) v += (unsigned long long)c[i];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0 && v) atomicAdd(out, v);
+}
+
+// parity hook (include/qhp.h qhp_pair_prune_stats): the pruned rows are made current for the present state (exactly what
+// a step does), V_s is evaluated through them with the counting variant of the kernel
+int qhp_pair_prune_stats_impl(qhp_system *s, int64_t *out_host) {
+  out_host[0] = s->staged && s->dense ? 1 : 0;
+  out_host[1] = out_host[2] = out_host[3] = 0;
+  if (!out_host[0]) return QHP_OK;
+  unsigned long long *cnt = (unsigned long long *)&s->counters[3];
+  QHP_CUDA_OK(s, cudaMemsetAsync(cnt, 0, sizeof(int64_t), s->stream));
+  StagedArgs a{};
+  int rc = staged_args(s, a, nullptr, cnt, 0);
+  if (rc) return rc;
+  rc = pair_dense_forces(s, a, 0, s->Pc, true);
+  if (rc) return rc;
+  long long hits = 0, entries = 0;
+  std::vector<long long> np(s->Pc);
+  QHP_CUDA_OK(s, cudaMemcpyAsync(&hits, cnt, sizeof(long long), cudaMemcpyDeviceToHost, s->stream));
+  QHP_CUDA_OK(s, cudaMemsetAsync(cnt, 0, sizeof(int64_t), s->stream));
+  k_sum_counts<<<296, 256, 0, s->stream>>>(s->nbr_count_p, (long long)s->Pc * s->N, cnt);
+  QHP_LAUNCH_OK(s);
+  QHP_CUDA_OK(s, cudaMemcpyAsync(&entries, cnt, sizeof(long long), cudaMemcpyDeviceToHost, s->stream));
+  QHP_CUDA_OK(s, cudaMemcpyAsync(np.data(), s->pruned_at + s->Pc, sizeof(long long) * s->Pc, cudaMemcpyDeviceToHost, s->stream));
+  QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
+  out_host[1] = 0;
+  for (long long v : np) out_host[1] += v;
+  out_host[2] = entries;
+  out_host[3] = hits;
   return QHP_OK;
 }

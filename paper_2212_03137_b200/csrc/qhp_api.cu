@@ -288,6 +288,7 @@ extern "C" int qhp_destroy(qhp_system *s) {
                   s->red, s->obs, s->gamma, s->Hf, s->hk, s->H4, s->Fc, s->vseg, s->tw, s->seg_slot, s->slot_atom,
                   s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p, s->ratio_tau, s->ratio_avv, s->ratio_avf, s->kappa};
   for (void *p : ptrs) if (p) cudaFree(p);
+  qhp_pair_dense_free(s);
   delete s;
   return QHP_OK;
 }
@@ -475,6 +476,23 @@ extern "C" int qhp_set_contraction(qhp_system *s, int variant) {
   QHP_CUDA_OK(s, cudaMemcpyAsync(s->d_Tc, s->T_Pc.data(), sizeof(double) * s->T_Pc.size(), cudaMemcpyHostToDevice, s->stream));
   QHP_CUDA_OK(s, cudaStreamSynchronize(s->stream));
   return QHP_OK;
+}
+
+extern "C" int qhp_set_pair_prune(qhp_system *s, double prune_skin) {
+  if (!s) return QHP_EINVAL;
+  if (!(prune_skin == prune_skin)) { s->err = "qhp_set_pair_prune: prune_skin is NaN"; return QHP_EINVAL; }
+  if (s->have_state) { s->err = "qhp_set_pair_prune: call before qhp_set_state"; return QHP_ESTATE; }
+  s->prune_skin = prune_skin;
+  return QHP_OK;
+}
+
+extern "C" int qhp_pair_prune_stats(qhp_system *s, int64_t *out_host) {
+  if (!s || !out_host) return QHP_EINVAL;
+  if (!s->have_state) { s->err = "no state"; return QHP_ESTATE; }
+  const int64_t launches = s->n_launch;       // this call's own launches are not counted
+  const int rc = qhp_pair_prune_stats_impl(s, out_host);
+  s->n_launch = launches;
+  return rc;
 }
 
 extern "C" int qhp_set_a_block(qhp_system *s, int kind) {

@@ -98,6 +98,17 @@ struct qhp_system {
   bool staged_f32 = true;                  // the staged kernel keeps an 8-byte fp16 copy for the packed-half pre-test (else fp64 pre-test)
   double staged_thr = 0.0;                 // threshold of that pre-test (r_c^2 + its error bound, a half)
   int staged_split = 1;                    // CTAs per (cell, bead)
+  // pruned per-bead rows + evaluation without pre-test (k_prune, k_pair_dense in pair_staged.cu)
+  double prune_skin = 0.5;                 // A; <= 0: off (qhp_set_pair_prune)
+  bool dense = false;                      // in use (decided with `staged` at the synchronising list build)
+  int dense_cap = 0;                       // staged atoms of k_pair_dense (two CTAs per SM)
+  uint16_t *nbr16p = nullptr;              // [Pc][N][nbr_stride] pruned rows
+  int32_t *nbr_count_p = nullptr;          // [Pc][N]
+  int64_t nbr16p_stride = 0;               // stride the pruned table was allocated for
+  double *pref4 = nullptr;                 // [Pc][N][4] bead positions at the last prune
+  double *prune_part = nullptr;            // [Pc][PRUNE_CHECK_CTAS] displacement maxima of k_prune_check
+  long long *pruned_at = nullptr;          // [Pc] rebuild count the pruned rows belong to (-1: none)
+  int *prune_work = nullptr;               // [Pc] work counters of k_prune
   double polyS[QHP_NPOLY]{}, polyE[QHP_NPOLY]{};   // alpha^3 S(w), alpha E(w) in u = 2 r^2/rc^2 - 1
   unsigned long long *d2max = nullptr;     // [2] double bits, max |xc - cref|^2, double-buffered by step parity
   int64_t *counters = nullptr;             // [8] device: 0 rebuilds, 1 overflow flag, 2 max row count, 3 in-cutoff count, 6 skin-too-small flag
@@ -171,6 +182,9 @@ int qhp_pair_forces(qhp_system *s, bool energy);     // pos4 -> Fs (+ U_s, count
 int qhp_pair_forces_beads(qhp_system *s, bool energy, int bead0, int nbeads);   // the launch of one bead slice
 int qhp_pair_setup(qhp_system *s);                   // polynomial tables, staged-kernel geometry
 bool qhp_pair_staged_fit(qhp_system *s, long long region);  // CTA size / capacity for a neighbourhood size
+int qhp_pair_dense_prepare(qhp_system *s, long long region); // pruned-row path: decide, (re)allocate, invalidate
+void qhp_pair_dense_free(qhp_system *s);
+int qhp_pair_prune_stats_impl(qhp_system *s, int64_t *out_host);
 int qhp_pair_partials(const qhp_system *s);          // upper bound of per-CTA energy partials
 // qtb.cu
 int qhp_qtb_init(qhp_system *s);
