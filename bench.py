@@ -244,10 +244,12 @@ def time_workload(sysg, cfg, top, x0, p0, K, args, world, local, dist_barrier):
         dist_barrier()
     ms = e0.elapsed_time(e1)
     prof = sysg.profile_read()
+    prof_pair = sysg.profile_read_pair()
     sysg.profile(False)
     c1 = sysg.counters()
+    prune = sysg.pair_prune_stats()
     ms = max_over_ranks(ms, world)
-    out = dict(ms=ms, prof=prof, c0=c0, c1=c1, clocks=clk.summary(), launches=int(c1["launches"] - c0["launches"]),
+    out = dict(ms=ms, prof=prof, prof_pair=prof_pair, prune=prune, c0=c0, c1=c1, clocks=clk.summary(), launches=int(c1["launches"] - c0["launches"]),
                value=job_throughput(world, N, P, K, ms * 1e-3), ns_day=K * cfg["dt_fs"] * 1e-6 / (ms * 1e-3) * 86400.0)
     return out
 
@@ -285,17 +287,30 @@ def kernel_blocks(cfg, N, m, pk, dfma_tf, amortised=None):
     """Per-kernel roofline blocks {ms, units, achieved, peak, frac} from the library's per-phase CUDA events."""
     P, Pc, prof, c1, c0 = cfg["P"], cfg["P_contract"], m["prof"], m["c1"], m["c0"]
     per = lambda k: prof[k]["ms"] / max(prof[k]["n"], 1)
-    pair_ms, int_ms = per("pair"), per("integrate")
+    phase_ms, int_ms = per("pair"), per("integrate")
     pair_beads = c1["pair_beads_in_cutoff"]             # ordered (full list): each pair from both sides
     flops = 0.5 * pair_beads * FLOP_PER_PAIR_BEAD       # algorithmic: every unordered pair-bead once
+    pp, dense = m.get("prof_pair"), bool(m.get("prune", {}).get("active"))
+    if dense:       # pruned-row path: the dominant kernel is k_pair_dense, timed launch by launch inside the pair phase
+        kname = "k_pair_dense"
+        pair_ms = pp[kname]["ms"] / max(pp[kname]["n"], 1)
+    else:
+        kname = "k_pair_staged" if c1.get("staged") else "k_pair"
+        pair_ms = phase_ms
     ach = flops / (pair_ms * 1e-3) / 1e12 if pair_ms > 0 else 0.0
-    kname = "k_pair_staged" if c1.get("staged") else "k_pair"
     tr = NCU_TRAFFIC.get((cfg["name"], kname))
     pair = dict(kernel=kname, bound="alu", ms_per_launch=pair_ms, units=0.5 * pair_beads, unit_name="unordered in-cutoff pair-beads",
                 flop_per_unit=FLOP_PER_PAIR_BEAD, achieved=ach, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s", frac=ach / FP64_PEAK_TFLOPS,
                 peak_source="derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz", peak_measured=dfma_tf,
                 frac_of_measured=ach / dfma_tf if dfma_tf > 0 else None, executed_tflops=2.0 * ach,
                 traffic=tr[0] if tr else None, traffic_source=tr[1] if tr else None)
+    if dense:
+        steps = max(pp[kname]["n"], 1)
+        pair["pair_phase"] = dict(ms_per_step=phase_ms, frac_of_phase=flops / (phase_ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                                  k_prune_check_ms_per_step=pp["k_prune_check"]["ms"] / steps,
+                                  k_prune_ms_per_step=pp["k_prune"]["ms"] / steps,
+                                  pruned_entries_per_pair_bead=m["prune"]["entries"] / max(pair_beads, 1),
+                                  what="V_s per step = k_prune_check + k_prune (returns at once unless a bead's rows are due) + k_pair_dense")
     if P == 1:      # adQTB / classical step (Q1): 7 x 8 B per DOF + 56 B per atom (pos4 write, Fs read)
         int_bytes, iname = 7.0 * 8 * 3 * N + 56.0 * N, "k_integrate_mol1"
     else:           # fused RPMD pass: 4 x 8 B per (DOF, bead) + (32 + 24) B x P' per atom
@@ -459,7 +474,7 @@ def main():
         if adqtb is not None:
             adqtb["cpu_baseline"] = cpu_baseline(workload("C3"))
 
-    pair_block = kernels["k_pair_staged"] if "k_pair_staged" in kernels else kernels["k_pair"]
+    pair_block = next(kernels[k] for k in ("k_pair_dense", "k_pair_staged", "k_pair") if k in kernels)
     roofline = dict(pair_block, note="achieved counts each unordered in-cutoff pair-bead once (110 flop); the kernel "
                                      "evaluates both directions (full list, no atomics), see executed_tflops; "
                                      "peak_measured = live qhp_dfma_probe")

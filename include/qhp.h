@@ -231,6 +231,9 @@ int qhp_counters(qhp_system *sys, int64_t *out_host, int n_out);
  * HOST pointers. */
 int qhp_profile(qhp_system *sys, int enable);
 int qhp_profile_read(qhp_system *sys, double *ms_host, int64_t *n_host);
+/* The pair-force phase launch by launch, from the same recording: ms_host[0..2], n_host[0..2] = {k_prune_check,
+ * k_prune, k_pair_dense} (all 0 when the pruned-row path does not serve the system).  HOST pointers; synchronises. */
+int qhp_profile_read_pair(qhp_system *sys, double *ms_host, int64_t *n_host);
 /* Synchronise the stream and report sticky CUDA / overflow errors. */
 int qhp_check(qhp_system *sys);
 const char *qhp_last_error(const qhp_system *sys); /* sys may be NULL: last error of a call without a handle

@@ -18,7 +18,7 @@ SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_respa", "qhp_set_a_block", "qhp
            "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
            "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma", "qhp_adqtb_ratio", "qhp_adqtb_kappa",
            "qhp_adqtb_segment", "qhp_counters", "qhp_profile", "qhp_profile_read", "qhp_check", "qhp_last_error", "qhp_philox_normals",
-           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar", "qhp_pibar_noalloc", "qhp_set_comm", "qhp_pair_slices", "qhp_set_pair_prune", "qhp_pair_prune_stats"]
+           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar", "qhp_pibar_noalloc", "qhp_set_comm", "qhp_pair_slices", "qhp_set_pair_prune", "qhp_pair_prune_stats", "qhp_profile_read_pair"]
 
 
 # int fn(void *ctx, void *device_buf, size_t bytes_per_rank, int rank, int world, void *cuda_stream)  (include/qhp.h)
@@ -116,6 +116,7 @@ def lib():
         L.qhp_pibar.argtypes = [vp, i64, vp, i64, C.c_double, i32, C.c_double, vp, C.POINTER(C.c_double), C.POINTER(i32)]
         L.qhp_set_pair_prune.argtypes = [vp, C.c_double]
         L.qhp_pair_prune_stats.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.qhp_profile_read_pair.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.qhp_pibar_noalloc.argtypes = [vp, i64, vp, i64, C.c_double, i32, C.c_double, vp, vp]
         for name in SYMBOLS:
             if name != "qhp_last_error":
@@ -365,6 +366,12 @@ class System:
 
     def profile(self, enable: bool):
         self._ok(self._L.qhp_profile(self._h, int(bool(enable))))
+
+    def profile_read_pair(self) -> dict:
+        ms, n = (C.c_double * 3)(), (C.c_int64 * 3)()
+        self._ok(self._L.qhp_profile_read_pair(self._h, ms, n))
+        keys = ["k_prune_check", "k_prune", "k_pair_dense"]
+        return {k: dict(ms=float(ms[i]), n=int(n[i])) for i, k in enumerate(keys)}
 
     def profile_read(self) -> dict:
         ms, n = (C.c_double * 5)(), (C.c_int64 * 5)()

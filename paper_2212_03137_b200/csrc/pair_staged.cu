@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const Stag
   double *Z = reinterpret_cast<double *>(XY + a.dcap);
   double *tab = reinterpret_cast<double *>(Z + a.dcap);
   double *qtab = tab + a.nt * a.nt * 4;                     // tables sized by the number of types: room for staged atoms
-  __shared__ int off[28], cbeg[27], next_atom;
+  __shared__ int off[28], cbeg[27];
 
   const int tid = threadIdx.x, lane = tid & 31, nthr = blockDim.x;
   const int cell = blockIdx.x / a.split, part = blockIdx.x % a.split, bead = a.bead0 + blockIdx.y;
@@ -370,7 +370,6 @@ __global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const Stag
   }
   __syncthreads();
   if (tid == 0) {
-    next_atom = 0;
     off[0] = 0;
     for (int s = 0; s < 27; ++s) off[s + 1] += off[s];
   }
@@ -930,10 +929,16 @@ static int pair_dense_forces(qhp_system *s, StagedArgs &a, int bead0, int nbeads
   p.part = s->prune_part; p.pruned_at = s->pruned_at; p.work = s->prune_work; p.nprune = s->pruned_at + s->Pc; p.counters = (const long long *)s->counters;
   p.move2 = 0.25 * s->prune_skin * s->prune_skin;
   p.thr_h = half_threshold(s, s->r_cut + s->prune_skin, nullptr);
-  k_prune_check<<<dim3(PRUNE_CHECK_CTAS, (unsigned)nbeads), 256, 0, s->stream>>>(p);
+  {
+    qhp_prof_scope ps(s, 5);
+    k_prune_check<<<dim3(PRUNE_CHECK_CTAS, (unsigned)nbeads), 256, 0, s->stream>>>(p);
+  }
   QHP_LAUNCH_OK(s);
   const size_t psm = (size_t)s->dense_cap * sizeof(uint2) + sizeof(uint32_t) * PRUNE_WARPS * PRUNE_QUEUE;
-  k_prune<<<dim3((unsigned)(s->ncell < PRUNE_CHECK_CTAS ? s->ncell : PRUNE_CHECK_CTAS), (unsigned)nbeads), PRUNE_THREADS, psm, s->stream>>>(p);
+  {
+    qhp_prof_scope ps(s, 6);
+    k_prune<<<dim3((unsigned)(s->ncell < PRUNE_CHECK_CTAS ? s->ncell : PRUNE_CHECK_CTAS), (unsigned)nbeads), PRUNE_THREADS, psm, s->stream>>>(p);
+  }
   QHP_LAUNCH_OK(s);
   a.dcap = s->dense_cap;
   a.nbr16 = s->nbr16p; a.nbr_count = s->nbr_count_p;
@@ -941,8 +946,11 @@ static int pair_dense_forces(qhp_system *s, StagedArgs &a, int bead0, int nbeads
   a.pruned_at = s->pruned_at;
   const size_t sm = (size_t)s->dense_cap * 24 + dense_tab_bytes(s);
   const dim3 grid((unsigned)(s->ncell * s->staged_split), (unsigned)nbeads);
-  if (count) k_pair_dense<true><<<grid, DNS_THREADS, sm, s->stream>>>(a);
-  else k_pair_dense<false><<<grid, DNS_THREADS, sm, s->stream>>>(a);
+  {
+    qhp_prof_scope ps(s, 7);
+    if (count) k_pair_dense<true><<<grid, DNS_THREADS, sm, s->stream>>>(a);
+    else k_pair_dense<false><<<grid, DNS_THREADS, sm, s->stream>>>(a);
+  }
   QHP_LAUNCH_OK(s);
   return QHP_OK;
 }

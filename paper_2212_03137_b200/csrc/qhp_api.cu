@@ -382,24 +382,14 @@ static int prof_drain(qhp_system *s) {
   s->prof_kind.clear();
   return QHP_OK;
 }
-struct prof_scope {
-  qhp_system *s; bool on;
-  prof_scope(qhp_system *s_, int kind) : s(s_), on(s_->prof) {
-    if (!on) return;
-    cudaEvent_t a, b;
-    cudaEventCreate(&a); cudaEventCreate(&b);
-    s->prof_ev.push_back(a); s->prof_ev.push_back(b); s->prof_kind.push_back(kind);
-    cudaEventRecord(a, s->stream);
-  }
-  ~prof_scope() { if (on) cudaEventRecord(s->prof_ev.back(), s->stream); }
-};
+typedef qhp_prof_scope prof_scope;
 
 extern "C" int qhp_profile(qhp_system *s, int enable) {
   if (!s) return QHP_EINVAL;
   if (enable) {
     int rc = prof_drain(s);
     if (rc) return rc;
-    for (int k = 0; k < 5; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
+    for (int k = 0; k < 8; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
   }
   s->prof = enable != 0;
   return QHP_OK;
@@ -644,6 +634,14 @@ extern "C" int qhp_adqtb_segment(qhp_system *s, double *Fc, double *vseg) {
   if (Fc) rc = qhp_qtb_export_segment(s, s->Fc, Fc);
   if (!rc && vseg) rc = qhp_qtb_export_segment(s, s->vseg, vseg);
   return rc;
+}
+
+extern "C" int qhp_profile_read_pair(qhp_system *s, double *ms_host, int64_t *n_host) {
+  if (!s) return QHP_EINVAL;
+  int rc = prof_drain(s);
+  if (rc) return rc;
+  for (int k = 0; k < 3; ++k) { if (ms_host) ms_host[k] = s->prof_ms[5 + k]; if (n_host) n_host[k] = s->prof_n[5 + k]; }
+  return QHP_OK;
 }
 
 extern "C" int qhp_counters(qhp_system *s, int64_t *out_host, int n_out) {

@@ -152,8 +152,8 @@ struct qhp_system {
   bool prof = false;
   std::vector<cudaEvent_t> prof_ev;      // flat list of (begin, end) pairs
   std::vector<int> prof_kind;            // phase of each pair
-  double prof_ms[5] = {0, 0, 0, 0, 0};
-  int64_t prof_n[5] = {0, 0, 0, 0, 0};
+  double prof_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // 0-4: phases of qhp_profile_read; 5-7: k_prune_check, k_prune, k_pair_dense
+  int64_t prof_n[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 
   // ---- run state (host) ----
   bool have_state = false;
@@ -216,5 +216,20 @@ int qhp_fft_launch(double *data, int n, int64_t batch, int sign, const double *t
 __host__ __device__ __forceinline__ long long qhp_seg_addr(int slot, int n_seg, int n) {
   return ((long long)(slot >> 2) * n_seg + n) * 12 + (slot & 3) * 3;
 }
+
+// CUDA events around a phase (or one launch) on the library stream while qhp_profile is on
+struct qhp_prof_scope {
+  qhp_system *s; bool on;
+  qhp_prof_scope(qhp_system *s_, int kind) : s(s_), on(s_->prof) {
+    if (!on) return;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    s->prof_ev.push_back(a); s->prof_ev.push_back(b); s->prof_kind.push_back(kind);
+    cudaEventRecord(a, s->stream);
+    idx = s->prof_ev.size() - 1;
+  }
+  ~qhp_prof_scope() { if (on) cudaEventRecord(s->prof_ev[idx], s->stream); }
+  size_t idx = 0;
+};
 
 void qhp_global_error(const char *msg);   // qhp_api.cu: error text of a call without a system handle (qhp_last_error(NULL))
