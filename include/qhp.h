@@ -95,7 +95,9 @@ int qhp_destroy(qhp_system *sys);
 /* Load bead positions / momenta (device [P][n_atoms][3]); transforms to normal modes (Eq. 4
  * inverted), builds cells + neighbour list on the centroids and evaluates the
  * forces.  step0 = index of the next step: Philox streams are functions of (seed, atom, mode,
- * step), so get_state -> set_state resumes bit-identically.  adQTB: step0 % n_seg == 0. */
+ * step), so get_state -> set_state resumes bit-identically up to the summation order of the freshly built
+ * neighbour list.  adQTB: step0 % n_seg == 0; the adapted gamma_z travels through qhp_adqtb_gamma /
+ * qhp_adqtb_set_gamma. */
 int qhp_set_state(qhp_system *sys, const double *x_beads, const double *p_beads, int64_t step0);
 int qhp_get_state(qhp_system *sys, double *x_beads, double *p_beads, int64_t *step_host);
 int qhp_set_state_host(qhp_system *sys, const double *x_beads, const double *p_beads, int64_t step0);
@@ -201,6 +203,14 @@ int qhp_contracted(qhp_system *sys, double *xc);
 /* adQTB: gamma_z(omega_j) [n_types][n_seg+1]; coloured force segment Fc and recorded
  * velocities vseg, both [3 n_atoms][n_seg] (NULL to skip). */
 int qhp_adqtb_gamma(qhp_system *sys, double *gamma);
+/* adQTB restart: load gamma_z(omega_j) [n_types][n_seg+1] (DEVICE pointer, values > 0) as written by qhp_adqtb_gamma
+ * of an earlier run, so that create -> qhp_adqtb_set_gamma -> qhp_set_state(x, p, step0) at a segment boundary
+ * continues an adapted run (the adaptation takes ps to 100s of ps) instead of restarting from gamma_0.
+ * Allowed before qhp_set_state, or at a segment boundary before the first step of the segment (QHP_ESTATE
+ * otherwise: the segment's coloured force has been generated with the old gamma).  Not restored: the RATIO
+ * window averages (Eq. 26; the first segment after a restart re-initialises them) -- kappa is an input the caller
+ * sets again. */
+int qhp_adqtb_set_gamma(qhp_system *sys, const double *gamma);
 /* adQTB: RATIO adaptation (Eq. 24-26) for the atom types with tau_ps[z] > 0:
  * gamma_z = Re<C_vF,z> / (m_z <C_vv,z>) from exponential-window averages of the segment spectra with
  * time constant tau_ps[z] (the first segment after this call initialises them); the other types keep

@@ -18,7 +18,7 @@ SYMBOLS = ["qhp_create", "qhp_destroy", "qhp_set_respa", "qhp_set_a_block", "qhp
            "qhp_get_state_host", "qhp_step", "qhp_forces", "qhp_observables", "qhp_observables_host",
            "qhp_neighbor_lists", "qhp_pair_list", "qhp_contracted", "qhp_adqtb_gamma", "qhp_adqtb_ratio", "qhp_adqtb_kappa",
            "qhp_adqtb_segment", "qhp_counters", "qhp_profile", "qhp_profile_read", "qhp_check", "qhp_last_error", "qhp_philox_normals",
-           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar", "qhp_pibar_noalloc", "qhp_set_comm", "qhp_pair_slices", "qhp_set_pair_prune", "qhp_pair_prune_stats", "qhp_profile_read_pair"]
+           "qhp_fft_c2c", "qhp_dfma_probe", "qhp_pibar", "qhp_pibar_noalloc", "qhp_set_comm", "qhp_pair_slices", "qhp_set_pair_prune", "qhp_pair_prune_stats", "qhp_profile_read_pair", "qhp_adqtb_set_gamma"]
 
 
 # int fn(void *ctx, void *device_buf, size_t bytes_per_rank, int rank, int world, void *cuda_stream)  (include/qhp.h)
@@ -116,6 +116,7 @@ def lib():
         L.qhp_pibar.argtypes = [vp, i64, vp, i64, C.c_double, i32, C.c_double, vp, C.POINTER(C.c_double), C.POINTER(i32)]
         L.qhp_set_pair_prune.argtypes = [vp, C.c_double]
         L.qhp_pair_prune_stats.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.qhp_adqtb_set_gamma.argtypes = [vp, vp]
         L.qhp_profile_read_pair.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.qhp_pibar_noalloc.argtypes = [vp, i64, vp, i64, C.c_double, i32, C.c_double, vp, vp]
         for name in SYMBOLS:
@@ -347,6 +348,12 @@ class System:
         g = self._empty((self.n_types, self.n_seg + 1))
         self._ok(self._L.qhp_adqtb_gamma(self._h, _ptr(g)))
         return g
+
+    def adqtb_set_gamma(self, gamma):
+        """Restart of an adapted adQTB run: gamma [n_types][n_seg+1] (CUDA fp64) as returned by adqtb_gamma."""
+        torch = _torch()
+        _chk_dev(gamma, torch.float64, self.n_types * (self.n_seg + 1), "gamma")
+        self._ok(self._L.qhp_adqtb_set_gamma(self._h, _ptr(gamma)))
 
     def adqtb_segment(self, want_fc=True, want_v=True):
         Fc = self._empty((3 * self.N, self.n_seg)) if want_fc else None

@@ -591,6 +591,17 @@ extern "C" int qhp_adqtb_gamma(qhp_system *s, double *gamma) {
   return QHP_OK;
 }
 
+extern "C" int qhp_adqtb_set_gamma(qhp_system *s, const double *gamma) {
+  if (!s || !gamma) return QHP_EINVAL;
+  if (s->th.kind != QHP_THERMO_ADQTB) { s->err = "not an adQTB system"; return QHP_ESTATE; }
+  if (s->have_state && (s->step % s->n_seg != 0 || s->fc_segment == s->step / s->n_seg)) {
+    s->err = "qhp_adqtb_set_gamma: only at a segment boundary, before the segment's first step";
+    return QHP_ESTATE;
+  }
+  QHP_CUDA_OK(s, cudaMemcpyAsync(s->gamma, gamma, sizeof(double) * s->nt * (s->n_seg + 1), cudaMemcpyDeviceToDevice, s->stream));
+  return QHP_OK;
+}
+
 extern "C" int qhp_adqtb_ratio(qhp_system *s, const double *tau_ps) {
   if (!s) return QHP_EINVAL;
   if (s->th.kind != QHP_THERMO_ADQTB) { s->err = "not an adQTB system"; return QHP_ESTATE; }

@@ -217,3 +217,37 @@ def test_n_seg_2048_segment_parity():
     g = sysg.adqtb_gamma().cpu().numpy()
     assert np.abs(g - g_ref).max() < 1e-9 * np.abs(g_ref).max()
     sysg.check()
+
+
+def test_restart_with_adapted_gamma_continues_the_run():
+    """create -> adqtb_set_gamma -> set_state at a segment boundary in a NEW handle continues an adapted run: the third
+    segment equals that of the uninterrupted run (and of the oracle, which ran uninterrupted) -- gamma_z is the only
+    adQTB state that has to travel with (x, p, step) for the SIMPLE scheme (Eq. 23); Philox is stateless."""
+    import paper_2212_03137_b200 as qhp
+    top = W.water_box(216)
+    n_seg = 64
+    a, ref, x0, p0 = make_pair(top, 1, 1, 0.5, "adqtb", gamma0=20.0, n_seg=n_seg, a_gamma=0.5)
+    a.set_state(to_dev(x0), to_dev(p0), 0)
+    ref.set_state(x0, p0, 0)
+    a.step(2 * n_seg)
+    ref.step(3 * n_seg)
+    x2, p2, st = a.get_state()
+    g2 = a.adqtb_gamma().clone()
+    assert st == 2 * n_seg and (g2 - 20.0).abs().max().item() > 1e-3      # the run has adapted
+    with pytest.raises(qhp.QhpError):
+        a.step(1) or a.adqtb_set_gamma(g2)                                # inside a segment: refused
+    b, _, _, _ = make_pair(top, 1, 1, 0.5, "adqtb", gamma0=20.0, n_seg=n_seg, a_gamma=0.5)
+    b.adqtb_set_gamma(g2)
+    b.set_state(x2, p2, 2 * n_seg)
+    b.step(n_seg)
+    xb, pb, stb = b.get_state()
+    xr, pr = ref.get_state()
+    assert stb == 3 * n_seg
+    assert np.abs(xb.cpu().numpy() - xr).max() < 1e-8
+    assert np.abs(b.adqtb_gamma().cpu().numpy() - ref.gamma).max() < 1e-9 * ref.gamma.max()
+    # without the setter the restarted handle would colour its noise with gamma_0
+    c, _, _, _ = make_pair(top, 1, 1, 0.5, "adqtb", gamma0=20.0, n_seg=n_seg, a_gamma=0.5)
+    c.set_state(x2, p2, 2 * n_seg)
+    c.step(n_seg)
+    assert np.abs(c.get_state()[0].cpu().numpy() - xr).max() > 1e-6
+    b.check()
