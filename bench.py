@@ -249,6 +249,8 @@ def time_workload(sysg, cfg, top, x0, p0, K, args, world, local, dist_barrier):
     prof_pair = sysg.profile_read_pair()
     sysg.profile(False)
     c1 = sysg.counters()
+    if c1["overflow"]:
+        raise RuntimeError(f"error flags {c1['overflow']} after the timed steps (list overflow / skin / staged region): the timing is void")
     prune = sysg.pair_prune_stats()
     ms = max_over_ranks(ms, world)
     out = dict(ms=ms, prof=prof, prof_pair=prof_pair, prune=prune, c0=c0, c1=c1, clocks=clk.summary(), launches=int(c1["launches"] - c0["launches"]),

@@ -521,10 +521,11 @@ __global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const Stag
 #define PRUNE_THREADS 512
 #endif
 #define PRUNE_WARPS (PRUNE_THREADS / 32)
-#define PRUNE_QUEUE (2 * STG_BLOCK)      // < 256 left over + 256 new entries per warp
+#define PRUNE_QUEUE (2 * STG_BLOCK)      // circular: < 256 entries waiting + 256 new ones per warp (a power of two)
 
 struct PruneArgs {
   int N, Pc, nt, cap, bead0;     // cap = dcap of the dense kernel (dummy at cap - 1)
+  int ccap, src_dummy;           // records staged here (>= both staged arrays); dummy index of the centroid rows
   int nc[3];
   double box[3], inv_box[3], cell_edge[3];
   const double *pos4;            // [Pc][N][4] current contracted beads, slot order
@@ -582,8 +583,8 @@ __device__ __forceinline__ bool prune_due(const PruneArgs &a, int bead) {
 __global__ void __launch_bounds__(PRUNE_THREADS, 2) k_prune(const PruneArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   uint2 *C = reinterpret_cast<uint2 *>(smem_raw);
-  uint32_t *queue = reinterpret_cast<uint32_t *>(C + a.cap);
-  __shared__ int off[28], cbeg[27], next_atom;
+  uint32_t *queue = reinterpret_cast<uint32_t *>(C + a.ccap);
+  __shared__ int off[28], cbeg[27];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = blockDim.x;
   const int bead = a.bead0 + blockIdx.y;
   if (!prune_due(a, bead)) return;
@@ -607,7 +608,6 @@ __global__ void __launch_bounds__(PRUNE_THREADS, 2) k_prune(const PruneArgs a) {
   }
   __syncthreads();
   if (tid == 0) {
-    next_atom = 0;
     off[0] = 0;
     for (int s = 0; s < 27; ++s) off[s + 1] += off[s];
   }
@@ -645,7 +645,7 @@ __global__ void __launch_bounds__(PRUNE_THREADS, 2) k_prune(const PruneArgs a) {
       }
     }
   }
-  if (tid == 0) C[a.cap - 1] = half_record(1e9, 1e9, 1e9);  // the dummy: no test against it passes
+  if (tid == 0) C[a.src_dummy] = half_record(1e9, 1e9, 1e9);   // the padding of the centroid rows: no test against it passes
   __syncthreads();
   const int h0 = off[13], nh = off[14] - off[13], slot0 = cbeg[13];
   const uint32_t sC = (uint32_t)__cvta_generic_to_shared(C),
@@ -653,74 +653,69 @@ __global__ void __launch_bounds__(PRUNE_THREADS, 2) k_prune(const PruneArgs a) {
   unsigned lt;
   asm volatile("mov.u32 %0, %%lanemask_lt;" : "=r"(lt));
   const uint32_t dummy = (uint32_t)(a.cap - 1);
-  for (;;) {
-    int t = 0;
-    if (lane == 0) t = atomicAdd(&next_atom, 1);
-    const int ii = __shfl_sync(0xffffffffu, t, 0);
-    if (ii >= nh) break;
+  // Rows are dealt to the warps round-robin; the next block of entries (of this row or of the warp's next row) and the
+  // next row's count are requested one block ahead.  Survivors go into a circular queue of 512 slots per warp
+  // (tail = entries of the row so far, head = entries written out, a multiple of 256).
+  const int nw = nthr >> 5, wrp = __shfl_sync(0xffffffffu, warp, 0);
+  int ii = wrp, n_nx = 0;
+  uint4 cur = make_uint4(0u, 0u, 0u, 0u);
+  if (ii < nh) {
+    n_nx = a.nbr_count[slot0 + ii];
+    cur = *reinterpret_cast<const uint4 *>(a.nbr16 + (long long)(slot0 + ii) * a.stride + 8 * lane);
+  }
+  for (; ii < nh; ii += nw) {
     const long long slot = slot0 + ii;
-    const int n = a.nbr_count[slot];
+    const int n = n_nx;
     const uint16_t *rowp = a.nbr16 + slot * a.stride;
     uint16_t *outp = a.nbr16p + ((long long)bead * a.N + slot) * a.stride;
-    const int nblk = (n + STG_BLOCK - 1) / STG_BLOCK;
-    uint4 cur = make_uint4(0u, 0u, 0u, 0u);
-    if (nblk > 0) cur = *reinterpret_cast<const uint4 *>(rowp + 8 * lane);
+    const int nblk = max(1, (n + STG_BLOCK - 1) / STG_BLOCK);
+    const bool more = ii + nw < nh;
+    if (more) n_nx = a.nbr_count[slot + nw];
     const uint2 ci = lds_u2(sC + (uint32_t)(h0 + ii) * 8);
-    uint32_t qa = sQ;
-    int written = 0;
-    // one 256-entry block of the pruned row from the first 256 queue slots (lane l: entries 32 j + l, j = 0..7)
+    uint32_t tail = 0, head = 0;
+    // one 256-entry block of the pruned row from queue slots head .. head + 255 (lane l: entries 32 j + l, j = 0..7)
     auto flush = [&]() {
       uint32_t e[8];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) e[j] = lds_u(sQ + (32 * j + lane) * 4);
-      *reinterpret_cast<uint4 *>(outp + written + 8 * lane) =
+      for (int j = 0; j < 8; ++j) e[j] = lds_u(sQ + ((head + 32 * j + lane) & (PRUNE_QUEUE - 1)) * 4);
+      *reinterpret_cast<uint4 *>(outp + head + 8 * lane) =
           make_uint4(e[0] | (e[1] << 16), e[2] | (e[3] << 16), e[4] | (e[5] << 16), e[6] | (e[7] << 16));
     };
     for (int m = 0; m < nblk; ++m) {
       uint4 nxt = cur;
       if (m + 1 < nblk) nxt = *reinterpret_cast<const uint4 *>(rowp + STG_BLOCK * (m + 1) + 8 * lane);
+      else if (more) nxt = *reinterpret_cast<const uint4 *>(rowp + (long long)nw * a.stride + 8 * lane);   // first block of the next row
       const uint32_t w[4] = {cur.x, cur.y, cur.z, cur.w};
       auto entry = [&](int j) { return (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu); };
       const int nst = min(8, (n - STG_BLOCK * m + 31) >> 5);
-      // the centroid table pads its rows with the dummy of the LARGER staged array of k_pair_staged: clamp to ours
-      auto rec = [&](int j) { return sC + min(entry(j) & STG_IDX_MASK, dummy) * 8; };
-      uint2 cj = lds_u2(rec(0));
+      uint2 cj = lds_u2(sC + (entry(0) & STG_IDX_MASK) * 8);
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         if (j >= nst) break;
         const uint32_t e = entry(j);
         const bool hit = half_test(ci, cj, a.thr_h);
-        if (j < 7) cj = lds_u2(rec(j + 1));
+        if (j < 7) cj = lds_u2(sC + (entry(j + 1) & STG_IDX_MASK) * 8);
         unsigned mask;
         asm volatile("{ .reg .pred p; setp.ne.u32 p, %1, 0; vote.sync.ballot.b32 %0, p, 0xffffffff; }" : "=r"(mask) : "r"((unsigned)hit));
-        if (hit) sts_u(qa + __popc(mask & lt) * 4, e);
-        qa += __popc(mask) * 4;
+        if (hit) sts_u(sQ + ((tail + __popc(mask & lt)) & (PRUNE_QUEUE - 1)) * 4, e);
+        tail += __popc(mask);
       }
       __syncwarp();
-      if (qa >= sQ + STG_BLOCK * 4) {
+      if (tail - head >= STG_BLOCK) {
         flush();
-        written += STG_BLOCK;
-        qa -= STG_BLOCK * 4;
-        uint32_t v[8];                                     // < 256 entries left over: to the front of the queue
-#pragma unroll
-        for (int k = 0; k < 8; ++k) v[k] = lds_u(sQ + (STG_BLOCK + 32 * k + lane) * 4);
-        __syncwarp();
-#pragma unroll
-        for (int k = 0; k < 8; ++k)
-          if (sQ + (32 * k + lane) * 4 < qa) sts_u(sQ + (32 * k + lane) * 4, v[k]);
+        head += STG_BLOCK;
         __syncwarp();
       }
       cur = nxt;
     }
-    const int cnt = (int)(qa - sQ) >> 2;                   // < 256
-    if (cnt > 0) {
-      const int pad = (cnt + 31) & ~31;
-      if (cnt + lane < pad) sts_u(qa + lane * 4, dummy);   // the last 32-entry step is completed with the dummy
+    if (tail > head) {                                     // < 256 entries left
+      const uint32_t pad = (tail + 31u) & ~31u;
+      if (tail + lane < pad) sts_u(sQ + ((tail + lane) & (PRUNE_QUEUE - 1)) * 4, dummy);   // complete the last 32-entry step
       __syncwarp();
       flush();                                             // entries behind `pad` are never read (row count)
       __syncwarp();
     }
-    if (lane == 0) a.nbr_count_p[(long long)bead * a.N + slot] = written + cnt;
+    if (lane == 0) a.nbr_count_p[(long long)bead * a.N + slot] = (int)tail;
   }
   }
 }
@@ -909,7 +904,7 @@ int qhp_pair_dense_prepare(qhp_system *s, long long region) {
     QHP_CUDA_OK(s, cudaMemsetAsync(s->prune_part, 0, sizeof(double) * (size_t)s->Pc * PRUNE_CHECK_CTAS, s->stream));
     QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_dense<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
     QHP_CUDA_OK(s, cudaFuncSetAttribute(k_pair_dense<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-    QHP_CUDA_OK(s, cudaFuncSetAttribute(k_prune, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    QHP_CUDA_OK(s, cudaFuncSetAttribute(k_prune, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));   // <= 8192 records + queues
   }
   QHP_CUDA_OK(s, cudaMemsetAsync(s->pruned_at, 0xff, sizeof(long long) * (size_t)s->Pc, s->stream));   // -1: stale
   QHP_CUDA_OK(s, cudaMemsetAsync(s->pruned_at + s->Pc, 0, sizeof(long long) * (size_t)s->Pc, s->stream));
@@ -934,7 +929,9 @@ static int pair_dense_forces(qhp_system *s, StagedArgs &a, int bead0, int nbeads
     k_prune_check<<<dim3(PRUNE_CHECK_CTAS, (unsigned)nbeads), 256, 0, s->stream>>>(p);
   }
   QHP_LAUNCH_OK(s);
-  const size_t psm = (size_t)s->dense_cap * sizeof(uint2) + sizeof(uint32_t) * PRUNE_WARPS * PRUNE_QUEUE;
+  p.src_dummy = s->staged_cap - 1;                      // the centroid rows are padded with the dummy of k_pair_staged
+  p.ccap = s->staged_cap > s->dense_cap ? s->staged_cap : s->dense_cap;
+  const size_t psm = (size_t)p.ccap * sizeof(uint2) + sizeof(uint32_t) * PRUNE_WARPS * PRUNE_QUEUE;
   {
     qhp_prof_scope ps(s, 6);
     k_prune<<<dim3((unsigned)(s->ncell < PRUNE_CHECK_CTAS ? s->ncell : PRUNE_CHECK_CTAS), (unsigned)nbeads), PRUNE_THREADS, psm, s->stream>>>(p);
