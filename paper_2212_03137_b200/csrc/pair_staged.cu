@@ -24,6 +24,14 @@
 // alpha^3 S a degree-15 polynomial in u = 2 r^2/r_c^2 - 1 whose coefficients (fitted at create time
 // from the Taylor series of S, qhp_pair_setup) sit in the kernel's constant bank.
 // Full list (each ordered pair evaluated from its own side): no atomics, fixed summation order.
+//
+// Kernels of this file:
+//   k_pair_staged<ENERGY, F32>   the design above (pre-test + compaction + evaluation on the centroid table every step):
+//                                energy variant of every staged system, force path when the pruned rows are off / do not fit;
+//   k_prune_check, k_prune       per contracted bead, a second table with the entries within r_c + prune_skin of the bead's
+//                                own positions, renewed on the device when the bead has moved prune_skin / 2 or the centroid
+//                                table was rebuilt (see the comment above k_prune_check);
+//   k_pair_dense<COUNT>          evaluation of those pruned rows without pre-test: the force path of C3 / C4.
 #include <math.h>
 #include <cuda_fp16.h>
 
