@@ -289,6 +289,8 @@ extern "C" int qhp_destroy(qhp_system *s) {
                   s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p, s->ratio_tau, s->ratio_avv, s->ratio_avf, s->kappa};
   for (void *p : ptrs) if (p) cudaFree(p);
   qhp_pair_dense_free(s);
+  if (s->flags_host) cudaFreeHost(s->flags_host);
+  if (s->flags_ev) cudaEventDestroy(s->flags_ev);
   delete s;
   return QHP_OK;
 }
@@ -403,12 +405,51 @@ extern "C" int qhp_profile_read(qhp_system *s, double *ms_host, int64_t *n_host)
   return QHP_OK;
 }
 
+static const char *flag_text(const int64_t *c) {
+  if (c[1]) return "neighbour table overflow: a row exceeded its capacity";
+  if (c[7]) return "staged pair kernel: a 27-cell neighbourhood outgrew shared memory between list builds";
+  if (c[6]) return "skin too small: a contracted bead is farther than skin/2 from its centroid, the centroid list cannot cover it";
+  return nullptr;
+}
+
+// The device error flags (sticky) reach the host without a synchronisation: qhp_step enqueues a copy of them into
+// pinned memory behind its work and looks at the last finished copy when it is entered again (and every 256 steps
+// of a long call), so a run does not go on for thousands of steps on truncated rows or missing forces.
+static int flags_poll(qhp_system *s) {
+  if (!s->flags_pending || cudaEventQuery(s->flags_ev) != cudaSuccess) { cudaGetLastError(); return QHP_OK; }
+  s->flags_pending = false;
+  if (const char *t = flag_text(s->flags_host)) { s->err = std::string(t) + " (seen by qhp_step; forces since then are not valid)"; return QHP_ESTATE; }
+  return QHP_OK;
+}
+static void flags_enqueue(qhp_system *s) {
+  if (s->flags_pending) return;
+  if (!s->flags_host) {
+    if (cudaMallocHost(&s->flags_host, sizeof(int64_t) * 8) != cudaSuccess || cudaEventCreateWithFlags(&s->flags_ev, cudaEventDisableTiming) != cudaSuccess) {
+      cudaGetLastError();
+      if (s->flags_host) { cudaFreeHost(s->flags_host); s->flags_host = nullptr; }
+      return;                                            // no polling: qhp_check still reports
+    }
+  }
+  if (cudaMemcpyAsync(s->flags_host, s->counters, sizeof(int64_t) * 8, cudaMemcpyDeviceToHost, s->stream) != cudaSuccess ||
+      cudaEventRecord(s->flags_ev, s->stream) != cudaSuccess) { cudaGetLastError(); return; }
+  s->flags_pending = true;
+}
+
 extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
   if (!s || nsteps < 0) return QHP_EINVAL;
   if (!s->have_state) { s->err = "qhp_step before qhp_set_state"; return QHP_ESTATE; }
   if (nsteps % s->n_alt != 0) { s->err = "nsteps must be a multiple of n_alt (qhp_set_respa)"; return QHP_EINVAL; }
   const bool adqtb = s->th.kind == QHP_THERMO_ADQTB;
+  {
+    const int rcf = flags_poll(s);
+    if (rcf) return rcf;
+  }
   for (int64_t k = 0; k < nsteps; ++k) {
+    if ((k & 255) == 255) {
+      const int rcf = flags_poll(s);
+      if (rcf) return rcf;
+      flags_enqueue(s);
+    }
     const int64_t st = s->step;
     int rc;
     if (adqtb && st % s->n_seg == 0 && s->fc_segment != st / s->n_seg) {
@@ -441,6 +482,7 @@ extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
       if (rc) return rc;
     }
   }
+  if (nsteps > 0) flags_enqueue(s);
   return QHP_OK;
 }
 
@@ -681,9 +723,7 @@ extern "C" int qhp_check(qhp_system *s) {
   if (s->counters) {
     int64_t c[8];
     QHP_CUDA_OK(s, cudaMemcpy(c, s->counters, sizeof(c), cudaMemcpyDeviceToHost));
-    if (c[1]) { s->err = "neighbour table overflow: a row exceeded its capacity"; return QHP_ESTATE; }
-    if (c[7]) { s->err = "staged pair kernel: a 27-cell neighbourhood outgrew shared memory between list builds"; return QHP_ESTATE; }
-    if (c[6]) { s->err = "skin too small: a contracted bead is farther than skin/2 from its centroid, the centroid list cannot cover it"; return QHP_ESTATE; }
+    if (const char *t = flag_text(c)) { s->err = t; return QHP_ESTATE; }
   }
   return QHP_OK;
 }

@@ -148,6 +148,11 @@ struct qhp_system {
   qhp_allgather_fn shard_allgather = nullptr;
   void *shard_ctx = nullptr;
 
+  // ---- error flags seen without a synchronisation (qhp_step): async copy of `counters` into pinned memory + event ----
+  int64_t *flags_host = nullptr;
+  cudaEvent_t flags_ev = nullptr;
+  bool flags_pending = false;
+
   // ---- per-phase profiling (qhp_profile) ----
   bool prof = false;
   std::vector<cudaEvent_t> prof_ev;      // flat list of (begin, end) pairs

@@ -199,6 +199,28 @@ def test_harmonic_oscillators_single_atom_molecules():
     assert np.abs(obs - ref.observables()).max() < 1e-9 * np.abs(ref.observables()).max()
 
 
+def test_step_sees_the_error_flags_without_a_check():
+    """qhp_step polls the device error flags asynchronously (include/qhp.h): a run with a list that cannot cover its
+    beads stops at a later qhp_step call instead of going on until someone calls qhp_check."""
+    import torch
+    import paper_2212_03137_b200 as qhp
+    top = W.water_box(216)
+    top["skin"] = 0.05
+    sysg, _, x0, p0 = make_pair(top, 4, 2, 0.5, "pile", sigma_bead=0.05)
+    sysg.set_state(to_dev(x0), to_dev(p0), 0)
+    sysg.step(2)                                   # the flag copy is enqueued behind these steps
+    torch.cuda.synchronize()
+    with pytest.raises(qhp.QhpError, match="skin too small"):
+        sysg.step(2)
+    good = W.water_box(216)
+    sysg2, _, x0, p0 = make_pair(good, 4, 2, 0.5, "pile")
+    sysg2.set_state(to_dev(x0), to_dev(p0), 0)
+    for _ in range(3):
+        sysg2.step(300)                            # crosses the 256-step poll inside a call
+        torch.cuda.synchronize()
+    sysg2.check()
+
+
 def test_staged_pretest_rejects_no_pair_inside_the_cutoff():
     """The staged kernel drops list entries by a packed-half distance pre-test before the fp64 test.  A pair it
     wrongly dropped near r_c would be invisible in the forces (the shifted force vanishes at r_c), so the
