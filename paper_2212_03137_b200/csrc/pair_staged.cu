@@ -459,10 +459,21 @@ __global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const Stag
     const bool lj_row = lj_mask != 0u;
     double Fx = 0.0, Fy = 0.0, Fz = 0.0;
 
-    auto eval = [&](uint32_t entry) {
-      const uint32_t sj = entry & STG_IDX_MASK, tj = entry >> STG_IDX_BITS;
-      const double2 xyj = lds_d2(sXY + sj * 16);
-      const double zj = lds_d(sZ + sj * 8);
+    // The staged records of an entry are requested one evaluation ahead (a warp issues in order: without this every
+    // evaluation starts on the latency of its own gathers).  Entries behind the row's last step are not initialised:
+    // the index is clamped to the dummy.
+    const uint32_t dummyi = (uint32_t)(a.dcap - 1);
+    double2 xyn = make_double2(0.0, 0.0);
+    double zn = 0.0;
+    auto fetch = [&](uint32_t entry) {
+      const uint32_t sj = min(entry & STG_IDX_MASK, dummyi);
+      xyn = lds_d2(sXY + sj * 16); zn = lds_d(sZ + sj * 8);
+    };
+    auto eval = [&](uint32_t entry, uint32_t next) {
+      const uint32_t tj = entry >> STG_IDX_BITS;
+      const double2 xyj = xyn;
+      const double zj = zn;
+      fetch(next);
       const double qq = qi * lds_d(sQt + tj * 8);
       const double dx = xyi.x - xyj.x, dy = xyi.y - xyj.y, dz = zi - zj;
       const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
@@ -487,10 +498,12 @@ __global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const Stag
       else if (more) nxt = *reinterpret_cast<const uint4 *>(rowp + (long long)istep * a.stride + 8 * lane);   // first block of the next row
       const uint32_t w[4] = {cur.x, cur.y, cur.z, cur.w};
       const int nst = min(8, (n - STG_BLOCK * m + 31) >> 5);
+      fetch(w[0] & 0xffffu);
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         if (j >= nst) break;
-        eval((j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu));
+        const int jn = j < 7 ? j + 1 : 7;                  // (the last step of a block re-requests its own record: harmless)
+        eval((j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu), (jn & 1) ? (w[jn >> 1] >> 16) : (w[jn >> 1] & 0xffffu));
       }
       cur = nxt;
     }
