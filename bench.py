@@ -372,7 +372,7 @@ def main():
     ap.add_argument("--a-block", choices=["exact", "cayley"], default="exact", help="cayley = BCOCB (PAPER.md:151); exact = the BASELINE.json configs")
     ap.add_argument("--n-alt", type=int, default=1, help="BAOAB-RESPA inner steps per V_s evaluation (PAPER.md Eq. 19); 1 = the BASELINE.json configs")
     ap.add_argument("--n-mol", type=int, default=0, help="profiling aid: the same workload on a box of this many waters (0 = the BASELINE.json size)")
-    ap.add_argument("--prune-skin", type=float, default=None, help="qhp_set_pair_prune: A; <= 0 = the unpruned pre-test pair kernel; default = the library's (0.5)")
+    ap.add_argument("--prune-skin", type=float, default=None, help="qhp_set_pair_prune: A; <= 0 = the unpruned pre-test pair kernel; default = the library's (0.6)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--shard-beads", action="store_true", help="N > 1: bead-sharded V_s over the ranks (qhp_set_comm, NCCL all-gather of F_s; N must divide P'); "

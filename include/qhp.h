@@ -135,7 +135,7 @@ int qhp_set_contraction(qhp_system *sys, int variant);
 
 /* Pruned per-bead rows of the staged pair kernel (an acceleration structure of R8; the centroid
  * table of R7 -- the list the paper describes and the oracle is compared with -- is unchanged).  With
- * prune_skin > 0 (default 0.5 A; must be < the list skin) every contracted bead keeps a second table holding the
+ * prune_skin > 0 (default 0.6 A; must be < the list skin) every contracted bead keeps a second table holding the
  * entries of the centroid table within r_cut + prune_skin of the bead's own positions; V_s is then evaluated on
  * those rows without a per-step pre-test.  A bead's rows are renewed on the device, without a host round trip,
  * when one of its atoms has moved more than prune_skin / 2 since they were made or the centroid table was

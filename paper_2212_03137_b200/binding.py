@@ -287,7 +287,7 @@ class System:
         self._ok(self._L.qhp_set_contraction(self._h, {"literal": 0, "trig": 1}[variant]))
 
     def set_pair_prune(self, prune_skin: float):
-        """Pruned per-bead rows of the staged pair kernel (include/qhp.h): prune_skin in A (default 0.5), <= 0 off.
+        """Pruned per-bead rows of the staged pair kernel (include/qhp.h): prune_skin in A (default 0.6), <= 0 off.
         Before set_state."""
         self._ok(self._L.qhp_set_pair_prune(self._h, float(prune_skin)))
 

@@ -99,7 +99,7 @@ struct qhp_system {
   double staged_thr = 0.0;                 // threshold of that pre-test (r_c^2 + its error bound, a half)
   int staged_split = 1;                    // CTAs per (cell, bead)
   // pruned per-bead rows + evaluation without pre-test (k_prune, k_pair_dense in pair_staged.cu)
-  double prune_skin = 0.5;                 // A; <= 0: off (qhp_set_pair_prune)
+  double prune_skin = 0.6;                 // A; <= 0: off (qhp_set_pair_prune); 0.6: best of the 0.3-1.0 sweep at C3 and C4
   bool dense = false;                      // in use (decided with `staged` at the synchronising list build)
   int dense_cap = 0;                       // staged atoms of k_pair_dense (two CTAs per SM)
   uint16_t *nbr16p = nullptr;              // [Pc][N][nbr_stride] pruned rows
