@@ -165,28 +165,27 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
   {
     const double ctr[3] = {(cx + 0.5) * a.cell_edge[0], (cy + 0.5) * a.cell_edge[1], (cz + 0.5) * a.cell_edge[2]};
     const double MAGIC = 6755399441055744.0;             // 1.5 * 2^52: (t + MAGIC) - MAGIC = rint(t) for |t| < 2^51
-    constexpr int UN = 4;                                // independent loads in flight per thread
-    for (int g0 = tid; g0 < total; g0 += UN * nthr) {
-      double4 p[UN];
-      int s = 0;
+    // one warp per stencil cell at a time: coalesced 32-byte records, no search for the cell of a staged index
+    constexpr int UN = 3;                                // independent loads in flight per lane
+    for (int s = warp; s < 27; s += nthr >> 5) {
+      const int o = off[s], n = off[s + 1] - o;
+      const double4 *src = pos + cbeg[s];
+      for (int k0 = lane; k0 < n; k0 += UN * 32) {
+        double4 p[UN];
 #pragma unroll
-      for (int u = 0; u < UN; ++u) {
-        const int g = g0 + u * nthr;
-        if (g < total) {
-          while (g >= off[s + 1]) ++s;
-          p[u] = pos[cbeg[s] + g - off[s]];
-        }
-      }
+        for (int u = 0; u < UN; ++u)
+          if (k0 + 32 * u < n) p[u] = src[k0 + 32 * u];
 #pragma unroll
-      for (int u = 0; u < UN; ++u) {
-        const int g = g0 + u * nthr;
-        if (g < total) {
-          double lx = p[u].x - ctr[0], ly = p[u].y - ctr[1], lz = p[u].z - ctr[2];
-          lx = fma(-a.box[0], (lx * a.inv_box[0] + MAGIC) - MAGIC, lx);
-          ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
-          lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
-          XY[g] = make_double2(lx, ly); Z[g] = lz;
-          if (F32) C[g] = half_record(lx, ly, lz);
+        for (int u = 0; u < UN; ++u) {
+          const int k = k0 + 32 * u;
+          if (k < n) {
+            double lx = p[u].x - ctr[0], ly = p[u].y - ctr[1], lz = p[u].z - ctr[2];
+            lx = fma(-a.box[0], (lx * a.inv_box[0] + MAGIC) - MAGIC, lx);
+            ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
+            lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
+            XY[o + k] = make_double2(lx, ly); Z[o + k] = lz;
+            if (F32) C[o + k] = half_record(lx, ly, lz);
+          }
         }
       }
     }
@@ -408,27 +407,26 @@ __global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const Stag
   {
     const double ctr[3] = {(cx + 0.5) * a.cell_edge[0], (cy + 0.5) * a.cell_edge[1], (cz + 0.5) * a.cell_edge[2]};
     const double MAGIC = 6755399441055744.0;
-    constexpr int UN = 4;
-    for (int g0 = tid; g0 < total; g0 += UN * nthr) {
-      double4 p[UN];
-      int s = 0;
+    // one warp per stencil cell at a time: coalesced 32-byte records, no search for the cell of a staged index
+    constexpr int UN = 3;                                // independent loads in flight per lane
+    for (int s = tid >> 5; s < 27; s += nthr >> 5) {
+      const int o = off[s], n = off[s + 1] - o;
+      const double4 *src = pos + cbeg[s];
+      for (int k0 = lane; k0 < n; k0 += UN * 32) {
+        double4 p[UN];
 #pragma unroll
-      for (int u = 0; u < UN; ++u) {
-        const int g = g0 + u * nthr;
-        if (g < total) {
-          while (g >= off[s + 1]) ++s;
-          p[u] = pos[cbeg[s] + g - off[s]];
-        }
-      }
+        for (int u = 0; u < UN; ++u)
+          if (k0 + 32 * u < n) p[u] = src[k0 + 32 * u];
 #pragma unroll
-      for (int u = 0; u < UN; ++u) {
-        const int g = g0 + u * nthr;
-        if (g < total) {
-          double lx = p[u].x - ctr[0], ly = p[u].y - ctr[1], lz = p[u].z - ctr[2];
-          lx = fma(-a.box[0], (lx * a.inv_box[0] + MAGIC) - MAGIC, lx);
-          ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
-          lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
-          XY[g] = make_double2(lx, ly); Z[g] = lz;
+        for (int u = 0; u < UN; ++u) {
+          const int k = k0 + 32 * u;
+          if (k < n) {
+            double lx = p[u].x - ctr[0], ly = p[u].y - ctr[1], lz = p[u].z - ctr[2];
+            lx = fma(-a.box[0], (lx * a.inv_box[0] + MAGIC) - MAGIC, lx);
+            ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
+            lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
+            XY[o + k] = make_double2(lx, ly); Z[o + k] = lz;
+          }
         }
       }
     }
@@ -639,29 +637,29 @@ __global__ void __launch_bounds__(PRUNE_THREADS, 2) k_prune(const PruneArgs a) {
   {
     const double ctr[3] = {(cx + 0.5) * a.cell_edge[0], (cy + 0.5) * a.cell_edge[1], (cz + 0.5) * a.cell_edge[2]};
     const double MAGIC = 6755399441055744.0;
-    constexpr int UN = 4;
-    for (int g0 = tid; g0 < total; g0 += UN * nthr) {
-      double4 p[UN];
-      int s = 0;
+    // one warp per stencil cell at a time (as in k_pair_dense); the home cell's positions become the reference of the
+    // displacement check
+    constexpr int UN = 3;
+    for (int s = tid >> 5; s < 27; s += nthr >> 5) {
+      const int o = off[s], n = off[s + 1] - o;
+      const double4 *src = pos + cbeg[s];
+      double4 *ref = reinterpret_cast<double4 *>(a.pref4) + (long long)bead * a.N + cbeg[s];
+      for (int k0 = lane; k0 < n; k0 += UN * 32) {
+        double4 p[UN];
 #pragma unroll
-      for (int u = 0; u < UN; ++u) {
-        const int g = g0 + u * nthr;
-        if (g < total) {
-          while (g >= off[s + 1]) ++s;
-          p[u] = pos[cbeg[s] + g - off[s]];
-        }
-      }
+        for (int u = 0; u < UN; ++u)
+          if (k0 + 32 * u < n) p[u] = src[k0 + 32 * u];
 #pragma unroll
-      for (int u = 0; u < UN; ++u) {
-        const int g = g0 + u * nthr;
-        if (g < total) {
-          double lx = p[u].x - ctr[0], ly = p[u].y - ctr[1], lz = p[u].z - ctr[2];
-          lx = fma(-a.box[0], (lx * a.inv_box[0] + MAGIC) - MAGIC, lx);
-          ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
-          lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
-          C[g] = half_record(lx, ly, lz);
-          if (g >= off[13] && g < off[14])               // home atoms: the reference of the displacement check
-            reinterpret_cast<double4 *>(a.pref4)[(long long)bead * a.N + cbeg[13] + g - off[13]] = p[u];
+        for (int u = 0; u < UN; ++u) {
+          const int k = k0 + 32 * u;
+          if (k < n) {
+            double lx = p[u].x - ctr[0], ly = p[u].y - ctr[1], lz = p[u].z - ctr[2];
+            lx = fma(-a.box[0], (lx * a.inv_box[0] + MAGIC) - MAGIC, lx);
+            ly = fma(-a.box[1], (ly * a.inv_box[1] + MAGIC) - MAGIC, ly);
+            lz = fma(-a.box[2], (lz * a.inv_box[2] + MAGIC) - MAGIC, lz);
+            C[o + k] = half_record(lx, ly, lz);
+            if (s == 13) ref[k] = p[u];
+          }
         }
       }
     }
