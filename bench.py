@@ -53,8 +53,8 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_dense<false> / k_pair_staged<false> launch (per launch, like `achieved`) and the
 # `ncu --set full` capture it was read from; refreshed whenever the kernel changes (the value is a property of that
 # capture, not of this run: `traffic_source` says which)
-NCU_TRAFFIC = {("C4", "k_pair_dense"): (9.21153e8 + 2.2901e7, "profiles/r2b_summary.md (prof_r2b_c4, ncu --set full)"),
-               ("C3", "k_pair_dense"): (2.30306e8 + 6.811e6, "profiles/r2b_summary.md (prof_r2b_c3, ncu --set full)"),
+NCU_TRAFFIC = {("C4", "k_pair_dense"): (9.21201e8 + 2.3565e7, "profiles/r2b_summary.md (prof_r2b_c4, ncu --set full)"),
+               ("C3", "k_pair_dense"): (2.30314e8 + 7.261e6, "profiles/r2b_summary.md (prof_r2b_c3, ncu --set full)"),
                ("C4", "k_pair_staged"): (1.363542e9 + 2.4354e7, "profiles/r2_summary.md (prof_r2_hot, ncu --set full)"),
                ("C3", "k_pair_staged"): (3.409152e8 + 7.760e6, "profiles/r2_summary.md (prof_r2_c3, ncu --set full)")}
 
