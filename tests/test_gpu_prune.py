@@ -68,3 +68,26 @@ def test_prune_skin_at_or_above_the_list_skin_falls_back():
     assert s.pair_prune_stats()["active"] == 0 and s.counters()["staged"] == 1
     s.step(3)
     s.check()
+
+
+def test_pair_phase_is_timed_launch_by_launch():
+    """qhp_profile_read_pair: one interval per step for each of k_prune_check, k_prune, k_pair_dense inside the pair
+    phase of qhp_profile_read; the three together do not exceed the phase."""
+    top = W.water_box(5832)
+    s, _, x0, p0 = make_pair(top, 4, 2, 0.25, "pile")
+    s.set_state(to_dev(x0), to_dev(p0), 0)
+    s.step(3)
+    s.profile(True)
+    s.step(6)
+    ph, pp = s.profile_read(), s.profile_read_pair()
+    s.profile(False)
+    assert ph["pair"]["n"] == 6
+    assert all(pp[k]["n"] == 6 and pp[k]["ms"] > 0 for k in ("k_prune_check", "k_prune", "k_pair_dense"))
+    assert sum(v["ms"] for v in pp.values()) <= ph["pair"]["ms"] * 1.001
+    assert pp["k_pair_dense"]["ms"] > pp["k_prune_check"]["ms"]
+    u = make_pair(top, 4, 2, 0.25, "pile")[0]
+    u.set_pair_prune(0.0)
+    u.set_state(to_dev(x0), to_dev(p0), 0)
+    u.profile(True)
+    u.step(2)
+    assert all(v["n"] == 0 for v in u.profile_read_pair().values()) and u.profile_read()["pair"]["n"] == 2
