@@ -148,10 +148,13 @@ __global__ void __launch_bounds__(STG_THREADS, 1) k_pair_staged(const StagedArgs
     off[tid + 1] = a.cell_start[c2 + 1] - a.cell_start[c2];
   }
   __syncthreads();
-  if (tid == 0) {
-    next_atom = 0;
-    off[0] = 0;
-    for (int s = 0; s < 27; ++s) off[s + 1] += off[s];
+  if (tid < 32) {                             // prefix over the 27 stencil cells by one warp
+    if (tid == 0) next_atom = 0;
+    int v = tid < 27 ? off[tid + 1] : 0;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, v, o); if (tid >= o) v += u; }
+    if (tid < 27) off[tid + 1] = v;
+    if (tid == 0) off[0] = 0;
   }
   __syncthreads();
   const int total = off[27];
@@ -376,9 +379,12 @@ __global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const Stag
     off[tid + 1] = a.cell_start[c2 + 1] - a.cell_start[c2];
   }
   __syncthreads();
-  if (tid == 0) {
-    off[0] = 0;
-    for (int s = 0; s < 27; ++s) off[s + 1] += off[s];
+  if (tid < 32) {                             // prefix over the 27 stencil cells by one warp
+    int v = tid < 27 ? off[tid + 1] : 0;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, v, o); if (tid >= o) v += u; }
+    if (tid < 27) off[tid + 1] = v;
+    if (tid == 0) off[0] = 0;
   }
   __syncthreads();
   const int total = off[27];
@@ -626,9 +632,12 @@ __global__ void __launch_bounds__(PRUNE_THREADS, 2) k_prune(const PruneArgs a) {
     off[tid + 1] = a.cell_start[c2 + 1] - a.cell_start[c2];
   }
   __syncthreads();
-  if (tid == 0) {
-    off[0] = 0;
-    for (int s = 0; s < 27; ++s) off[s + 1] += off[s];
+  if (tid < 32) {                             // prefix over the 27 stencil cells by one warp
+    int v = tid < 27 ? off[tid + 1] : 0;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, v, o); if (tid >= o) v += u; }
+    if (tid < 27) off[tid + 1] = v;
+    if (tid == 0) off[0] = 0;
   }
   __syncthreads();
   const int total = off[27];
