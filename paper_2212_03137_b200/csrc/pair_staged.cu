@@ -443,17 +443,23 @@ __global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const Stag
   const uint32_t sXY = (uint32_t)__cvta_generic_to_shared(XY), sZ = (uint32_t)__cvta_generic_to_shared(Z),
                  sTab = (uint32_t)__cvta_generic_to_shared(tab), sQt = (uint32_t)__cvta_generic_to_shared(qtab);
   unsigned long long hits = 0;
+  // per-row pointers advance by fixed strides (kept in registers: the compiler otherwise rebuilds each address from
+  // the kernel parameters in every row, ~60 instructions of 64-bit arithmetic)
+  const uint16_t *rowp = table + (long long)(slot0 + ii) * a.stride + 8 * lane;
+  const int32_t *cntp = counts + slot0 + ii;
+  const double *typp = reinterpret_cast<const double *>(pos + slot0 + ii) + 3;
+  const long long row_step = (long long)istep * a.stride;
+  asm volatile("" : "+l"(rowp), "+l"(cntp), "+l"(typp));
 
-  for (; ii < nh; ii += istep) {
+  for (; ii < nh; ii += istep, rowp += row_step, cntp += istep, typp += 4 * istep) {
     const uint32_t ei = (uint32_t)(h0 + ii);
     const long long slot = slot0 + ii;
     const int n = n_nx, ti = ti_nx;
-    const uint16_t *rowp = table + slot * a.stride;
     const int nblk = max(1, (n + STG_BLOCK - 1) / STG_BLOCK);
     const bool more = ii + istep < nh;
     if (more) {
-      n_nx = counts[slot + istep];
-      ti_nx = (int)__double_as_longlong(pos[slot + istep].w);
+      n_nx = cntp[istep];
+      ti_nx = (int)__double_as_longlong(typp[4 * istep]);
     }
     const double2 xyi = lds_d2(sXY + ei * 16);
     const double zi = lds_d(sZ + ei * 8);
@@ -498,8 +504,8 @@ __global__ void __launch_bounds__(DNS_THREADS, DNS_CTAS) k_pair_dense(const Stag
 
     for (int m = 0; m < nblk; ++m) {
       uint4 nxt = cur;
-      if (m + 1 < nblk) nxt = *reinterpret_cast<const uint4 *>(rowp + STG_BLOCK * (m + 1) + 8 * lane);
-      else if (more) nxt = *reinterpret_cast<const uint4 *>(rowp + (long long)istep * a.stride + 8 * lane);   // first block of the next row
+      if (m + 1 < nblk) nxt = *reinterpret_cast<const uint4 *>(rowp + STG_BLOCK * (m + 1));
+      else if (more) nxt = *reinterpret_cast<const uint4 *>(rowp + row_step);   // first block of the next row
       const uint32_t w[4] = {cur.x, cur.y, cur.z, cur.w};
       const int nst = min(8, (n - STG_BLOCK * m + 31) >> 5);
       fetch(w[0] & 0xffffu);
