@@ -42,6 +42,7 @@ struct IntArgs {
   int do_step;
   double w_fast, w_slow;   // kick weights (dt/2 * 418.4 units) of V_f and V_s in this pass
   long long step;
+  const long long *step_base;   // NULL, or device: added to `step` for the Philox counters (CUDA-graph replays, qhp_api.cu)
   unsigned long long seed;
   double hdt;
   // adQTB (P = 1)
@@ -314,7 +315,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
     for (int w = t; w < na * P; w += blockDim.x) {
       const int al = w % na, n = w / na;
       double z[3];
-      qhp_normals3(a.seed, (uint32_t)(tl.a0 + al), (uint32_t)n, QHP_TAG_PILE, (uint64_t)a.step, z);
+      qhp_normals3(a.seed, (uint32_t)(tl.a0 + al), (uint32_t)n, QHP_TAG_PILE, (uint64_t)(a.step + (a.step_base ? *a.step_base : 0LL)), z);
       ft[n * TD + 3 * al] = z[0]; ft[n * TD + 3 * al + 1] = z[1]; ft[n * TD + 3 * al + 2] = z[2];
     }
     __syncthreads();
@@ -484,7 +485,7 @@ __global__ void __launch_bounds__(128) k_integrate_mol1(const IntArgs a, int n_m
       const long long slot = slot_[al];
       const double *cf = a.coef + ty * QHP_NCOEF;
       double z[3] = {0.0, 0.0, 0.0};
-      if (THERMO == 1 && a.do_step) qhp_normals3(a.seed, (uint32_t)atom, 0u, QHP_TAG_PILE, (uint64_t)a.step, z);
+      if (THERMO == 1 && a.do_step) qhp_normals3(a.seed, (uint32_t)atom, 0u, QHP_TAG_PILE, (uint64_t)(a.step + (a.step_base ? *a.step_base : 0LL)), z);
       double dsum = 0.0;
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
@@ -730,6 +731,7 @@ int qhp_nm_integrate(qhp_system *s, bool kick_prev, bool do_step, int64_t step) 
   const double hA = 0.5 * s->dt * QHP_ACC;
   const int na = s->n_alt;
   a.do_step = do_step; a.step = step;
+  a.step_base = s->graph_capturing ? s->graph_step_base : nullptr;
   a.w_fast = (kick_prev ? hA : 0.0) + (do_step ? hA : 0.0);
   a.w_slow = (kick_prev && step % na == 0 ? na * hA : 0.0) + (do_step && step % na == 0 ? na * hA : 0.0);
   if (do_step) s->flag_idx = (int)(step & 1);

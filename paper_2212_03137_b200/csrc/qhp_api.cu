@@ -11,6 +11,7 @@
 int qhp_pair_geometry(const qhp_system *s, int *NB_out, int *L_out, unsigned *gx, unsigned *gy);
 
 static std::string g_create_err;
+static void graph_drop(qhp_system *s);   // the CUDA graph of qhp_step bakes kernel arguments: dropped whenever they may change
 
 static bool supported_P(int P) {
   static const int ok[] = {1, 2, 3, 4, 5, 6, 8, 12, 16, 24, 32};
@@ -289,6 +290,9 @@ extern "C" int qhp_destroy(qhp_system *s) {
                   s->spec_cta, s->spec_part, s->Cvv, s->CvF, s->stage_x, s->stage_p, s->ratio_tau, s->ratio_avv, s->ratio_avf, s->kappa};
   for (void *p : ptrs) if (p) cudaFree(p);
   qhp_pair_dense_free(s);
+  graph_drop(s);
+  if (s->graph_step_base) cudaFree(s->graph_step_base);
+  if (s->graph_stream) cudaStreamDestroy(s->graph_stream);
   if (s->flags_host) cudaFreeHost(s->flags_host);
   if (s->flags_ev) cudaEventDestroy(s->flags_ev);
   delete s;
@@ -318,6 +322,7 @@ extern "C" int qhp_set_state(qhp_system *s, const double *x_beads, const double 
   if (!s || !x_beads || !p_beads || step0 < 0) { if (s) s->err = "null state pointer or negative step"; return QHP_EINVAL; }
   if (step0 % s->n_alt != 0) { s->err = "step0 must be a multiple of n_alt"; return QHP_ESTATE; }
   if (s->th.kind == QHP_THERMO_ADQTB && step0 % s->n_seg != 0) { s->err = "adQTB state can only be set at a segment boundary"; return QHP_ESTATE; }
+  graph_drop(s);
   int rc = qhp_nm_to_modes(s, x_beads, p_beads);
   if (rc) return rc;
   QHP_CUDA_OK(s, cudaMemsetAsync(s->d2max, 0, sizeof(unsigned long long) * 2, s->stream));
@@ -435,6 +440,61 @@ static void flags_enqueue(qhp_system *s) {
   s->flags_pending = true;
 }
 
+#define QHP_GRAPH_STEPS 32
+static int one_step(qhp_system *s);
+
+__global__ void k_set_i64(long long *p, long long v) { *p = v; }
+
+static bool graph_eligible(const qhp_system *s) {
+  return !s->graph_off && s->N <= 32768 && s->th.kind != QHP_THERMO_ADQTB && s->n_alt == 1 && s->shard_world <= 1 && !s->prof;
+}
+static void graph_drop(qhp_system *s) {
+  if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
+}
+// capture QHP_GRAPH_STEPS steps from the current (even, steady-state) step, instantiate, and run them once
+static int graph_capture(qhp_system *s) {
+  if (!s->graph_step_base) {
+    if (cudaMalloc(&s->graph_step_base, sizeof(long long)) != cudaSuccess) { cudaGetLastError(); s->graph_off = true; return QHP_OK; }
+  }
+  // the caller's stream may be the legacy default stream, which cannot be captured: the steps are recorded on a
+  // stream of the library's own (nothing runs on it) and the instantiated graph is launched on the caller's stream
+  if (!s->graph_stream && cudaStreamCreateWithFlags(&s->graph_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); s->graph_off = true; return QHP_OK; }
+  k_set_i64<<<1, 1, 0, s->stream>>>(s->graph_step_base, 0LL);
+  const int64_t step0 = s->step, launches0 = s->n_launch;
+  const int flag0 = s->flag_idx;
+  cudaStream_t user = s->stream;
+  if (cudaStreamBeginCapture(s->graph_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); s->graph_off = true; return QHP_OK; }
+  s->stream = s->graph_stream;
+  s->graph_capturing = true;
+  int rc = QHP_OK;
+  for (int k = 0; k < QHP_GRAPH_STEPS && !rc; ++k) rc = one_step(s);
+  s->graph_capturing = false;
+  s->stream = user;
+  cudaGraph_t g = nullptr;
+  const cudaError_t e = cudaStreamEndCapture(s->graph_stream, &g);
+  if (rc || e != cudaSuccess || !g) {                    // e.g. a launch kind that cannot be captured: plain launches from now on
+    cudaGetLastError();
+    if (g) cudaGraphDestroy(g);
+    s->graph_off = true;
+    s->step = step0; s->n_launch = launches0; s->flag_idx = flag0; s->err.clear();
+    return QHP_OK;
+  }
+  const cudaError_t ei = cudaGraphInstantiate(&s->graph_exec, g, 0);
+  cudaGraphDestroy(g);
+  if (ei != cudaSuccess) { cudaGetLastError(); s->graph_exec = nullptr; s->graph_off = true; s->step = step0; s->n_launch = launches0; s->flag_idx = flag0; return QHP_OK; }
+  s->graph_step0 = step0;
+  s->graph_launches = s->n_launch - launches0;
+  QHP_CUDA_OK(s, cudaGraphLaunch(s->graph_exec, s->stream));   // the host state already stands behind these steps
+  return QHP_OK;
+}
+static int graph_replay(qhp_system *s) {
+  k_set_i64<<<1, 1, 0, s->stream>>>(s->graph_step_base, (long long)(s->step - s->graph_step0));
+  QHP_CUDA_OK(s, cudaGraphLaunch(s->graph_exec, s->stream));
+  s->step += QHP_GRAPH_STEPS;                            // even number of steps: flag_idx and pending_kick are unchanged
+  s->n_launch += s->graph_launches;
+  return QHP_OK;
+}
+
 extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
   if (!s || nsteps < 0) return QHP_EINVAL;
   if (!s->have_state) { s->err = "qhp_step before qhp_set_state"; return QHP_ESTATE; }
@@ -444,12 +504,47 @@ extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
     const int rcf = flags_poll(s);
     if (rcf) return rcf;
   }
-  for (int64_t k = 0; k < nsteps; ++k) {
+  int64_t k = 0;
+  // Small systems are launch-bound (C0: 648 atoms, 3 launches of a few microseconds each per step): steps are replayed
+  // QHP_GRAPH_STEPS at a time from a CUDA graph captured once.  Everything that varies from step to step is decided
+  // on the device (rebuild flag, its parity: the graph has an even number of steps) except the Philox step index,
+  // which the kernels take as the baked index + a device-side base set before each replay.
+  if (graph_eligible(s) && nsteps >= 2 * QHP_GRAPH_STEPS) {
+    while (k < nsteps && (!s->pending_kick || (s->step & 1))) {   // steady state, even step index
+      const int rc1 = one_step(s);
+      if (rc1) return rc1;
+      ++k;
+    }
+    if (!s->graph_exec && !s->graph_off) {
+      const int rcg = graph_capture(s);                  // also runs the captured steps once
+      if (rcg) return rcg;
+      if (s->graph_exec) k += QHP_GRAPH_STEPS;
+    }
+    while (s->graph_exec && nsteps - k >= QHP_GRAPH_STEPS) {
+      const int rcf = flags_poll(s);
+      if (rcf) return rcf;
+      const int rcg = graph_replay(s);
+      if (rcg) return rcg;
+      k += QHP_GRAPH_STEPS;
+      flags_enqueue(s);
+    }
+  }
+  for (; k < nsteps; ++k) {
     if ((k & 255) == 255) {
       const int rcf = flags_poll(s);
       if (rcf) return rcf;
       flags_enqueue(s);
     }
+    const int rc1 = one_step(s);
+    if (rc1) return rc1;
+  }
+  if (nsteps > 0) flags_enqueue(s);
+  return QHP_OK;
+}
+
+static int one_step(qhp_system *s) {
+  const bool adqtb = s->th.kind == QHP_THERMO_ADQTB;
+  {
     const int64_t st = s->step;
     int rc;
     if (adqtb && st % s->n_seg == 0 && s->fc_segment != st / s->n_seg) {
@@ -482,7 +577,6 @@ extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
       if (rc) return rc;
     }
   }
-  if (nsteps > 0) flags_enqueue(s);
   return QHP_OK;
 }
 
@@ -494,6 +588,7 @@ extern "C" int qhp_set_respa(qhp_system *s, int n_alt) {
   // the closing half kicks of the last step are still pending and carry the weights of the OLD n_alt
   // (w_slow = n_alt dt/2, qhp_nm_integrate): apply them before the weights change
   if (s->have_state) { const int rc = flush_kick(s); if (rc) return rc; }
+  graph_drop(s);
   s->n_alt = n_alt;
   return QHP_OK;
 }
@@ -530,6 +625,7 @@ extern "C" int qhp_pair_prune_stats(qhp_system *s, int64_t *out_host) {
 extern "C" int qhp_set_a_block(qhp_system *s, int kind) {
   if (!s) return QHP_EINVAL;
   if (kind != QHP_ABLOCK_EXACT && kind != QHP_ABLOCK_CAYLEY) { s->err = "unknown A block"; return QHP_EINVAL; }
+  graph_drop(s);
   s->a_block = kind;
   return QHP_OK;
 }

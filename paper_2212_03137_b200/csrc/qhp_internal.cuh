@@ -153,6 +153,14 @@ struct qhp_system {
   cudaEvent_t flags_ev = nullptr;
   bool flags_pending = false;
 
+  // ---- CUDA graph of QHP_GRAPH_STEPS steps for small, launch-bound systems (qhp_step) ----
+  cudaGraphExec_t graph_exec = nullptr;
+  cudaStream_t graph_stream = nullptr;     // capture stream (the caller's may be the legacy default stream)
+  long long *graph_step_base = nullptr;    // device: offset added to the step indices baked into the graph (Philox counters)
+  int64_t graph_step0 = 0;                 // step index the graph was captured at
+  int64_t graph_launches = 0;              // kernel launches inside one replay
+  bool graph_capturing = false, graph_off = false;
+
   // ---- per-phase profiling (qhp_profile) ----
   bool prof = false;
   std::vector<cudaEvent_t> prof_ev;      // flat list of (begin, end) pairs
