@@ -107,10 +107,11 @@ int qhp_get_state_host(qhp_system *sys, double *x_beads, double *p_beads, int64_
  * ring-polymer A blocks, PILE/TRPMD O block gamma_n = max(gamma0, omega_n) (l.146), or, for
  * adQTB, classical BAOAB whose O block carries the coloured force (Eq. 12-14, l.199), with the
  * segment generation (l.203-209) and gamma_z(omega) adaptation (Eq. 21-23, l.248) at segment
- * boundaries.  Enqueues its work and returns; never waits for the device.  Small systems (n_atoms <= 32768, PILE or
- * no thermostat, n_alt = 1, no qhp_set_comm, profiling off) are launch-bound: calls of >= 64 steps replay 32 steps at
- * a time from a CUDA graph captured once per state (same kernels and arguments, the Philox step index taken from
- * device memory): the trajectory is bit-identical to plain launches, qhp_counters counts the replayed kernels.  The sticky error flags of the device
+ * boundaries.  Enqueues its work and returns; never waits for the device.  Small systems (n_atoms <= 32768, n_alt = 1,
+ * no qhp_set_comm, profiling off) are launch-bound: longer calls replay 32 steps at a time from a CUDA graph captured
+ * once per state (same kernels and arguments; the Philox step index and the adQTB segment position are taken from
+ * device memory; an adQTB replay never crosses a segment boundary): the trajectory is bit-identical to plain
+ * launches, qhp_counters counts the replayed kernels.  The sticky error flags of the device
  * (list-row overflow, staged neighbourhood outgrew shared memory, skin smaller than the bead spread: qhp_counters
  * [5]) are copied to pinned memory behind the work of every call and every 256 steps of a long one, and looked at
  * without waiting when qhp_step is entered again or reaches the next 256-step mark: QHP_ESTATE then (text in

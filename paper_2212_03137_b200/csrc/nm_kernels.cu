@@ -57,6 +57,12 @@ struct IntArgs {
   double kT;
 };
 
+// step index within the noise segment; under a CUDA-graph replay the baked index is shifted by the device-side base
+// (replays never cross a segment boundary: qhp_api.cu)
+__device__ __forceinline__ int seg_step(const IntArgs &a) {
+  return a.step_base ? (int)((a.n_loc + *a.step_base) % a.n_seg) : a.n_loc;
+}
+
 // ---------------------------------------------------------------------------------------------
 // V_f of one (molecule, bead): harmonic bonds, harmonic angles, optional tether (BASELINE.json
 // configs[0]; oracle O3).  x, f point at the bead's row of the shared tiles; a0 = first atom of
@@ -284,7 +290,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
 #pragma unroll
       for (int k = 0; k < PF; ++k) pl[k] = a.Pm[k * a.ND + dof];
     }
-    if (THERMO == 2 && a.do_step) fc_early = a.Fc[qhp_seg_addr(a.seg_slot[atom], a.n_seg, a.n_loc) + c];
+    if (THERMO == 2 && a.do_step) fc_early = a.Fc[qhp_seg_addr(a.seg_slot[atom], a.n_seg, seg_step(a)) + c];
   }
 
   // ---- phase 1: Q -> bead positions (shared tile), V_f per (molecule, bead) -------------------------
@@ -349,7 +355,7 @@ __global__ void __launch_bounds__(P >= 24 ? 160 : 288, P >= 24 ? 3 : 1) k_integr
           p = mc.c1[n] * p + (mc.c2k[n] * sqm) * ft[n * TD + t];
         } else if (THERMO == 2) {
           // classical BAOAB carrying the coloured force (Eq. 12, l.199; readings G14, G16)
-          const long long k = qhp_seg_addr(a.seg_slot[atom], a.n_seg, a.n_loc) + c;
+          const long long k = qhp_seg_addr(a.seg_slot[atom], a.n_seg, seg_step(a)) + c;
           const double pn = a.qa * p + a.qbA * fc_early;
           a.vseg[k] = (p + pn) / (2.0 * m);
           p = pn;
@@ -461,7 +467,7 @@ __global__ void __launch_bounds__(128) k_integrate_mol1(const IntArgs a, int n_m
       const int atom = s0 + al;
       ty_[al] = __ldg(a.type + atom);
       slot_[al] = __ldg(a.rank + atom);
-      segb_[al] = THERMO == 2 ? qhp_seg_addr(__ldg(a.seg_slot + atom), a.n_seg, a.n_loc) : 0;
+      segb_[al] = THERMO == 2 ? qhp_seg_addr(__ldg(a.seg_slot + atom), a.n_seg, seg_step(a)) : 0;
     }
 #pragma unroll
     for (int al = 0; al < 4; ++al) {

@@ -446,7 +446,14 @@ static int one_step(qhp_system *s);
 __global__ void k_set_i64(long long *p, long long v) { *p = v; }
 
 static bool graph_eligible(const qhp_system *s) {
-  return !s->graph_off && s->N <= 32768 && s->th.kind != QHP_THERMO_ADQTB && s->n_alt == 1 && s->shard_world <= 1 && !s->prof;
+  return !s->graph_off && s->N <= 32768 && s->n_alt == 1 && s->shard_world <= 1 && !s->prof;   // larger boxes are GPU-bound: measured, no gain
+}
+// adQTB: a replay must stay inside one noise segment whose coloured force exists (generation and adaptation are host-
+// driven events at the segment boundaries); other thermostats: always
+static bool graph_window_ok(const qhp_system *s) {
+  if (s->th.kind != QHP_THERMO_ADQTB) return true;
+  const int64_t seg = s->step / s->n_seg;
+  return s->fc_segment == seg && (s->step + QHP_GRAPH_STEPS - 1) / s->n_seg == seg && (s->step + QHP_GRAPH_STEPS) % s->n_seg != 0;
 }
 static void graph_drop(qhp_system *s) {
   if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
@@ -510,21 +517,23 @@ extern "C" int qhp_step(qhp_system *s, int64_t nsteps) {
   // on the device (rebuild flag, its parity: the graph has an even number of steps) except the Philox step index,
   // which the kernels take as the baked index + a device-side base set before each replay.
   if (graph_eligible(s) && nsteps >= 2 * QHP_GRAPH_STEPS) {
-    while (k < nsteps && (!s->pending_kick || (s->step & 1))) {   // steady state, even step index
-      const int rc1 = one_step(s);
-      if (rc1) return rc1;
-      ++k;
-    }
-    if (!s->graph_exec && !s->graph_off) {
-      const int rcg = graph_capture(s);                  // also runs the captured steps once
-      if (rcg) return rcg;
-      if (s->graph_exec) k += QHP_GRAPH_STEPS;
-    }
-    while (s->graph_exec && nsteps - k >= QHP_GRAPH_STEPS) {
+    while (nsteps - k >= QHP_GRAPH_STEPS + 2 && !s->graph_off) {
+      if (!s->pending_kick || (s->step & 1) || !graph_window_ok(s)) {   // not in the steady state, odd step index, or an
+        const int rc1 = one_step(s);                                     // adQTB segment boundary ahead: plain steps
+        if (rc1) return rc1;
+        ++k;
+        continue;
+      }
       const int rcf = flags_poll(s);
       if (rcf) return rcf;
-      const int rcg = graph_replay(s);
-      if (rcg) return rcg;
+      if (!s->graph_exec) {
+        const int rcg = graph_capture(s);                // also runs the captured steps once
+        if (rcg) return rcg;
+        if (!s->graph_exec) break;
+      } else {
+        const int rcg = graph_replay(s);
+        if (rcg) return rcg;
+      }
       k += QHP_GRAPH_STEPS;
       flags_enqueue(s);
     }
