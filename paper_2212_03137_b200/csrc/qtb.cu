@@ -160,6 +160,13 @@ __device__ __noinline__ void fft_smem(double2 *buf, int n, int sign, const doubl
   else fft_smem_sg<1>(buf, n, tw, tw_n, t);
 }
 
+// The segment kernels only transform forward (the inverse is conj(forward(conj(.)))): their own non-inlined body.  With
+// both directions in one function (fft_smem) ptxas spilled 6.9 KB per call in the context of k_qtb_noise, with the
+// forward direction alone 1.1 KB: noise generation 41.8 -> 30.5 ms per C3 segment.
+__device__ __noinline__ void fft_fwd(double2 *buf, int n, const double2 *__restrict__ tw, int tw_n, int t) {
+  fft_smem_sg<-1>(buf, n, tw, tw_n, t);
+}
+
 __global__ void k_twiddle(double2 *tw, int n) {
   const int m = blockIdx.x * blockDim.x + threadIdx.x;
   if (m >= n) return;
@@ -285,7 +292,7 @@ __global__ void __launch_bounds__(512, 1) k_qtb_noise(int n_seg, unsigned long l
   for (int pass = 0; pass < 3; ++pass) {
     qtb_fill_noise(nbuf, zb, nf, nw, n_seg, pass, pass < 2 ? at[pass] : -1, seed, seg, t, blockDim.x);
     __syncthreads();
-    fft_smem(nbuf, nf, -1, tw, nf, t);
+    fft_fwd(nbuf, nf, tw, nf, t);
     // inverse transform = conj(forward(conj(.))): one transform direction in this kernel
 #pragma unroll 8
     for (int q = t; q < nf; q += blockDim.x) {
@@ -293,7 +300,7 @@ __global__ void __launch_bounds__(512, 1) k_qtb_noise(int n_seg, unsigned long l
       nbuf[FPAD(q)] = make_double2(p.x, -p.y);
     }
     __syncthreads();
-    fft_smem(nbuf, nf, -1, tw, nf, t);
+    fft_fwd(nbuf, nf, tw, nf, t);
     // every pass writes its own pieces of the pair's 48-byte half rows (x0 y0 z0 x1 y1 z1); L2 merges them
     for (int n = t; n < n_seg; n += blockDim.x) {
       double2 y = nbuf[FPAD(n + 2 * n_seg)];
@@ -315,7 +322,7 @@ __global__ void __launch_bounds__(512, 1) k_qtb_noise(int n_seg, unsigned long l
 // shared array per CTA, the thread groups adding in a fixed order; per-CTA sums -> fixed-order reduction.
 // ---------------------------------------------------------------------------------------------
 template <int DPR>
-__global__ void __launch_bounds__(512, 1) k_qtb_spectra(int n_seg, const int32_t *__restrict__ cta_tab,
+__global__ void __launch_bounds__(DPR == 3 ? 384 : 256, 1) k_qtb_spectra(int n_seg, const int32_t *__restrict__ cta_tab,
                                                         const double *__restrict__ vseg, const double *__restrict__ Fc,
                                                         const double2 *__restrict__ tw, int tw_n, double *part) {
   extern __shared__ double2 sbuf_all[];
@@ -348,7 +355,7 @@ __global__ void __launch_bounds__(512, 1) k_qtb_spectra(int n_seg, const int32_t
     __syncthreads();
     if (q + 1 < rounds) issue(q + 1, nxt);
     double2 *sbuf = cur + (size_t)c * bl;
-    fft_smem(sbuf, nk, -1, tw, tw_n, t);
+    fft_fwd(sbuf, nk, tw, tw_n, t);
     for (int cc = 0; cc < DPR; ++cc) {                   // the thread groups add in a fixed order
       if (c == cc)
         for (int j = t; j < nf; j += gsz) {
