@@ -160,6 +160,101 @@ __device__ __noinline__ void fft_smem(double2 *buf, int n, int sign, const doubl
   else fft_smem_sg<1>(buf, n, tw, tw_n, t);
 }
 
+// ---- 8 elements per thread (n / 8 threads per transform): half the registers of the 16-element passes, twice the warps.
+// 8-point DFT, decimation in time: X_k = E_k + w8^k O_k, X_{k+4} = E_k - w8^k O_k with E, O the 4-point DFTs of the even
+// and odd inputs; in place, natural order.
+template <int SG>
+__device__ __forceinline__ void dft8(double2 (&v)[8]) {
+  dft4<SG>(v[0], v[2], v[4], v[6]);
+  dft4<SG>(v[1], v[3], v[5], v[7]);
+  const double r2 = 0.70710678118654752440, sg = (SG < 0) ? -1.0 : 1.0;
+  const double2 o0 = v[1];
+  const double2 o1 = cmul(v[3], make_double2(r2, sg * r2));
+  const double2 o2 = make_double2(-sg * v[5].y, sg * v[5].x);          // * (SG i)
+  const double2 o3 = cmul(v[7], make_double2(-r2, sg * r2));
+  const double2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6];
+  v[0] = make_double2(e0.x + o0.x, e0.y + o0.y); v[4] = make_double2(e0.x - o0.x, e0.y - o0.y);
+  v[1] = make_double2(e1.x + o1.x, e1.y + o1.y); v[5] = make_double2(e1.x - o1.x, e1.y - o1.y);
+  v[2] = make_double2(e2.x + o2.x, e2.y + o2.y); v[6] = make_double2(e2.x - o2.x, e2.y - o2.y);
+  v[3] = make_double2(e3.x + o3.x, e3.y + o3.y); v[7] = make_double2(e3.x - o3.x, e3.y - o3.y);
+}
+
+// one Stockham pass of radix R (8, 4 or 2) at stride Ns, 8 elements per thread (t < n / 8)
+template <int R, int SG>
+__device__ __forceinline__ void fft_pass8(double2 *buf, int n, int Ns, const double2 *__restrict__ tw, int tw_n, int t,
+                                          const double2 wpre = make_double2(0.0, 0.0), bool have_w = false) {
+  constexpr int G = 8 / R;
+  const int nth = n >> 3, nb = n / R;
+  const bool on = t < nth;
+  double2 v[8];
+  int j0[G];
+  if (on) {
+#pragma unroll
+    for (int q = 0; q < G; ++q) {
+      const int j = t + q * nth, k = j & (Ns - 1);
+#pragma unroll
+      for (int u = 0; u < R; ++u) v[q * R + u] = buf[FPAD(j + u * nb)];
+      if (k) {
+        const double2 w1 = have_w ? wpre : twiddle(tw, tw_n, k, Ns * R, SG);
+        double2 w = w1;
+#pragma unroll
+        for (int u = 1; u < R; ++u) {
+          v[q * R + u] = cmul(v[q * R + u], w);
+          if (u + 1 < R) w = cmul(w, w1);
+        }
+      }
+      j0[q] = (j - k) * R + k;
+    }
+  }
+  __syncthreads();
+  if (on) {
+    if (R == 8) {
+      dft8<SG>(v);
+#pragma unroll
+      for (int u = 0; u < 8; ++u) buf[FPAD(j0[0] + u * Ns)] = v[u];
+    } else if (R == 4) {
+#pragma unroll
+      for (int q = 0; q < G; ++q) {
+        dft4<SG>(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) buf[FPAD(j0[q] + u * Ns)] = v[4 * q + u];
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < G; ++q) {
+        const double2 x0 = v[2 * q], x1 = v[2 * q + 1];
+        buf[FPAD(j0[q])] = make_double2(x0.x + x1.x, x0.y + x1.y);
+        buf[FPAD(j0[q] + Ns)] = make_double2(x0.x - x1.x, x0.y - x1.y);
+      }
+    }
+  }
+  __syncthreads();
+}
+
+// forward transform of buf[0..n), n >= 8 a power of two, by n / 8 threads per transform (all threads of the CTA call):
+// n = r0 * 8^m: the factor r0 in {1, 2, 4} first, then m radix-8 passes whose table entries are requested up front
+__device__ __noinline__ void fft_fwd8(double2 *buf, int n, const double2 *__restrict__ tw, int tw_n, int t) {
+  int r0 = n, m8 = 0;
+  while (r0 >= 8 && (r0 & 7) == 0) { r0 >>= 3; ++m8; }
+  double2 w8[4] = {make_double2(1.0, 0.0), make_double2(1.0, 0.0), make_double2(1.0, 0.0), make_double2(1.0, 0.0)};
+  {
+    int Ns = r0;
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+      if (p < m8) {
+        const int k = t & (Ns - 1);
+        if (t < (n >> 3)) w8[p] = twiddle(tw, tw_n, k, Ns * 8, -1);
+        Ns <<= 3;
+      }
+  }
+  int Ns = 1;
+  if (r0 == 2) { fft_pass8<2, -1>(buf, n, 1, tw, tw_n, t); Ns = 2; }
+  else if (r0 == 4) { fft_pass8<4, -1>(buf, n, 1, tw, tw_n, t); Ns = 4; }
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+    if (p < m8) { fft_pass8<8, -1>(buf, n, Ns, tw, tw_n, t, w8[p], true); Ns <<= 3; }
+}
+
 // The segment kernels only transform forward (the inverse is conj(forward(conj(.)))): their own non-inlined body.  With
 // both directions in one function (fft_smem) ptxas spilled 6.9 KB per call in the context of k_qtb_noise, with the
 // forward direction alone 1.1 KB: noise generation 41.8 -> 30.5 ms per C3 segment.
@@ -322,7 +417,7 @@ __global__ void __launch_bounds__(512, 1) k_qtb_noise(int n_seg, unsigned long l
 // shared array per CTA, the thread groups adding in a fixed order; per-CTA sums -> fixed-order reduction.
 // ---------------------------------------------------------------------------------------------
 template <int DPR>
-__global__ void __launch_bounds__(DPR == 3 ? 384 : 256, 1) k_qtb_spectra(int n_seg, const int32_t *__restrict__ cta_tab,
+__global__ void __launch_bounds__(DPR == 3 ? 768 : 512, 1) k_qtb_spectra(int n_seg, const int32_t *__restrict__ cta_tab,
                                                         const double *__restrict__ vseg, const double *__restrict__ Fc,
                                                         const double2 *__restrict__ tw, int tw_n, double *part) {
   extern __shared__ double2 sbuf_all[];
@@ -355,7 +450,7 @@ __global__ void __launch_bounds__(DPR == 3 ? 384 : 256, 1) k_qtb_spectra(int n_s
     __syncthreads();
     if (q + 1 < rounds) issue(q + 1, nxt);
     double2 *sbuf = cur + (size_t)c * bl;
-    fft_fwd(sbuf, nk, tw, tw_n, t);
+    fft_fwd8(sbuf, nk, tw, tw_n, t);
     for (int cc = 0; cc < DPR; ++cc) {                   // the thread groups add in a fixed order
       if (c == cc)
         for (int j = t; j < nf; j += gsz) {
@@ -565,10 +660,10 @@ int qhp_qtb_adapt(qhp_system *s) {
   const size_t smem = sizeof(double2) * 2 * dpr * (nk + 1) + sizeof(double) * 2 * nf;      // two buffers
   if (dpr == 3) {
     QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_spectra<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_qtb_spectra<3><<<s->n_spec_cta, 3 * fft_threads(nk), smem, s->stream>>>(ns, s->spec_cta, s->vseg, s->Fc, (const double2 *)s->tw, 4 * ns, s->spec_part);
+    k_qtb_spectra<3><<<s->n_spec_cta, 3 * (nk / 8 < 32 ? 32 : nk / 8), smem, s->stream>>>(ns, s->spec_cta, s->vseg, s->Fc, (const double2 *)s->tw, 4 * ns, s->spec_part);
   } else {
     QHP_CUDA_OK(s, cudaFuncSetAttribute(k_qtb_spectra<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_qtb_spectra<1><<<s->n_spec_cta, fft_threads(nk), smem, s->stream>>>(ns, s->spec_cta, s->vseg, s->Fc, (const double2 *)s->tw, 4 * ns, s->spec_part);
+    k_qtb_spectra<1><<<s->n_spec_cta, (nk / 8 < 32 ? 32 : nk / 8), smem, s->stream>>>(ns, s->spec_cta, s->vseg, s->Fc, (const double2 *)s->tw, 4 * ns, s->spec_part);
   }
   QHP_LAUNCH_OK(s);
   k_qtb_reduce<<<(nt * nf + 127) / 128, 128, 0, s->stream>>>(nt, ns, s->n_spec_cta, s->spec_cta, s->spec_part,
